@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- template-segments/s of the matched-filter + chi^2 hot path on B200.
+
+Contract (driver): `python bench.py --gpus N --steps K --warmup W [--impl reference]` prints ONE JSON line.
+
+  step      = one pass of the whole hot path (a1-a5: template generation, correlate, p band inverse
+              FFTs, rho, chi^2, window maxima, trigger compaction + read-back) over the whole bank of
+              BASELINE.json:configs[2] (N = 2^20, 1024 templates, p = 16) against one segment.
+  value     = template-segments/s with segment, PSD and bank resident in HBM when the timed region starts.
+  e2e       = the same through the C ABI with HOST buffers: every step uploads the segment and the PSD
+              (gwmf_load_segment from pinned host memory), filters the bank and reads the triggers back.
+  roofline  = the dominant kernel's algorithmic HBM bytes / its device time (CUDA events recorded by the
+              library on its own stream around every launch, gwmf_filter_timed), against the measured
+              copy bandwidth in MEASURED_PEAKS.json.
+  cpu_baseline = the fp64 oracle as it stands, on the host cores, on a bounded sample of the workload.
+  N > 1     : one process per GPU; every rank filters the whole bank against its own segment (seed +
+              rank): independent units, no data-path collective, weak scaling.
+
+`--impl reference` times the oracle (the reference arm of this tier) on the same config and metric.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_0906_4175_b200 import inputs  # noqa: E402
+
+METRIC = "template-segments/sec at N=2^20, p=16 (SNR+chi^2)"
+UNIT = "template-segments/s"
+FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback, only if MEASURED_PEAKS.json is absent
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def shard_plan(world_size: int, rank: int, n_templates: int):
+    """Weak scaling: every rank owns `n_templates` template-segments (the whole bank against its own
+    segment, seed offset = rank).  Returns (segment_seed_offset, first_template, count)."""
+    assert 0 <= rank < world_size
+    return rank, 0, n_templates
+
+
+def reduce_max_ms(ms: float, dist=None, device=None) -> float:
+    """MAX over ranks of a duration (all ranks get the result)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ms
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_rate(w, s64, Sn, n_templates: int, threads: int):
+    """Template-segments/s of the oracle on `n_templates` templates of the workload (evenly spread over the bank)."""
+    import oracle
+    idx = np.linspace(0, len(w.masses) - 1, n_templates).astype(int)
+    sub = [w.masses[i] for i in idx]
+    t0 = time.perf_counter()
+    out = oracle.filter_bank(s64, Sn, sub, w.p, w.window, w.rho_thresh, n_threads=threads)
+    dt = time.perf_counter() - t0
+    assert np.all(out["status"] == 0)
+    return n_templates / dt, dt
+
+
+def base_line(args, w, value, ms_per_step, dtype):
+    return {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+        "config": {"workload": "BASELINE.json:configs[2]: N=2^20 (256 s at 4096 Hz), 1024 templates "
+                               "(total mass 2-34 Msun, grid uniform in eta and chirp mass), p=16, threshold 6, "
+                               "window 4096; Eq. 2 coloured Gaussian noise + 10 injections, seed 2 (+rank)",
+                   "n": w.n, "templates": len(w.masses), "p": w.p, "window": w.window,
+                   "rho_thresh": w.rho_thresh, "units_per_step": len(w.masses) * args.gpus},
+    }
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = inputs.workload(2)
+    s64 = inputs.segment(w).astype(np.float32).astype(np.float64)
+    Sn = w.psd
+    cores = min(host_cores(), 32)
+    per_step = cores                      # one template-segment per thread and step
+    for _ in range(args.warmup):
+        oracle_rate(w, s64, Sn, per_step, cores)
+    t_total = 0.0
+    for _ in range(args.steps):
+        _, dt = oracle_rate(w, s64, Sn, per_step, cores)
+        t_total += dt
+    value = per_step * args.steps / t_total
+    line = base_line(args, w, value, 1e3 * t_total / args.steps, "f64")
+    sample = f"{per_step} of the 1024 templates per step (evenly spread over the bank), full N=2^20 segment, p=16"
+    line["impl"] = "reference"
+    line["config"]["units_per_step"] = per_step
+    line["config"]["sample"] = sample
+    line["cpu_baseline"] = {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    line["e2e"] = {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    line["gpu_launches"] = 0
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_0906_4175_b200 import gwmf
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    w = inputs.workload(2)
+    seed_off, first, count = shard_plan(world, rank, len(w.masses))
+    w.seed += seed_off
+    s32 = inputs.segment(w).astype(np.float32)
+    Sn = w.psd
+    T = len(w.masses)
+
+    f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}")
+    f.make_bank(w.masses)
+    s_dev = torch.from_numpy(s32).to(dev)
+    sn_dev = torch.from_numpy(Sn).to(dev)
+    f.load_segment(s_dev, sn_dev)
+
+    def step_resident():
+        f.filter(first, count)
+        return f.triggers()
+
+    sampler = ClockSampler(local)
+    for _ in range(max(args.warmup, 3)):
+        trig = step_resident()
+    barrier()
+    sampler.start()
+    l0 = f.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(f.stream)
+    for _ in range(args.steps):
+        trig = step_resident()
+    e1.record(f.stream)
+    barrier()
+    launches = f.launch_count - l0
+    ms = reduce_max_ms(e0.elapsed_time(e1), dist if world > 1 else None, dev)
+    value = world * count * args.steps / (ms * 1e-3)
+
+    # per-kernel device times (events inside the library, on its stream)
+    reps = 3
+    k_ms = np.zeros(2)
+    k_launch = np.zeros(2)
+    for _ in range(reps):
+        (m1, m2), (n1_, n2_) = f.filter_timed(first, count)
+        k_ms += (m1, m2)
+        k_launch += (n1_, n2_)
+    batch_templates = count / (k_launch / reps)             # templates per launch
+    bytes_per_launch = batch_templates * w.p * w.n * 8.0    # pass 1 writes / pass 2 reads p*N complex fp32 per template
+    avg_ms = k_ms / k_launch
+    gbs = bytes_per_launch / (avg_ms * 1e-3) / 1e9
+    peak, peak_src = measured_peak()
+    dom = int(np.argmax(k_ms))
+    names = ["k_pass1 (template+correlate+FFT pass 1, writes p*N*8 B/template)",
+             "k_pass2 (FFT pass 2 + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"]
+
+    # end to end through the C ABI with host buffers
+    s_pin = torch.from_numpy(s32).pin_memory()
+    sn_pin = torch.from_numpy(Sn).pin_memory()
+
+    def step_e2e():
+        f.load_segment(s_pin, sn_pin)
+        f.filter(first, count)
+        return f.triggers()
+
+    for _ in range(3):
+        trig = step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record(f.stream)
+    for _ in range(args.steps):
+        trig = step_e2e()
+    g1.record(f.stream)
+    barrier()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    ms_e2e = reduce_max_ms(max(g0.elapsed_time(g1), wall_ms), dist if world > 1 else None, dev)
+    clocks = sampler.stop()
+    e2e_value = world * count * args.steps / (ms_e2e * 1e-3)
+
+    if rank == 0:
+        line = base_line(args, w, value, ms / args.steps, "f32")
+        line["config"]["l2"] = ("no flush: every launch streams a band intermediate of batch*p*N*8 B = 1 GiB, "
+                                "8x the 126 MB L2, so nothing survives from one launch to the next")
+        line["config"]["batch_templates_per_launch"] = float(batch_templates[0])
+        line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(s32.nbytes + Sn.nbytes),
+                       "d2h_bytes_per_step": int(12 + trig.nbytes), "ms_per_step": ms_e2e / args.steps}
+        line["gpu_launches"] = int(launches)
+        line["clocks"] = clocks
+        line["triggers_per_step"] = int(len(trig))
+        line["roofline"] = {
+            "bound": "hbm", "kernel": names[dom], "achieved": float(gbs[dom]), "peak": peak, "unit": "GB/s",
+            "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": TRAFFIC_BYTES.get(dom),
+            "bytes_per_launch": float(bytes_per_launch[dom]), "avg_launch_ms": float(avg_ms[dom]),
+            "kernels": {"k_pass1": {"avg_launch_ms": float(avg_ms[0]), "GB/s": float(gbs[0]), "frac": float(gbs[0] / peak),
+                                    "share_of_step": float(k_ms[0] / k_ms.sum())},
+                        "k_pass2": {"avg_launch_ms": float(avg_ms[1]), "GB/s": float(gbs[1]), "frac": float(gbs[1] / peak),
+                                    "share_of_step": float(k_ms[1] / k_ms.sum())}},
+            "path": {"bytes_per_unit": 16.0 * w.p * w.n, "achieved": 16.0 * w.p * w.n * value / world / 1e9,
+                     "frac": 16.0 * w.p * w.n * value / world / 1e9 / peak,
+                     "note": "whole step (both passes + epilogue) against the 16*p*N B/template two-pass model; "
+                             "frac vs nominal 8 TB/s = %.3f" % (16.0 * w.p * w.n * value / world / 8e12)},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            cores = min(host_cores(), 32)
+            nt = cores * (2 if cores <= 16 else 1)
+            rate, dt = oracle_rate(w, s32.astype(np.float64), Sn, nt, cores)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{nt} of the 1024 templates (evenly spread), full N=2^20 segment, "
+                                              f"p=16, {dt:.1f} s wall",
+                                    "context": "paper: 16x total speed-up, GeForce 8800 Ultra vs one 2.5 GHz Q9300 core "
+                                               "(PAPER.md:5) -- other hardware, context only"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of
+# each kernel (profiles/), index 0 = k_pass1, 1 = k_pass2; None until a capture exists.
+TRAFFIC_BYTES = {0: None, 1: None}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="gwmf", choices=["gwmf", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,146 @@
+/* gwmf.h -- C ABI of the B200 inspiral matched-filter + chi^2 hot path (arxiv/paper_0906_4175).
+ *
+ * What the library computes (citations are PAPER.md lines; readings are listed in DESIGN.md):
+ *   z(t)   = 4 int h~_c(f) s~*(f) / S_n(f) e^{2 pi i f t} df                  Eq. 1
+ *   rho(t) = |z(t)| / sigma,  sigma^2 = 4 int |h~_c|^2 / S_n df               Eq. 3-4
+ *   chi^2(t) = (p/sigma^2) sum_l |z_l(t) - z(t)/p|^2, z_l = Eq. 1 restricted to the l-th of p
+ *              frequency bands of equal expected SNR^2                       Eq. 5
+ *   templates: 2PN stationary-phase phase, Newtonian f^(-7/6) amplitude, between 40 Hz and
+ *              min(f_ISCO, Nyquist)
+ *   events: per window of W samples, the sample of maximum rho if rho > threshold, with its
+ *           chi^2                                                            PAPER.md:184 (+ DESIGN.md reading 12)
+ *
+ * Conventions
+ *   - Every function returns GWMF_OK (0) or a negative gwmf_status; nothing throws or aborts.
+ *   - All device work is enqueued on the CUDA stream given to gwmf_create.  Calls marked "async"
+ *     return before the work completes; calls marked "syncs" wait for the stream.
+ *   - Ownership: the caller owns every array it passes and the workspace; the library copies what
+ *     it needs during the call and owns only the gwmf_ctx.
+ *   - One context per stream; calls on one context are not re-entrant.
+ *   - There is no CPU fallback: gwmf_create fails with GWMF_E_CUDA if no sm_100 device is current.
+ *   - Determinism: identical inputs give bit-identical outputs; triggers come back sorted by
+ *     (template_id, window index).
+ */
+#ifndef GWMF_H
+#define GWMF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* G Msun / c^3 in seconds (nominal solar mass parameter); masses are in solar masses. */
+#define GWMF_T_SUN 4.9254909476412675e-6
+
+typedef enum {
+  GWMF_OK = 0,
+  GWMF_E_ARG = -1,            /* null pointer, n not a power of two in [2^14, 2^22], p < 1 or > 32,
+                                 window not dividing n, non-positive mass, bad S_n                  */
+  GWMF_E_EMPTY_TEMPLATE = -2, /* k_high <= k_low: f_ISCO <= f_low (total mass >~ 110 Msun)          */
+  GWMF_E_STATE = -3,          /* filter before a bank and a segment are loaded, etc.                */
+  GWMF_E_CAPACITY = -4,       /* output buffer too small; *n_out still receives the needed count   */
+  GWMF_E_CUDA = -5,           /* a CUDA call failed; gwmf_last_cuda_error() has the text            */
+  GWMF_E_WORKSPACE = -6       /* workspace smaller than gwmf_workspace_bytes()                      */
+} gwmf_status;
+
+typedef struct gwmf_ctx gwmf_ctx;                      /* opaque */
+
+typedef struct { double m1, m2; } gwmf_mass_pair;      /* solar masses, > 0, any order */
+
+typedef struct {                                       /* one event, 16 bytes */
+  int32_t template_id;                                 /* index into the bank                     */
+  int32_t sample;                                      /* j* in [0, n)                            */
+  float   rho;                                         /* |z[j*]| / sigma                         */
+  float   chisq;                                       /* chi^2[j*], 2p-2 degrees of freedom      */
+} gwmf_trigger;
+
+typedef struct {
+  int64_t n;             /* samples per segment: power of two, 2^14 .. 2^22 (2^20)   */
+  double  fs;            /* sampling rate in Hz (4096)                                            */
+  double  f_low;         /* low-frequency cut-off in Hz (40); the bin at exactly f_low is in      */
+  int32_t p;             /* chi^2 bands, 1 .. 32 (16)                               */
+  double  rho_thresh;    /* SNR threshold, strict '>'                                             */
+  int32_t window;        /* W: trigger window in samples, power of two, divides n                 */
+  int32_t max_templates; /* capacity of the bank                                                  */
+  int32_t batch;         /* templates filtered per kernel launch (0 = library default); sizes the
+                            band-intermediate buffer: batch * p * n * 8 bytes                     */
+} gwmf_params;
+
+/* Bytes of DEVICE memory the caller must provide to gwmf_create (0 if params are invalid). */
+size_t gwmf_workspace_bytes(const gwmf_params* params);
+
+/* Create a context.  d_workspace: DEVICE pointer, 256-byte aligned, >= gwmf_workspace_bytes(params),
+ * owned by the caller and kept alive until gwmf_destroy.  cuda_stream: a cudaStream_t (NULL = the
+ * legacy default stream).  Builds the twiddle tables (async). */
+int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_bytes,
+                void* cuda_stream, gwmf_ctx** out);
+
+/* Load the template bank: per template the 2PN phase coefficients and
+ * k_high = min(ceil(f_cut/df), n/2), f_cut = min(1/(6^1.5 pi M), fs/2).  host_masses: HOST array of
+ * n_templates pairs, 1 <= n_templates <= max_templates.  sigma and the p+1 band edges depend on S_n and
+ * are (re)computed on the device by gwmf_load_segment / here if a segment is already loaded.  async. */
+int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_templates);
+
+/* Load one strain segment and its PSD (Eq. 1 inputs).
+ *   s  : n fp32 samples of s(t), HOST or DEVICE pointer.
+ *   Sn : n/2+1 fp64 samples of the one-sided PSD at f_k = k fs/n, HOST or DEVICE pointer.  Entries
+ *        below f_low and the Nyquist entry are ignored (Eq. 2 diverges at f -> 0).  Entries inside
+ *        [f_low, fs/2) must be finite and > 0 -- checked on the device; a violation is reported by
+ *        the next syncing call as GWMF_E_ARG.
+ * Computes on the device: the data spectrum D[k] = sum_j s[j] e^{-2 pi i jk/n} with the library's own
+ * FFT, the weighted spectrum w[k] = (4/n) D[k] f_k^(-7/6) / S_n[k], the fp64 power table
+ * C[k] = sum_{k'<=k} f^(-7/3)/S_n (Eq. 4) and, if a bank is loaded, sigma and band edges of every
+ * template.  The arrays may be freed after the call returns (host sources are staged synchronously
+ * with respect to the host; device sources are read on the stream before the call returns control
+ * to later work on that stream).  async for device sources. */
+int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn);
+
+/* Matched-filter templates [first_template, first_template + n_templates) against the loaded segment:
+ * p band inverse FFTs, rho and chi^2 at every sample (Eq. 3, 5) and the per-window
+ * maxima above threshold.  Trigger slots of those templates are reset first.  async. */
+int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
+
+/* Measurement: the same work as gwmf_filter, with CUDA events recorded on the context's stream around
+ * every launch of the two hot kernels.  host_ms[0] / host_ms[1] receive the summed device time (ms) of
+ * the pass-1 (correlate + first FFT pass) and pass-2 (second FFT pass + rho/chi^2/trigger epilogue)
+ * launches, host_launches[0..1] the number of launches of each.  syncs. */
+int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
+                      int32_t* host_launches);
+
+/* Collect the events of all templates filtered since the last gwmf_load_segment, sorted by
+ * (template_id, window).  host_out: HOST array of `capacity` triggers (may be NULL if capacity = 0).
+ * *n_out receives the number of events found; GWMF_E_CAPACITY if it exceeds capacity (nothing is
+ * written beyond capacity).  syncs. */
+int gwmf_triggers(gwmf_ctx* ctx, gwmf_trigger* host_out, int64_t capacity, int64_t* n_out);
+
+/* sigma of every loaded template (Eq. 4 with unit amplitude constant), HOST array of n_templates
+ * doubles.  Needs a bank and a segment.  syncs. */
+int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma);
+
+/* Band edges e_0..e_p of every loaded template, HOST array of n_templates*(p+1) int32.  syncs. */
+int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges);
+
+/* Debug/parity: full rho(t) and chi^2(t) of one template, n floats each, HOST arrays (either may be
+ * NULL).  Runs the same kernels as gwmf_filter on that template with series output enabled; does not
+ * touch trigger slots.  syncs. */
+int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host_chisq);
+
+/* Debug/parity: the library's batched complex FFT alone.  X[k] = sum_j x[j] e^{+2 pi i jk/n}
+ * (unnormalised inverse transform, the e^{2 pi i f t} of Eq. 1).  in/out: DEVICE arrays of n
+ * interleaved complex fp32 (re, im), n = params.n; in != out.  async. */
+int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out);
+
+/* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
+int64_t gwmf_launch_count(const gwmf_ctx* ctx);
+
+void gwmf_destroy(gwmf_ctx* ctx);
+
+const char* gwmf_strerror(int status);
+const char* gwmf_last_cuda_error(const gwmf_ctx* ctx);   /* "" if none */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWMF_H */

@@ -1,0 +1,81 @@
+// gwmf_internal.cuh -- shared declarations of the CUDA side (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "../../include/gwmf.h"
+
+namespace gwmf {
+
+constexpr int kN2 = 1024;        // second-pass transform length (columns k2), fixed for every N
+constexpr int kLogN2 = 10;
+constexpr int kMaxBands = 32;
+constexpr int kColsPerCta = 8;   // pass-1 column tile: 8 columns x 8 B = 64 B segments per output row
+constexpr int kP2Warps = 8;      // pass-2 rows (j1 values) per CTA, one warp each
+
+// Per-template record (device).  Phase in TURNS: psi(u) = (((c0 u^2 + c2) u + c3) u + c4) u - 1/8 with
+// u = f^(-1/3); this is Psi0/(2 pi) of the 2PN SPA phase (BASELINE.json:configs[0]).
+struct TemplateMeta {
+  double c0, c2, c3, c4;
+  double sigma;                  // Eq. 4, amplitude constant 1
+  float scale_rho2;              // (sigma_ref / sigma)^2: rho^2 = |z_scaled|^2 * scale_rho2
+  int32_t k_high;                // first bin above the template
+  int32_t edges[kMaxBands + 1];  // band l = bins [edges[l], edges[l+1])
+  int32_t pad_;
+};
+
+// One (template, window) trigger slot, updated with a 128-bit compare-and-swap.
+//   key  = (bits(rho) << 32) | (0xFFFFFFFF - sample)   -> max key = max rho, lowest sample on ties
+//   aux  = bits(chi^2) in the low word
+struct alignas(16) Slot {
+  unsigned long long key;
+  unsigned long long aux;
+};
+
+struct Layout {                  // byte offsets into the caller's workspace
+  size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, slots, counts, offsets, trig_out,
+         series_rho, series_chi, flags, y, total;
+  size_t y_bytes;
+  int batch;
+};
+
+struct Ctx {
+  gwmf_params prm;
+  int64_t n;
+  int log_n;
+  int n1;                        // n / kN2
+  int na, nb;                    // n1 = na * nb (pass-1 stage radices)
+  int k_low;
+  int n_windows;
+  double df;
+  Layout lay;
+  char* ws;
+  cudaStream_t stream;
+  int n_templates;
+  bool have_bank, have_segment;
+  int64_t launches;
+  std::string cuda_err;
+  TemplateMeta* h_meta;          // host staging of the bank (pinned)
+};
+
+// ---- launchers (defined in the .cu files) --------------------------------------------------------
+cudaError_t launch_tables(Ctx* c);
+cudaError_t launch_segment_prepare(Ctx* c);                       // after s/Sn are on the device
+cudaError_t launch_bank_setup(Ctx* c);
+cudaError_t launch_pass1_filter(Ctx* c, int first, int count);
+cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
+cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,
+                                float* series_chi);
+cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out);
+inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, float2* d_out) {
+  cudaError_t e = launch_pass1_dense(c, d_in, d_mid);
+  return e != cudaSuccess ? e : launch_pass2_dense(c, d_mid, d_out);
+}
+cudaError_t launch_reset_slots(Ctx* c, int first, int count);
+cudaError_t launch_compact(Ctx* c);
+
+template <typename T>
+inline T* ws_ptr(Ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
+
+}  // namespace gwmf

@@ -1,0 +1,211 @@
+// pass1.cu -- first pass of the band inverse FFTs (step a2 + first half of a3), with the correlate
+// fused in: the input Q[k] = w[k] f_k^(-7/6) e^{i Psi0(f_k)} is GENERATED per bin (template phase in fp64,
+// reduced to turns, then fp32 sincospi) and never stored.
+//
+// Index algebra.  n = n1 * 1024.  Input bin k = 1024 k1 + k2, output sample j = j1 + n1 j2.
+//   z_l[j1 + n1 j2] = sum_{k2} e^{2 pi i j2 k2/1024} Y_l[j1][k2]                               (pass 2)
+//   Y_l[j1][k2]     = e^{2 pi i j1 k2/n} sum_{k1 in band l} Q[1024 k1 + k2] e^{2 pi i j1 k1/n1}  (this file)
+// The n1-point column transform is itself split n1 = NA * NB with k1 = NB a + b, j1 = ja + NA jb:
+//   stage 1 (thread = (b, column)):  V[ja][b] = sum_a Q[NB a + b] w_NA^{ja a}, times e^{2 pi i ja (1024 b + k2)/n}
+//   stage 2 (thread = (ja, column)): Y[ja + NA jb] = e^{2 pi i NA jb k2/n} sum_b w_NB^{jb b} V[ja][b]
+// A band is a contiguous run of bins, i.e. of rows k1, so stage 1 only touches the groups of `a` that
+// the band reaches (pruned input); for NA > 32 a CTA produces the 32 outputs ja = G m + r of one residue r.
+#include "fft_reg.cuh"
+#include "gwmf_internal.cuh"
+
+namespace gwmf {
+
+struct P1Args {
+  const TemplateMeta* meta;   // already offset to the first template of the batch
+  const float2* wq;           // weighted spectrum, n/2
+  const double* u_tab;        // f^(-1/3), n/2
+  const float2* tw_n1;        // e^{2 pi i m/n1}
+  const float2* dense_in;     // DENSE only: n complex inputs
+  float2* y;                  // [batch][p][n1][1024]
+  int p;
+  int log_n;
+  int n1;
+};
+
+__device__ __forceinline__ float2 cis_frac(unsigned num, int log_n) {
+  // e^{2 pi i num / 2^log_n}, num < 2^log_n <= 2^22: the argument 2 num / n is exact in fp32
+  float s, c;
+  sincospif(2.0f * (float)num / (float)(1u << log_n), &s, &c);
+  return make_float2(c, s);
+}
+
+template <int NA, int NB, bool DENSE>
+__global__ void __launch_bounds__(256) k_pass1(P1Args a) {
+  constexpr int FR = NA >= 32 ? 32 : NA;        // stage-1 transform length = ja outputs per CTA
+  constexpr int G = NA / FR;                    // residues r of ja = G m + r
+  constexpr int GA = NA >= 32 ? 16 : NA;        // inputs a per group
+  constexpr int NGROUPS = NA / GA;
+  constexpr int C = kColsPerCta;
+  constexpr int SROW = NB * C + C;              // padded stride of S[m][..] in float2
+
+  extern __shared__ float2 smem[];
+  float2* S = smem;                             // [FR][SROW]
+  float2* A = S + FR * SROW;                    // [FR][C]   e^{2 pi i ja k2/n}
+  float2* Bt = A + FR * C;                      // [NB][C]   e^{2 pi i NA jb k2/n}
+
+  const int tid = threadIdx.x;
+  const int x = tid >> 3, c = tid & 7;
+  const int k2 = blockIdx.x * C + c;
+  const int l = blockIdx.y;
+  const int tb = blockIdx.z / G, r = blockIdx.z % G;
+  const unsigned nmask = (1u << a.log_n) - 1u;
+  const int n1 = a.n1;
+
+  int e_lo, e_hi;
+  double c0 = 0, c2 = 0, c3 = 0, c4 = 0;
+  if constexpr (DENSE) {
+    e_lo = 0;
+    e_hi = 1 << a.log_n;
+  } else {
+    const TemplateMeta* m = a.meta + tb;
+    e_lo = m->edges[l];
+    e_hi = m->edges[l + 1];
+    c0 = m->c0; c2 = m->c2; c3 = m->c3; c4 = m->c4;
+  }
+  // rows and a-range touched by the band (uniform over the CTA)
+  const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
+  const int a_lo = row_lo / NB, a_hi = (e_hi > e_lo) ? row_hi / NB : -1;
+
+  if (x < FR) A[x * C + c] = cis_frac(((unsigned)((G * x + r) * k2)) & nmask, a.log_n);
+  if (x < NB) Bt[x * C + c] = cis_frac(((unsigned)(NA * x) * (unsigned)k2) & nmask, a.log_n);
+  __syncthreads();
+
+  // ------------------------------------------------------------------ stage 1: thread (b = x, c)
+  if (x < NB) {
+    const int b = x;
+    float2 acc[FR];
+#pragma unroll
+    for (int m = 0; m < FR; ++m) acc[m] = make_float2(0.f, 0.f);
+#pragma unroll 1
+    for (int g = 0; g < NGROUPS; ++g) {
+      const int a_base = GA * g;
+      if (a_base > a_hi || a_base + GA - 1 < a_lo) continue;
+      float2 xin[FR];
+#pragma unroll
+      for (int ap = 0; ap < FR; ++ap) {
+        float2 q = make_float2(0.f, 0.f);
+        if (ap < GA) {
+          const int aa = a_base + ap;
+          const int k = ((NB * aa + b) << kLogN2) + k2;
+          if (aa >= a_lo && aa <= a_hi && k >= e_lo && k < e_hi) {
+            if constexpr (DENSE) {
+              q = a.dense_in[k];
+            } else {
+              // correlate: template phasor times weighted data bin (Eq. 1 integrand)
+              const double u = a.u_tab[k];
+              double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
+              t -= rint(t);
+              float sn, cs;
+              sincospif(2.0f * (float)t, &sn, &cs);
+              q = cmul(a.wq[k], make_float2(cs, sn));
+            }
+            if constexpr (G > 1) {
+              if (r > 0) q = cmul(q, a.tw_n1[(r * ap * NB) % n1]);       // w_NA^{r a'}
+            }
+          }
+        }
+        xin[ap] = q;
+      }
+      fft_dif<FR>(xin);
+#pragma unroll
+      for (int m = 0; m < FR; ++m) {
+        float2 v = xin[brev<FR>(m)];
+        if constexpr (NGROUPS > 1) {
+          if (g > 0) v = cmul(v, a.tw_n1[(a_base * (G * m + r) * NB) % n1]);   // w_NA^{a_base ja}
+        }
+        acc[m] = cadd(acc[m], v);
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < FR; ++m) {
+      const int ja = G * m + r;
+      const float2 tw = cmul(a.tw_n1[(ja * b) % n1], A[m * C + c]);   // e^{2 pi i ja (1024 b + k2)/n}
+      S[m * SROW + b * C + c] = cmul(acc[m], tw);
+    }
+  }
+  __syncthreads();
+
+  // ------------------------------------------------------------------ stage 2: thread (m = x, c)
+  if (x < FR) {
+    const int m = x;
+    float2 v[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) v[b] = S[m * SROW + b * C + c];
+    fft_dif<NB>(v);
+    const int band_index = DENSE ? 0 : (tb * a.p + l);
+    float2* out = a.y + ((size_t)band_index * n1 + (size_t)(G * m + r)) * kN2 + k2;
+#pragma unroll
+    for (int jb = 0; jb < NB; ++jb)
+      out[(size_t)jb * NA * kN2] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
+  }
+}
+
+template <int NA, int NB, bool DENSE>
+static cudaError_t launch_p1(Ctx* c, const P1Args& args, int batch, int bands) {
+  constexpr int FR = NA >= 32 ? 32 : NA;
+  constexpr int G = NA / FR;
+  constexpr int SROW = NB * kColsPerCta + kColsPerCta;
+  const size_t smem = (size_t)(FR * SROW + FR * kColsPerCta + NB * kColsPerCta) * sizeof(float2);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass1<NA, NB, DENSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid(kN2 / kColsPerCta, bands, batch * G);
+  k_pass1<NA, NB, DENSE><<<grid, 256, smem, c->stream>>>(args);
+  c->launches++;
+  return cudaGetLastError();
+}
+
+template <bool DENSE>
+static cudaError_t dispatch_p1(Ctx* c, const P1Args& args, int batch, int bands) {
+  switch (c->na) {
+    case 1:
+      if (c->nb == 16) return launch_p1<1, 16, DENSE>(c, args, batch, bands);
+      return launch_p1<1, 32, DENSE>(c, args, batch, bands);
+    case 2: return launch_p1<2, 32, DENSE>(c, args, batch, bands);
+    case 4: return launch_p1<4, 32, DENSE>(c, args, batch, bands);
+    case 8: return launch_p1<8, 32, DENSE>(c, args, batch, bands);
+    case 16: return launch_p1<16, 32, DENSE>(c, args, batch, bands);
+    case 32: return launch_p1<32, 32, DENSE>(c, args, batch, bands);
+    case 64: return launch_p1<64, 32, DENSE>(c, args, batch, bands);
+    case 128: return launch_p1<128, 32, DENSE>(c, args, batch, bands);
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
+  P1Args args;
+  args.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
+  args.wq = ws_ptr<float2>(c, c->lay.wq);
+  args.u_tab = ws_ptr<double>(c, c->lay.u_tab);
+  args.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
+  args.dense_in = nullptr;
+  args.y = ws_ptr<float2>(c, c->lay.y);
+  args.p = c->prm.p;
+  args.log_n = c->log_n;
+  args.n1 = c->n1;
+  return dispatch_p1<false>(c, args, count, c->prm.p);
+}
+
+cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
+  P1Args args;
+  args.meta = nullptr;
+  args.wq = nullptr;
+  args.u_tab = nullptr;
+  args.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
+  args.dense_in = d_in;
+  args.y = d_mid;
+  args.p = 1;
+  args.log_n = c->log_n;
+  args.n1 = c->n1;
+  return dispatch_p1<true>(c, args, 1, 1);
+}
+
+}  // namespace gwmf

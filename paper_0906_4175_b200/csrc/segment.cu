@@ -1,0 +1,173 @@
+// segment.cu -- per-context tables, per-segment preparation (step a0) and per-template sigma / band
+// edges (step a1's reductions).  None of this is on the per-template hot path.
+#include "gwmf_internal.cuh"
+
+namespace gwmf {
+
+// ---------------------------------------------------------------------------------------------------
+// Tables that depend only on the parameters.
+//   u_tab[k]  = f_k^(-1/3) (fp64), k = 0 .. n/2-1 (u_tab[0] = 0)
+//   tw_n1[m]  = e^{2 pi i m / n1}, m = 0 .. n1-1        (pass-1 inter-stage twiddles)
+//   tw_p2[jm][c] = e^{2 pi i jm c / 1024}, 32 x 32      (pass-2 inter-stage twiddles)
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_tables(double* __restrict__ u_tab, float2* __restrict__ tw_n1, float2* __restrict__ tw_p2,
+                         int half_n, int n1, double df) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < half_n) u_tab[i] = (i == 0) ? 0.0 : rcbrt((double)i * df);
+  if (i < n1) {
+    double s, c;
+    sincospi(2.0 * (double)i / (double)n1, &s, &c);
+    tw_n1[i] = make_float2((float)c, (float)s);
+  }
+  if (i < 1024) {
+    int jm = i >> 5, cc = i & 31;
+    double s, c;
+    sincospi(2.0 * (double)(jm * cc) / 1024.0, &s, &c);
+    tw_p2[i] = make_float2((float)c, (float)s);
+  }
+}
+
+cudaError_t launch_tables(Ctx* c) {
+  int half = (int)(c->n / 2);
+  int work = half > 1024 ? half : 1024;
+  k_tables<<<(work + 255) / 256, 256, 0, c->stream>>>(ws_ptr<double>(c, c->lay.u_tab),
+                                                      ws_ptr<float2>(c, c->lay.tw_n1),
+                                                      ws_ptr<float2>(c, c->lay.tw_p2), half, c->n1, c->df);
+  c->launches++;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Segment preparation.
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_real_to_complex(const float* __restrict__ s, float2* __restrict__ x, int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) x[i] = make_float2(s[i], 0.f);
+}
+
+// g[k] = f_k^(-7/3) / S_n[k] = u^7 / S_n[k] for k_low <= k < n/2, else 0 (integrand of Eq. 4).
+// flags[0] is raised if S_n is not finite and positive inside the band.
+__global__ void k_power_terms(const double* __restrict__ sn, const double* __restrict__ u_tab,
+                              double* __restrict__ g, int* __restrict__ flags, int k_low, int half_n) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= half_n) return;
+  double v = 0.0;
+  if (k >= k_low) {
+    double S = sn[k];
+    if (!(S > 0.0) || isinf(S)) {
+      atomicOr(flags, 1);
+    } else {
+      double u = u_tab[k], u2 = u * u, u4 = u2 * u2;
+      v = u4 * u2 * u / S;
+    }
+  }
+  g[k] = v;
+}
+
+// Inclusive fp64 prefix sum C[k] = sum_{k' <= k} g[k'] with a fixed summation order: one CTA of 1024
+// threads, thread t sums the contiguous chunk [t*L, (t+1)*L) sequentially, chunk totals are scanned
+// sequentially by thread 0, then every thread rewrites its chunk.  (Once per segment; 4 MiB.)
+__global__ void __launch_bounds__(1024) k_prefix(const double* __restrict__ g, double* __restrict__ c_tab,
+                                                 int half_n) {
+  __shared__ double part[1024];
+  int t = threadIdx.x;
+  int L = (half_n + 1023) / 1024;
+  int lo = t * L, hi = min(lo + L, half_n);
+  double acc = 0.0;
+  for (int k = lo; k < hi; ++k) acc += g[k];
+  part[t] = acc;
+  __syncthreads();
+  if (t == 0) {
+    double run = 0.0;
+    for (int i = 0; i < 1024; ++i) { double v = part[i]; part[i] = run; run += v; }
+  }
+  __syncthreads();
+  acc = part[t];
+  for (int k = lo; k < hi; ++k) { acc += g[k]; c_tab[k] = acc; }
+}
+
+// wq[k] = (4/n) conj(Z[k]) f_k^(-7/6) / S_n[k] / sigma_ref for k_low <= k < n/2, else 0, where
+// Z = sum_j s[j] e^{+2 pi i jk/n} (so conj(Z) is the ordinary forward DFT D[k] of the real segment,
+// DESIGN.md reading 1) and sigma_ref = sqrt(4 df C[n/2-1]) keeps every later fp32 quantity O(rho)
+// whatever the units of s and S_n.
+__global__ void k_weighted_spectrum(const float2* __restrict__ Z, const double* __restrict__ sn,
+                                    const double* __restrict__ u_tab, const double* __restrict__ c_tab,
+                                    float2* __restrict__ wq, int k_low, int half_n, double four_over_n,
+                                    double four_df) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= half_n) return;
+  float2 out = make_float2(0.f, 0.f);
+  if (k >= k_low) {
+    double S = sn[k];
+    if (S > 0.0 && !isinf(S)) {
+      double sigma_ref = sqrt(four_df * c_tab[half_n - 1]);
+      double u = u_tab[k];
+      double amp = u * u * u * sqrt(u);                 // f^(-7/6)
+      double w = four_over_n * amp / (S * sigma_ref);
+      float2 z = Z[k];
+      out = make_float2((float)(w * (double)z.x), (float)(-w * (double)z.y));
+    }
+  }
+  wq[k] = out;
+}
+
+cudaError_t launch_segment_prepare(Ctx* c) {
+  const int half = (int)(c->n / 2);
+  float2* y = ws_ptr<float2>(c, c->lay.y);
+  float2* X = y;                       // n complex: the segment as complex input
+  float2* mid = y + c->n;              // n complex: pass-1 output
+  float2* Z = y + 2 * c->n;            // n complex: transform
+  k_real_to_complex<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(ws_ptr<float>(c, c->lay.s_in), X, c->n);
+  c->launches++;
+  cudaError_t e = launch_fft_dense(c, X, mid, Z);
+  if (e != cudaSuccess) return e;
+  int* flags = ws_ptr<int>(c, c->lay.flags);
+  cudaMemsetAsync(flags, 0, sizeof(int), c->stream);
+  k_power_terms<<<(half + 255) / 256, 256, 0, c->stream>>>(ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab),
+                                                           ws_ptr<double>(c, c->lay.g_tab), flags, c->k_low, half);
+  k_prefix<<<1, 1024, 0, c->stream>>>(ws_ptr<double>(c, c->lay.g_tab), ws_ptr<double>(c, c->lay.c_tab), half);
+  k_weighted_spectrum<<<(half + 255) / 256, 256, 0, c->stream>>>(
+      Z, ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab), ws_ptr<double>(c, c->lay.c_tab),
+      ws_ptr<float2>(c, c->lay.wq), c->k_low, half, 4.0 / (double)c->n, 4.0 * c->df);
+  c->launches += 3;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// sigma and band edges of every template (Eq. 4; equal-power bands):
+//   sigma^2 = 4 df C[k_high-1];  e_0 = k_low;  e_l = 1 + min{k : C[k] >= (l/p) C[k_high-1]};  e_p = k_high.
+// One thread per template; the edges are binary searches in the monotone fp64 table.
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_bank_setup(TemplateMeta* __restrict__ meta, const double* __restrict__ c_tab, int n_templates,
+                             int p, int k_low, int half_n, double four_df) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_templates) return;
+  TemplateMeta m = meta[t];
+  double total = c_tab[m.k_high - 1];
+  double ref = c_tab[half_n - 1];
+  m.sigma = sqrt(four_df * total);
+  m.scale_rho2 = (float)(ref / total);
+  m.edges[0] = k_low;
+  for (int l = 1; l < p; ++l) {
+    double target = ((double)l / (double)p) * total;
+    int lo = k_low, hi = m.k_high - 1;          // smallest k in [lo, hi] with C[k] >= target
+    while (lo < hi) {
+      int mid = (lo + hi) >> 1;
+      if (c_tab[mid] >= target) hi = mid; else lo = mid + 1;
+    }
+    m.edges[l] = lo + 1;
+  }
+  m.edges[p] = m.k_high;
+  for (int l = p + 1; l <= kMaxBands; ++l) m.edges[l] = m.k_high;
+  meta[t] = m;
+}
+
+cudaError_t launch_bank_setup(Ctx* c) {
+  k_bank_setup<<<(c->n_templates + 127) / 128, 128, 0, c->stream>>>(
+      ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<double>(c, c->lay.c_tab), c->n_templates, c->prm.p, c->k_low,
+      (int)(c->n / 2), 4.0 * c->df);
+  c->launches++;
+  return cudaGetLastError();
+}
+
+}  // namespace gwmf

@@ -1,0 +1,276 @@
+"""GPU-vs-oracle parity, element by element on the same seeded inputs, through the C ABI
+(paper_0906_4175_b200.gwmf is argument marshalling only).  Run with `-m gpu` on a B200."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import parity
+from paper_0906_4175_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gw():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_0906_4175_b200 import gwmf
+    gwmf.load_library()
+    return gwmf
+
+
+def _run_gpu(gw, w, s, Sn, masses=None, batch=0, window=None, thresh=None, p=None):
+    masses = w.masses if masses is None else masses
+    f = gw.Filter(w.n, p or w.p, window or w.window, len(masses), rho_thresh=w.rho_thresh if thresh is None else thresh,
+                  batch=batch)
+    f.make_bank(masses)
+    f.load_segment(s.astype(np.float32), Sn)
+    f.filter()
+    return f
+
+
+# ----------------------------------------------------------------------------- the FFT alone
+@pytest.mark.parametrize("log_n", [14, 15, 16, 17, 18, 19, 20, 21, 22])
+def test_fft_inverse_alone(gw, log_n):
+    import torch
+    n = 1 << log_n
+    k = np.arange(n)
+    x = (inputs.normal(100 + log_n, 0, k) + 1j * inputs.normal(100 + log_n, 1, k)).astype(np.complex64)
+    f = gw.Filter(n, 4, 4096, 1)
+    X = f.fft_inverse(torch.from_numpy(x).cuda())
+    f.synchronize()
+    want = oracle.fft(x.astype(np.complex128), +1)
+    got = X.cpu().numpy().astype(np.complex128)
+    rms = math.sqrt(n) * 1.41
+    err = np.max(np.abs(got - want)) / rms
+    assert err < 4e-6, err
+    # closed form: an impulse at j0 -> a pure tone (catches a transposed index map at any size)
+    imp = np.zeros(n, np.complex64); imp[12345 % n] = 1.0
+    T = f.fft_inverse(torch.from_numpy(imp).cuda()).cpu().numpy()
+    tone = np.exp(2j * np.pi * ((12345 % n) * k % n) / n)
+    assert np.max(np.abs(T - tone)) < 2e-6
+
+
+# ----------------------------------------------------------------------------- config 0, everything
+def test_config0_full(gw):
+    w = inputs.workload(0)
+    s = inputs.segment(w)
+    Sn = w.psd
+    f = _run_gpu(gw, w, s, Sn)
+    out = oracle.filter_bank(s.astype(np.float32).astype(np.float64), Sn, w.masses, w.p, w.window, w.rho_thresh)
+    parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
+    s32 = s.astype(np.float32).astype(np.float64)
+    for t, (m1, m2) in enumerate(w.masses):
+        rho_o, chi_o, _, _ = oracle.filter_template(s32, Sn, m1, m2, w.p)
+        rho_g, chi_g = f.series(t)
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, w.p, f"config0 template {t}")
+    trig = f.triggers()
+    compared, exempt = parity.assert_triggers(trig, out, w.rho_thresh, w.window, w.p)
+    assert compared >= 1
+    mine = [t for t in trig if t["template_id"] == 4]
+    assert len(mine) == 1 and abs(int(mine[0]["sample"]) - 9000) <= 3
+
+
+def test_config0_noise_free_closed_forms(gw):
+    # P6 on the GPU: rho = A = 12 at t_c, chi^2 = 0.001021 (closed form), other templates as tabulated
+    w = inputs.workload(0)
+    s = inputs.segment(w, noise=False)
+    f = _run_gpu(gw, w, s, w.psd)
+    rho, chi = f.series(4)
+    assert int(np.argmax(rho)) == 9000
+    assert rho[9000] == pytest.approx(12.0, abs=1e-3 + 12e-4)
+    assert chi[9000] == pytest.approx(0.001021435, abs=1e-3)
+    rho1, chi1 = f.series(2)                       # (6,10): 9011, 9.245720, 25.878613
+    assert int(np.argmax(rho1)) == 9011 and rho1[9011] == pytest.approx(9.245720, abs=2e-3)
+    assert chi1[9011] == pytest.approx(25.878613, rel=1e-3)
+
+
+# ----------------------------------------------------------------------------- ragged mid-size cases
+@pytest.mark.parametrize("log_n,p,window,batch", [(15, 5, 2048, 3), (16, 7, 8192, 2), (17, 16, 4096, 0),
+                                                  (19, 3, 1 << 19, 5)])
+def test_midsize_full_series(gw, log_n, p, window, batch):
+    n = 1 << log_n
+    masses = [(1.0, 1.0), (1.4, 1.4), (3.0, 1.2), (5.0, 5.0), (10.0, 1.4), (12.0, 9.0), (20.0, 14.0)]
+    D = inputs.noise_spectrum(n, 40 + log_n)
+    D = D + inputs.injection_spectrum(n, 3.0, 1.2, 11.0, n // 3) + inputs.injection_spectrum(n, 12.0, 9.0, 9.0, n - 5)
+    s = inputs.time_series(D, n).astype(np.float32)
+    Sn = inputs.psd_array(n)
+    w = inputs.Workload(config=-1, n=n, p=p, rho_thresh=5.0, window=window, masses=masses, seed=0)
+    f = _run_gpu(gw, w, s, Sn, batch=batch)
+    out = oracle.filter_bank(s.astype(np.float64), Sn, masses, p, window, 5.0)
+    parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
+    for t, (m1, m2) in enumerate(masses):
+        rho_o, chi_o, _, _ = oracle.filter_template(s.astype(np.float64), Sn, m1, m2, p)
+        rho_g, chi_g = f.series(t)
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, p, f"n=2^{log_n} template {t}")
+    compared, _ = parity.assert_triggers(f.triggers(), out, 5.0, window, p)
+    assert compared >= 2
+
+
+# ----------------------------------------------------------------------------- configs 1, 2, 4: sampled templates
+def _sampled_config(gw, config, sample_ids, n_templates=None):
+    w = inputs.workload(config, n_templates)
+    s = inputs.segment(w).astype(np.float32)
+    Sn = w.psd
+    f = _run_gpu(gw, w, s, Sn)
+    trig = f.triggers()
+    sub = [w.masses[i] for i in sample_ids]
+    s64 = s.astype(np.float64)
+    out = oracle.filter_bank(s64, Sn, sub, w.p, w.window, w.rho_thresh)
+    sig, edges = f.sigma(), f.band_edges()
+    parity.assert_sigma_edges(sig[sample_ids], edges[sample_ids], out["sigma"], out["edges"])
+    compared, exempt = parity.assert_triggers(trig, out, w.rho_thresh, w.window, w.p, template_ids=sample_ids)
+    # full series of two of the sampled templates
+    for i in sample_ids[:2]:
+        rho_o, chi_o, _, _ = oracle.filter_template(s64, Sn, w.masses[i][0], w.masses[i][1], w.p)
+        rho_g, chi_g = f.series(i)
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, w.p, f"config {config} template {i}")
+    return w, trig, compared
+
+
+def test_config1_all_templates(gw):
+    w = inputs.workload(1)
+    s = inputs.segment(w).astype(np.float32)
+    Sn = w.psd
+    f = _run_gpu(gw, w, s, Sn)
+    out = oracle.filter_bank(s.astype(np.float64), Sn, w.masses, w.p, w.window, w.rho_thresh)
+    parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
+    compared, exempt = parity.assert_triggers(f.triggers(), out, w.rho_thresh, w.window, w.p)
+    assert compared >= 3
+    for t in (0, 97, 255):
+        rho_o, chi_o, _, _ = oracle.filter_template(s.astype(np.float64), Sn, w.masses[t][0], w.masses[t][1], w.p)
+        rho_g, chi_g = f.series(t)
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, w.p, f"config 1 template {t}")
+
+
+def test_config2_headline_sampled(gw):
+    w0 = inputs.workload(2)
+    inj = sorted({b for (b, *_rest) in w0.injections})[:6]
+    ids = sorted(set(inj + [0, 31, 500, 1023]))
+    w, trig, compared = _sampled_config(gw, 2, ids)
+    assert compared >= len(inj)
+    # order-of-magnitude check on noise exceedances: exp(-18) * N * T ~ 16 samples
+    assert len(trig) < 2000
+
+
+def test_config4_long_segment_sampled(gw):
+    w0 = inputs.workload(4)
+    inj = sorted({b for (b, *_rest) in w0.injections})[:2]
+    ids = sorted(set(inj + [0, 511]))
+    _sampled_config(gw, 4, ids)
+
+
+def test_config3_stream_segments_sampled(gw):
+    w = inputs.workload(3)
+    x = inputs.stream(w).astype(np.float32)
+    Sn = w.psd
+    f = gw.Filter(w.n, w.p, w.window, len(w.masses), rho_thresh=w.rho_thresh)
+    f.make_bank(w.masses)
+    ids = [0, 2047, 4095]
+    for q in (0, 7):
+        seg = inputs.stream_segment(x, q, w.n)
+        f.load_segment(seg, Sn)
+        f.filter()
+        trig = f.triggers()
+        out = oracle.filter_bank(seg.astype(np.float64), Sn, [w.masses[i] for i in ids], w.p, w.window, w.rho_thresh)
+        parity.assert_triggers(trig, out, w.rho_thresh, w.window, w.p, template_ids=ids)
+        rho_o, chi_o, _, _ = oracle.filter_template(seg.astype(np.float64), Sn, *w.masses[ids[1]], w.p)
+        rho_g, chi_g = f.series(ids[1])
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, w.p, f"config 3 segment {q}")
+
+
+# ----------------------------------------------------------------------------- edge cases and the boundary
+def test_p_extremes_and_covariance(gw):
+    n = 1 << 15
+    masses = [(2.0, 1.5), (9.0, 7.0)]
+    s = inputs.time_series(inputs.noise_spectrum(n, 9) + inputs.injection_spectrum(n, 2.0, 1.5, 10.0, 777), n).astype(np.float32)
+    Sn = inputs.psd_array(n)
+    for p in (1, 2, 32):
+        w = inputs.Workload(config=-1, n=n, p=p, rho_thresh=5.5, window=n, masses=masses, seed=0)
+        f = _run_gpu(gw, w, s, Sn)
+        for t, (m1, m2) in enumerate(masses):
+            rho_o, chi_o, _, _ = oracle.filter_template(s.astype(np.float64), Sn, m1, m2, p)
+            rho_g, chi_g = f.series(t)
+            parity.assert_series(rho_g, chi_g, rho_o, chi_o, p, f"p={p} template {t}")
+            if p == 1:
+                assert np.all(chi_g == 0.0)
+    # (S_n, s) -> (c S_n, sqrt(c) s) leaves rho and chi^2 unchanged (P8), also at physical scales
+    w = inputs.Workload(config=-1, n=n, p=8, rho_thresh=5.5, window=4096, masses=masses, seed=0)
+    f1 = _run_gpu(gw, w, s, Sn)
+    r1, c1 = f1.series(0)
+    c = 9e-46
+    f2 = _run_gpu(gw, w, (s.astype(np.float64) * math.sqrt(c)), Sn * c)
+    r2, c2 = f2.series(0)
+    assert np.max(np.abs(r1 - r2)) < 2e-4 and np.max(np.abs(c1 - c2) / np.maximum(c1, 1)) < 1e-3
+    assert f2.sigma()[0] == pytest.approx(f1.sigma()[0] / math.sqrt(c), rel=1e-12)
+
+
+def test_determinism_and_refilter(gw):
+    w = inputs.workload(0)
+    s = inputs.segment(w)
+    f = _run_gpu(gw, w, s, w.psd)
+    a = f.triggers().copy()
+    r1, c1 = f.series(4)
+    f.filter()                      # slots are reset, not accumulated
+    b = f.triggers()
+    r2, c2 = f.series(4)
+    assert a.tobytes() == b.tobytes() and np.array_equal(r1, r2) and np.array_equal(c1, c2)
+    f.filter(2, 3)                  # partial re-filter keeps the other templates' events
+    assert f.triggers().tobytes() == a.tobytes()
+
+
+def test_error_codes(gw):
+    assert gw.workspace_bytes(1000, 4, 8, 1) == 0             # n not a power of two
+    assert gw.workspace_bytes(1 << 14, 0, 4096, 1) == 0       # p < 1
+    assert gw.workspace_bytes(1 << 14, 4, 3000, 1) == 0       # window not a power of two
+    f = gw.Filter(1 << 14, 4, 4096, 4)
+    with pytest.raises(gw.GwmfError) as e:
+        f.filter()
+    assert e.value.status == gw.E_ARG or e.value.status == gw.E_STATE
+    with pytest.raises(gw.GwmfError) as e:
+        f.make_bank([(8.0, -1.0)])
+    assert e.value.status == gw.E_ARG
+    with pytest.raises(gw.GwmfError) as e:
+        f.make_bank([(80.0, 80.0)])                            # f_ISCO = 27 Hz < 40 Hz
+    assert e.value.status == gw.E_EMPTY_TEMPLATE
+    with pytest.raises(gw.GwmfError) as e:
+        f.make_bank([(8.0, 8.0)] * 5)                          # over capacity
+    assert e.value.status == gw.E_ARG
+    w = inputs.workload(0)
+    f.make_bank(w.masses[:4])
+    with pytest.raises(gw.GwmfError) as e:
+        f.filter()
+    assert e.value.status == gw.E_STATE
+    s = inputs.segment(w)
+    f.load_segment(s, w.psd)
+    f.filter()
+    with pytest.raises(gw.GwmfError) as e:
+        f.triggers(capacity=0)                                 # config 0 has at least the injection's event
+    assert e.value.status == gw.E_CAPACITY
+    bad = w.psd.copy(); bad[500] = 0.0
+    f.load_segment(s, bad)
+    with pytest.raises(gw.GwmfError) as e:
+        f.triggers()
+    assert e.value.status == gw.E_ARG
+
+
+def test_no_triggers_when_threshold_is_high(gw):
+    w = inputs.workload(0)
+    f = _run_gpu(gw, w, inputs.segment(w), w.psd, thresh=50.0)
+    assert len(f.triggers()) == 0
+
+
+def test_device_resident_inputs(gw):
+    import torch
+    w = inputs.workload(0)
+    s = inputs.segment(w).astype(np.float32)
+    f = _run_gpu(gw, w, s, w.psd)
+    a = f.triggers().copy()
+    g = gw.Filter(w.n, w.p, w.window, len(w.masses), rho_thresh=w.rho_thresh)
+    g.make_bank(w.masses)
+    g.load_segment(torch.from_numpy(s).cuda(), torch.from_numpy(w.psd).cuda())
+    g.filter()
+    assert g.triggers().tobytes() == a.tobytes()
