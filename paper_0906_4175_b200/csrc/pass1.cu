@@ -25,6 +25,7 @@ struct P1Args {
   int p;
   int log_n;
   int n1;
+  int skip_narrow;            // generic kernel: leave bands of <= 32 rows to k_pass1_narrow
 };
 
 __device__ __forceinline__ float2 cis_frac(unsigned num, int log_n) {
@@ -70,6 +71,10 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
   // rows and a-range touched by the band (uniform over the CTA)
   const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
   const int a_lo = row_lo / NB, a_hi = (e_hi > e_lo) ? row_hi / NB : -1;
+  if constexpr (!DENSE && NB == 32) {
+    // bands of at most 32 rows (and empty bands) belong to k_pass1_narrow
+    if (a.skip_narrow && (e_hi <= e_lo || row_hi - row_lo + 1 <= 32)) return;
+  }
 
   if (x < FR) A[x * C + c] = cis_frac(((unsigned)((G * x + r) * k2)) & nmask, a.log_n);
   if (x < NB) Bt[x * C + c] = cis_frac(((unsigned)(NA * x) * (unsigned)k2) & nmask, a.log_n);
@@ -145,6 +150,112 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// Narrow bands (at most 32 input rows; 15 of the 16 bands of a typical template).  With so few rows
+// stage 1 degenerates: every b = k1 mod 32 has at most one non-zero a, so V[ja][b] is a single product
+// Q[k] e^{2 pi i ja k/n} and needs neither a transform over a nor a shared-memory exchange.  A thread
+// owns (ja, column): it forms its <= 32 stage-2 inputs from the band's rows (staged once per CTA in
+// shared memory, where the template phasor is evaluated), runs the 32-point transform over b in
+// registers with the tail of zero inputs pruned at compile time, and streams out its 32 rows.
+// The rows are rotated so that the band's first row sits at b' = 0; the rotation factor
+// w_32^{jb b0} is folded into the output twiddle table.
+// CTA = CJ values of ja x CC = 256/CJ columns.
+// ---------------------------------------------------------------------------------------------------
+template <int RMAX, int CC>
+__device__ __forceinline__ void narrow_body(const P1Args& a, const float2* __restrict__ E, const float2* __restrict__ Bt,
+                                            float2 A, int R, int row_lo, int ja, int c, float2* __restrict__ out,
+                                            size_t row_stride) {
+  float2 v[32];
+  const int n1m = a.n1 - 1;
+#pragma unroll
+  for (int i = 0; i < 32; ++i) {
+    v[i] = make_float2(0.f, 0.f);
+    if (i < RMAX) {
+      if (i < R) {
+        const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], A);      // e^{2 pi i ja k/n}, k = 1024 k1 + k2
+        v[i] = cmul(E[i * CC + c], t);
+      }
+    }
+  }
+  fft_dif<32>(v);
+#pragma unroll
+  for (int jb = 0; jb < 32; ++jb) out[(size_t)jb * row_stride] = cmul(v[brev<32>(jb)], Bt[jb * CC + c]);
+}
+
+template <int CJ>
+__global__ void __launch_bounds__(256, 2) k_pass1_narrow(P1Args a) {
+  constexpr int CC = 256 / CJ;
+  extern __shared__ float2 smem[];
+  float2* Bt = smem;              // [32][CC]  e^{2 pi i (NA jb k2/n + jb b0/32)}
+  float2* E = smem + 32 * CC;     // [R][CC]   Q of the band's rows, this column tile
+
+  const int tid = threadIdx.x;
+  const int c = tid % CC, x = tid / CC;
+  const int tiles = kN2 / CC;
+  const int tile = blockIdx.x % tiles, jblk = blockIdx.x / tiles;
+  const int l = blockIdx.y, tb = blockIdx.z;
+  const int na = a.n1 >> 5;
+  const int ja = jblk * CJ + x;
+  const int k2 = tile * CC + c;
+  const unsigned nmask = (1u << a.log_n) - 1u;
+
+  const TemplateMeta* m = a.meta + tb;
+  const int e_lo = m->edges[l], e_hi = m->edges[l + 1];
+  float2* out = a.y + ((size_t)(tb * a.p + l) * a.n1 + (size_t)ja) * kN2 + k2;
+  const size_t row_stride = (size_t)na * kN2;
+  if (e_hi <= e_lo) {             // empty band: z_l = 0
+#pragma unroll
+    for (int jb = 0; jb < 32; ++jb) out[(size_t)jb * row_stride] = make_float2(0.f, 0.f);
+    return;
+  }
+  const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
+  const int R = row_hi - row_lo + 1;
+  if (R > 32) return;             // wide band: k_pass1
+
+  const unsigned rot = (unsigned)(row_lo & 31) << (a.log_n - 5);           // b0 * n/32
+  for (int idx = tid; idx < 32 * CC; idx += 256) {
+    const unsigned jb = idx / CC, kk2 = tile * CC + idx % CC;
+    Bt[idx] = cis_frac(((unsigned)na * jb * kk2 + jb * rot) & nmask, a.log_n);
+  }
+  const double c0 = m->c0, c2 = m->c2, c3 = m->c3, c4 = m->c4;
+  for (int idx = tid; idx < R * CC; idx += 256) {
+    const int k = ((row_lo + idx / CC) << kLogN2) + tile * CC + idx % CC;
+    float2 q = make_float2(0.f, 0.f);
+    if (k >= e_lo && k < e_hi) {
+      // correlate: template phasor times weighted data bin (Eq. 1 integrand)
+      const double u = a.u_tab[k];
+      double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
+      t -= rint(t);
+      float sn, cs;
+      sincospif(2.0f * (float)t, &sn, &cs);
+      q = cmul(a.wq[k], make_float2(cs, sn));
+    }
+    E[idx] = q;
+  }
+  __syncthreads();
+  const float2 A = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
+  if (R <= 8) narrow_body<8, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
+  else if (R <= 16) narrow_body<16, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
+  else narrow_body<32, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
+}
+
+template <int CJ>
+static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
+  constexpr int CC = 256 / CJ;
+  const size_t smem = (size_t)(64 * CC) * sizeof(float2);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_narrow<CJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid((kN2 / CC) * (c->na / CJ), c->prm.p, batch);
+  k_pass1_narrow<CJ><<<grid, 256, smem, c->stream>>>(args);
+  c->launches++;
+  return cudaGetLastError();
+}
+
 template <int NA, int NB, bool DENSE>
 static cudaError_t launch_p1(Ctx* c, const P1Args& args, int batch, int bands) {
   constexpr int FR = NA >= 32 ? 32 : NA;
@@ -191,6 +302,21 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
   args.p = c->prm.p;
   args.log_n = c->log_n;
   args.n1 = c->n1;
+  args.skip_narrow = 0;
+  if (c->nb == 32) {
+    // narrow bands first (most of the work), then the wide bands; each kernel skips the other's bands
+    args.skip_narrow = 1;
+    cudaError_t e;
+    switch (c->na) {
+      case 1: e = launch_narrow<1>(c, args, count); break;
+      case 2: e = launch_narrow<2>(c, args, count); break;
+      case 4: e = launch_narrow<4>(c, args, count); break;
+      case 8: e = launch_narrow<8>(c, args, count); break;
+      case 16: e = launch_narrow<16>(c, args, count); break;
+      default: e = launch_narrow<32>(c, args, count); break;
+    }
+    if (e != cudaSuccess) return e;
+  }
   return dispatch_p1<false>(c, args, count, c->prm.p);
 }
 
@@ -205,6 +331,7 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.p = 1;
   args.log_n = c->log_n;
   args.n1 = c->n1;
+  args.skip_narrow = 0;
   return dispatch_p1<true>(c, args, 1, 1);
 }
 
