@@ -1,9 +1,11 @@
 // pass2.cu -- second pass of the band inverse FFTs fused with the statistics and the trigger maxima
 // (second half of step a3, steps a4 and a5).
 //
-// One warp owns one output residue j1 and walks over the p bands.  For each band it reads the
-// contiguous 1024-point row Y_l[j1][0..1023] once (8 KB), transforms it in registers (32 x 32, one
-// transpose through a private shared-memory tile) and accumulates, per output sample it owns,
+// One warp owns one output residue j1 and walks over the p bands.  For each band the contiguous
+// 1024-point row Y_l[j1][0..1023] (8 KB) is brought into the warp's shared-memory buffer by one TMA bulk
+// copy (cp.async.bulk + mbarrier), issued one band ahead so that HBM latency hides behind the previous
+// band's arithmetic; the warp transforms it in registers (32 x 32, one transpose through the same,
+// XOR-swizzled buffer) and accumulates, per output sample it owns,
 //     z   = sum_l z_l            (Sigma_l z_l = z: no separate full-band transform)
 //     q   = sum_l |z_l|^2
 // so that rho^2 = |z|^2 / sigma^2 (Eq. 3) and chi^2 = (p/sigma^2)(q - |z|^2/p), which is Eq. 5
@@ -54,38 +56,93 @@ __device__ __forceinline__ void slot_max(Slot* s, unsigned long long key, unsign
   }
 }
 
+// ---- TMA (bulk async copy) + mbarrier helpers --------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  unsigned ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// one contiguous row global -> shared, completion signalled on the mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_load_row(void* dst, const void* src, unsigned bytes, unsigned long long* bar,
+                                              unsigned long long policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+
+constexpr int kRowBytes = kN2 * (int)sizeof(float2);      // 8 KB
+
+// Shared memory: [tw 32x32][warp 0: buf0, buf1][warp 1: ...]...[mbarriers 2 per warp].
+// A warp's current input buffer doubles as its transpose tile (XOR-swizzled, so no padding is needed).
 template <bool STORE>
 __global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
-  extern __shared__ float2 smem2[];
-  float2* tw_s = smem2;                       // [32][32]
-
+  extern __shared__ __align__(128) float2 smem2[];
+  float2* tw_s = smem2;                                   // [32][32]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
-  __syncthreads();
+  float2* bufs = smem2 + 1024 + warp * (2 * kN2);         // two 1024-point row buffers
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * 2 * kN2) + 2 * warp;
 
   const int j1 = blockIdx.x * kP2Warps + warp;
   const int tb = blockIdx.y;
-  float2* my = smem2 + 1024 + warp * (32 * 33);   // private transpose tile, row stride 33
+  const int p = a.p;
+  const float2* row0 = a.y + ((size_t)(tb * p) * a.n1 + j1) * kN2;
+  const size_t band_stride = (size_t)a.n1 * kN2;
+
+  unsigned long long policy;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+  if (lane == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_expect_tx(&bars[0], kRowBytes);
+    bulk_load_row(bufs, row0, kRowBytes, &bars[0], policy);
+  }
+  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
+  __syncthreads();
 
   float2 az[32];
   float aq[32];
 #pragma unroll
   for (int i = 0; i < 32; ++i) { az[i] = make_float2(0.f, 0.f); aq[i] = 0.f; }
 
-  const int p = a.p;
 #pragma unroll 1
   for (int l = 0; l < p; ++l) {
-    const float2* row = a.y + ((size_t)(tb * p + l) * a.n1 + j1) * kN2;
+    float2* cur = bufs + (l & 1) * kN2;
+    if (l + 1 < p && lane == 0) {
+      // the other buffer was last touched (generic proxy) in iteration l-1: order that before the async write
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(&bars[(l + 1) & 1], kRowBytes);
+      bulk_load_row(bufs + ((l + 1) & 1) * kN2, row0 + (size_t)(l + 1) * band_stride, kRowBytes, &bars[(l + 1) & 1], policy);
+    }
+    mbar_wait(&bars[l & 1], (l >> 1) & 1);
     float2 x[32];
 #pragma unroll
-    for (int m = 0; m < 32; ++m) x[m] = __ldcs(row + 32 * m + lane);      // k2 = 32 m + lane; streamed once
+    for (int m = 0; m < 32; ++m) x[m] = cur[32 * m + lane];               // k2 = 32 m + lane
+    __syncwarp();
     fft_dif<32>(x);                                                       // over m -> jm
 #pragma unroll
     for (int jm = 0; jm < 32; ++jm)
-      my[jm * 33 + lane] = cmul(x[brev<32>(jm)], tw_s[jm * 32 + lane]);   // times e^{2 pi i jm c/1024}
+      cur[jm * 32 + (lane ^ jm)] = cmul(x[brev<32>(jm)], tw_s[jm * 32 + lane]);   // times e^{2 pi i jm c/1024}
     __syncwarp();
 #pragma unroll
-    for (int cc = 0; cc < 32; ++cc) x[cc] = my[lane * 33 + cc];           // now lane = jm, index = c
+    for (int cc = 0; cc < 32; ++cc) x[cc] = cur[lane * 32 + (cc ^ lane)];   // now lane = jm, index = c
     __syncwarp();
     fft_dif<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
     if constexpr (STORE) {
@@ -127,7 +184,7 @@ __global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
   }
 }
 
-constexpr size_t kP2Smem = (1024 + kP2Warps * 32 * 33) * sizeof(float2);
+constexpr size_t kP2Smem = (1024 + kP2Warps * 2 * kN2) * sizeof(float2) + kP2Warps * 2 * sizeof(unsigned long long);
 
 static cudaError_t p2_configure() {
   static bool done = false;
