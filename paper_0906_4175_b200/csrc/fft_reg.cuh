@@ -96,4 +96,82 @@ __device__ __forceinline__ void fft_dif(float2 (&x)[R]) {
   DifStages<R, R / 2>::run(x);
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// Decimation in time, radix 2, FMA form.  Input in bit-reversed order (x[brev<R>(n)] = input n), output
+// in natural order (X[k] = x[k]).  A butterfly with a general twiddle w costs 6 FMAs instead of the
+// 8 operations of the multiply-then-add form:  t = a + w b  (4 FMA),  u = 2 a - t  (2 FMA).
+// NZ < R declares that only inputs n < NZ are non-zero: their bit-reversed positions are the multiples
+// of R/NZ, the first log2(R/NZ) stages reduce to copies and are skipped.
+// ---------------------------------------------------------------------------------------------------
+template <int Q>
+__device__ __forceinline__ void bfly_w32(float2& a, float2& b) {
+  constexpr int q = Q & 31;
+  if constexpr (q == 0) {
+    const float2 t = cadd(a, b), u = csub(a, b);
+    a = t; b = u;
+  } else if constexpr (q == 8) {            // w = i
+    const float2 t = make_float2(a.x - b.y, a.y + b.x), u = make_float2(a.x + b.y, a.y - b.x);
+    a = t; b = u;
+  } else if constexpr (q == 4) {            // w = (1 + i) / sqrt 2
+    constexpr float h = (float)cos32_tab(4);
+    const float s = b.x - b.y, d = b.x + b.y;
+    const float2 t = make_float2(fmaf(h, s, a.x), fmaf(h, d, a.y));
+    b = make_float2(fmaf(2.f, a.x, -t.x), fmaf(2.f, a.y, -t.y));
+    a = t;
+  } else if constexpr (q == 12) {           // w = (-1 + i) / sqrt 2
+    constexpr float h = (float)cos32_tab(4);
+    const float s = b.x + b.y, d = b.x - b.y;
+    const float2 t = make_float2(fmaf(-h, s, a.x), fmaf(h, d, a.y));
+    b = make_float2(fmaf(2.f, a.x, -t.x), fmaf(2.f, a.y, -t.y));
+    a = t;
+  } else {
+    constexpr float c = (float)cos32(q), s = (float)sin32(q);
+    const float2 t = make_float2(fmaf(c, b.x, fmaf(-s, b.y, a.x)), fmaf(c, b.y, fmaf(s, b.x, a.y)));
+    b = make_float2(fmaf(2.f, a.x, -t.x), fmaf(2.f, a.y, -t.y));
+    a = t;
+  }
+}
+
+template <int R, int H, int BASE, int M>
+struct DitInner {
+  __device__ __forceinline__ static void run(float2 (&x)[R]) {
+    if constexpr (M < H) {
+      bfly_w32<M * (16 / H)>(x[BASE + M], x[BASE + M + H]);    // W_{2H}^M = W_32^{M*16/H}, M < H <= 16: q < 16
+      DitInner<R, H, BASE, M + 1>::run(x);
+    }
+  }
+};
+template <int R, int H, int BASE>
+struct DitBlocks {
+  __device__ __forceinline__ static void run(float2 (&x)[R]) {
+    if constexpr (BASE < R) {
+      DitInner<R, H, BASE, 0>::run(x);
+      DitBlocks<R, H, BASE + 2 * H>::run(x);
+    }
+  }
+};
+template <int R, int H>
+struct DitStages {
+  __device__ __forceinline__ static void run(float2 (&x)[R]) {
+    if constexpr (H < R) {
+      DitBlocks<R, H, 0>::run(x);
+      DitStages<R, H * 2>::run(x);
+    }
+  }
+};
+
+template <int R, int NZ = R>
+__device__ __forceinline__ void fft_dit(float2 (&x)[R]) {
+  static_assert(R >= 1 && R <= 32 && (R & (R - 1)) == 0, "R must be a power of two <= 32");
+  static_assert(NZ >= 1 && NZ <= R && (NZ & (NZ - 1)) == 0, "NZ must be a power of two <= R");
+  constexpr int REP = R / NZ;                 // only positions that are multiples of REP hold data
+  if constexpr (REP > 1) {
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+      if (i % REP != 0) x[i] = x[i - i % REP];
+  }
+  DitStages<R, REP>::run(x);
+}
+
 }  // namespace gwmf

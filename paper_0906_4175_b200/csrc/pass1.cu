@@ -169,18 +169,17 @@ __device__ __forceinline__ void narrow_body(const P1Args& a, const float2* __res
   float2 v[32];
   const int n1m = a.n1 - 1;
 #pragma unroll
-  for (int i = 0; i < 32; ++i) {
-    v[i] = make_float2(0.f, 0.f);
-    if (i < RMAX) {
-      if (i < R) {
-        const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], A);      // e^{2 pi i ja k/n}, k = 1024 k1 + k2
-        v[i] = cmul(E[i * CC + c], t);
-      }
+  for (int i = 0; i < RMAX; ++i) {
+    float2 q = make_float2(0.f, 0.f);
+    if (i < R) {
+      const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], A);        // e^{2 pi i ja k/n}, k = 1024 k1 + k2
+      q = cmul(E[i * CC + c], t);
     }
+    v[brev<32>(i)] = q;
   }
-  fft_dif<32>(v);
+  fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
 #pragma unroll
-  for (int jb = 0; jb < 32; ++jb) out[(size_t)jb * row_stride] = cmul(v[brev<32>(jb)], Bt[jb * CC + c]);
+  for (int jb = 0; jb < 32; ++jb) out[(size_t)jb * row_stride] = cmul(v[jb], Bt[jb * CC + c]);
 }
 
 template <int CJ>

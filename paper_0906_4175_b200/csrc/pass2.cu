@@ -4,8 +4,8 @@
 // One warp owns one output residue j1 and walks over the p bands.  For each band the contiguous
 // 1024-point row Y_l[j1][0..1023] (8 KB) is brought into the warp's shared-memory buffer by one TMA bulk
 // copy (cp.async.bulk + mbarrier), issued one band ahead so that HBM latency hides behind the previous
-// band's arithmetic; the warp transforms it in registers (32 x 32, one transpose through the same,
-// XOR-swizzled buffer) and accumulates, per output sample it owns,
+// band's arithmetic; the warp transforms it in registers (32 x 32, one transpose through the same
+// buffer, re-read with row stride 33) and accumulates, per output sample it owns,
 //     z   = sum_l z_l            (Sigma_l z_l = z: no separate full-band transform)
 //     q   = sum_l |z_l|^2
 // so that rho^2 = |z|^2 / sigma^2 (Eq. 3) and chi^2 = (p/sigma^2)(q - |z|^2/p), which is Eq. 5
@@ -87,16 +87,17 @@ __device__ __forceinline__ void bulk_load_row(void* dst, const void* src, unsign
 }
 
 constexpr int kRowBytes = kN2 * (int)sizeof(float2);      // 8 KB
+constexpr int kBufElems = 32 * 33;                        // row buffer, also the stride-33 transpose tile
 
 // Shared memory: [tw 32x32][warp 0: buf0, buf1][warp 1: ...]...[mbarriers 2 per warp].
-// A warp's current input buffer doubles as its transpose tile (XOR-swizzled, so no padding is needed).
+// A warp's current input buffer doubles as its transpose tile (row stride 33 -> conflict-free both ways).
 template <bool STORE>
 __global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
   extern __shared__ __align__(128) float2 smem2[];
   float2* tw_s = smem2;                                   // [32][32]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float2* bufs = smem2 + 1024 + warp * (2 * kN2);         // two 1024-point row buffers
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * 2 * kN2) + 2 * warp;
+  float2* bufs = smem2 + 1024 + warp * (2 * kBufElems);   // two row buffers
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * 2 * kBufElems) + 2 * warp;
 
   const int j1 = blockIdx.x * kP2Warps + warp;
   const int tb = blockIdx.y;
@@ -124,35 +125,35 @@ __global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
 
 #pragma unroll 1
   for (int l = 0; l < p; ++l) {
-    float2* cur = bufs + (l & 1) * kN2;
+    float2* cur = bufs + (l & 1) * kBufElems;
     if (l + 1 < p && lane == 0) {
       // the other buffer was last touched (generic proxy) in iteration l-1: order that before the async write
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_expect_tx(&bars[(l + 1) & 1], kRowBytes);
-      bulk_load_row(bufs + ((l + 1) & 1) * kN2, row0 + (size_t)(l + 1) * band_stride, kRowBytes, &bars[(l + 1) & 1], policy);
+      bulk_load_row(bufs + ((l + 1) & 1) * kBufElems, row0 + (size_t)(l + 1) * band_stride, kRowBytes, &bars[(l + 1) & 1], policy);
     }
     mbar_wait(&bars[l & 1], (l >> 1) & 1);
     float2 x[32];
 #pragma unroll
-    for (int m = 0; m < 32; ++m) x[m] = cur[32 * m + lane];               // k2 = 32 m + lane
+    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cur[32 * m + lane];     // k2 = 32 m + lane
     __syncwarp();
-    fft_dif<32>(x);                                                       // over m -> jm
+    fft_dit<32>(x);                                                       // over m -> jm
 #pragma unroll
     for (int jm = 0; jm < 32; ++jm)
-      cur[jm * 32 + (lane ^ jm)] = cmul(x[brev<32>(jm)], tw_s[jm * 32 + lane]);   // times e^{2 pi i jm c/1024}
+      cur[jm * 33 + lane] = cmul(x[jm], tw_s[jm * 32 + lane]);   // times e^{2 pi i jm c/1024}
     __syncwarp();
 #pragma unroll
-    for (int cc = 0; cc < 32; ++cc) x[cc] = cur[lane * 32 + (cc ^ lane)];   // now lane = jm, index = c
+    for (int cc = 0; cc < 32; ++cc) x[brev<32>(cc)] = cur[lane * 33 + cc];   // now lane = jm, index = c
     __syncwarp();
-    fft_dif<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
+    fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
     if constexpr (STORE) {
 #pragma unroll
       for (int jc = 0; jc < 32; ++jc)
-        a.dense_out[(size_t)j1 + ((size_t)(lane + 32 * jc) << a.log_n1)] = x[brev<32>(jc)];
+        a.dense_out[(size_t)j1 + ((size_t)(lane + 32 * jc) << a.log_n1)] = x[jc];
     } else {
 #pragma unroll
       for (int jc = 0; jc < 32; ++jc) {
-        const float2 z = x[brev<32>(jc)];
+        const float2 z = x[jc];
         az[jc] = cadd(az[jc], z);
         aq[jc] = fmaf(z.x, z.x, fmaf(z.y, z.y, aq[jc]));
       }
@@ -184,7 +185,7 @@ __global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
   }
 }
 
-constexpr size_t kP2Smem = (1024 + kP2Warps * 2 * kN2) * sizeof(float2) + kP2Warps * 2 * sizeof(unsigned long long);
+constexpr size_t kP2Smem = (1024 + kP2Warps * 2 * kBufElems) * sizeof(float2) + kP2Warps * 2 * sizeof(unsigned long long);
 
 static cudaError_t p2_configure() {
   static bool done = false;
