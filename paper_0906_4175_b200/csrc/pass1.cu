@@ -183,7 +183,7 @@ __device__ __forceinline__ void narrow_body(const P1Args& a, const float2* __res
 }
 
 template <int CJ>
-__global__ void __launch_bounds__(256, 2) k_pass1_narrow(P1Args a) {
+__global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   constexpr int CC = 256 / CJ;
   extern __shared__ float2 smem[];
   float2* Bt = smem;              // [32][CC]  e^{2 pi i (NA jb k2/n + jb b0/32)}
@@ -234,7 +234,8 @@ __global__ void __launch_bounds__(256, 2) k_pass1_narrow(P1Args a) {
   }
   __syncthreads();
   const float2 A = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
-  if (R <= 8) narrow_body<8, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
+  if (R <= 4) narrow_body<4, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
+  else if (R <= 8) narrow_body<8, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
   else if (R <= 16) narrow_body<16, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
   else narrow_body<32, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
 }
