@@ -35,11 +35,26 @@ __host__ __device__ constexpr int brev(int k) {
   return r;
 }
 
+// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2 work on an aligned register pair) ------------
+// A complex number (re, im) is one packed operand, so a complex add is ONE instruction and a butterfly with
+// a general twiddle THREE (see bfly_w32).  ptxas folds the half swap (.LO_HI), the negation of one half
+// (.NP) and of both halves into operand modifiers, and takes compile-time constants as immediates.  The
+// FMA pipe does the same work per flop as with scalar FFMA; what is halved is the issue-slot count.
+typedef unsigned long long pk2;
+__device__ __forceinline__ pk2 pk(float lo, float hi) { pk2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ pk2 pk(float2 v) { return pk(v.x, v.y); }
+__device__ __forceinline__ float2 unpk(pk2 v) { float2 r; asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v)); return r; }
+__device__ __forceinline__ pk2 fma2(pk2 a, pk2 b, pk2 c) { pk2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ pk2 add2(pk2 a, pk2 b) { pk2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ pk2 sub2(pk2 a, pk2 b) { pk2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ pk2 mul2(pk2 a, pk2 b) { pk2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
+// a * b:  (a.x b.x, a.y b.x) + (-a.y b.y, a.x b.y)
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-  return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+  return unpk(fma2(pk(b.y, b.y), pk(-a.y, a.x), mul2(pk(b.x, b.x), pk(a))));
 }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return unpk(add2(pk(a), pk(b))); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return unpk(sub2(pk(a), pk(b))); }
 
 // d * e^{+2 pi i Q/32} with Q a compile-time constant
 template <int Q>
@@ -55,7 +70,7 @@ __device__ __forceinline__ float2 mul_w32(float2 d) {
   else if constexpr (q == 28) { constexpr float h = (float)cos32_tab(4); return make_float2(h * (d.x + d.y), -h * (d.x - d.y)); }
   else {
     constexpr float c = (float)cos32(q), s = (float)sin32(q);
-    return make_float2(fmaf(d.x, c, -d.y * s), fmaf(d.x, s, d.y * c));
+    return unpk(fma2(pk(-s, s), pk(d.y, d.x), mul2(pk(c, c), pk(d))));
   }
 }
 
@@ -100,7 +115,8 @@ __device__ __forceinline__ void fft_dif(float2 (&x)[R]) {
 // ---------------------------------------------------------------------------------------------------
 // Decimation in time, radix 2, FMA form.  Input in bit-reversed order (x[brev<R>(n)] = input n), output
 // in natural order (X[k] = x[k]).  A butterfly with a general twiddle w costs 6 FMAs instead of the
-// 8 operations of the multiply-then-add form:  t = a + w b  (4 FMA),  u = 2 a - t  (2 FMA).
+// 8 operations of the multiply-then-add form:  t = a + w b  (4 FMA),  u = 2 a - t  (2 FMA); packed as
+// fp32x2 that is 3 instructions, and 2 for the trivial twiddles 1 and i.
 // NZ < R declares that only inputs n < NZ are non-zero: their bit-reversed positions are the multiples
 // of R/NZ, the first log2(R/NZ) stages reduce to copies and are skipped.
 // ---------------------------------------------------------------------------------------------------
@@ -110,26 +126,16 @@ __device__ __forceinline__ void bfly_w32(float2& a, float2& b) {
   if constexpr (q == 0) {
     const float2 t = cadd(a, b), u = csub(a, b);
     a = t; b = u;
-  } else if constexpr (q == 8) {            // w = i
-    const float2 t = make_float2(a.x - b.y, a.y + b.x), u = make_float2(a.x + b.y, a.y - b.x);
-    a = t; b = u;
-  } else if constexpr (q == 4) {            // w = (1 + i) / sqrt 2
-    constexpr float h = (float)cos32_tab(4);
-    const float s = b.x - b.y, d = b.x + b.y;
-    const float2 t = make_float2(fmaf(h, s, a.x), fmaf(h, d, a.y));
-    b = make_float2(fmaf(2.f, a.x, -t.x), fmaf(2.f, a.y, -t.y));
-    a = t;
-  } else if constexpr (q == 12) {           // w = (-1 + i) / sqrt 2
-    constexpr float h = (float)cos32_tab(4);
-    const float s = b.x + b.y, d = b.x - b.y;
-    const float2 t = make_float2(fmaf(-h, s, a.x), fmaf(h, d, a.y));
-    b = make_float2(fmaf(2.f, a.x, -t.x), fmaf(2.f, a.y, -t.y));
-    a = t;
-  } else {
+  } else if constexpr (q == 8) {            // w = i:  t = a + (-b.y, b.x),  u = a + (b.y, -b.x)
+    const pk2 t = add2(pk(a), pk(-b.y, b.x)), u = add2(pk(a), pk(b.y, -b.x));
+    a = unpk(t); b = unpk(u);
+  } else {                                  // t = a + c b + s (-b.y, b.x);  u = 2 a - t
     constexpr float c = (float)cos32(q), s = (float)sin32(q);
-    const float2 t = make_float2(fmaf(c, b.x, fmaf(-s, b.y, a.x)), fmaf(c, b.y, fmaf(s, b.x, a.y)));
-    b = make_float2(fmaf(2.f, a.x, -t.x), fmaf(2.f, a.y, -t.y));
-    a = t;
+    pk2 t = fma2(pk(c, c), pk(b), pk(a));
+    t = fma2(pk(-s, s), pk(b.y, b.x), t);
+    const float2 tt = unpk(t);
+    b = unpk(fma2(pk(2.f, 2.f), pk(a), pk(-tt.x, -tt.y)));
+    a = tt;
   }
 }
 
