@@ -64,8 +64,8 @@ typedef struct {
   double  rho_thresh;    /* SNR threshold, strict '>'                                             */
   int32_t window;        /* W: trigger window in samples, power of two, divides n                 */
   int32_t max_templates; /* capacity of the bank                                                  */
-  int32_t batch;         /* templates filtered per kernel launch (0 = library default); sizes the
-                            band-intermediate buffer: batch * p * n * 8 bytes                     */
+  int32_t batch;         /* templates filtered per kernel launch, 0 .. 64 (0 = library default); sizes
+                            the band-intermediate buffer: batch * p * n * 8 bytes                  */
 } gwmf_params;
 
 /* Bytes of DEVICE memory the caller must provide to gwmf_create (0 if params are invalid). */

@@ -23,7 +23,7 @@ bool params_ok(const gwmf_params* p) {
   if (p->p < 1 || p->p > kMaxBands) return false;
   if (!is_pow2(p->window) || p->window > p->n) return false;
   if (p->max_templates < 1) return false;
-  if (p->batch < 0) return false;
+  if (p->batch < 0 || p->batch > kMaxBatch) return false;
   if (!(p->rho_thresh >= 0.0)) return false;
   return true;
 }
@@ -34,7 +34,7 @@ int default_batch(const gwmf_params* p) {
   double per = (double)p->p * (double)p->n * 8.0;
   int b = (int)(1073741824.0 / per);
   if (b < 1) b = 1;
-  if (b > 64) b = 64;
+  if (b > kMaxBatch) b = kMaxBatch;
   if (b > p->max_templates) b = p->max_templates;
   return b;
 }
@@ -145,6 +145,7 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->df = params->fs / (double)params->n;
   c->k_low = (int)ceil(params->f_low / c->df);
   c->n_windows = (int)(c->n / params->window);
+  c->n_sms = prop.multiProcessorCount;
   c->lay = L;
   c->ws = (char*)d_workspace;
   c->stream = (cudaStream_t)cuda_stream;

@@ -22,7 +22,7 @@ struct TemplateMeta {
   float scale_rho2;              // (sigma_ref / sigma)^2: rho^2 = |z_scaled|^2 * scale_rho2
   int32_t k_high;                // first bin above the template
   int32_t edges[kMaxBands + 1];  // band l = bins [edges[l], edges[l+1])
-  int32_t pad_;
+  uint32_t wide_mask;            // bit l: band l goes through the generic pass-1 kernel (> 32 input rows)
 };
 
 // One (template, window) trigger slot, updated with a 128-bit compare-and-swap.
@@ -35,7 +35,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, y, total;
+         series_rho, series_chi, flags, q, y, total;
   size_t y_bytes;
   int batch;
 };
@@ -48,6 +48,7 @@ struct Ctx {
   int na, nb;                    // n1 = na * nb (pass-1 stage radices)
   int k_low;
   int n_windows;
+  int n_sms;                     // multiprocessors of the device (persistent-kernel grid size)
   double df;
   Layout lay;
   char* ws;
@@ -65,15 +66,41 @@ cudaError_t launch_segment_prepare(Ctx* c);                       // after s/Sn 
 cudaError_t launch_bank_setup(Ctx* c);
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count);
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
+cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid);
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,
                                 float* series_chi);
 cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out);
 inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, float2* d_out) {
   cudaError_t e = launch_pass1_dense(c, d_in, d_mid);
+  if (e == cudaSuccess) e = launch_rowstage_dense(c, d_mid);
   return e != cudaSuccess ? e : launch_pass2_dense(c, d_mid, d_out);
 }
 cudaError_t launch_reset_slots(Ctx* c, int first, int count);
 cudaError_t launch_compact(Ctx* c);
+
+// The (template, band) pairs of a batch whose bit is set in TemplateMeta::wide_mask, as band indices
+// tb * p + l in ascending order, identical in every CTA (so that CTAs can split the list by position).
+// s_list: batch * p ints, s_cnt: batch + 1 ints of shared memory.  Returns the list length.
+#ifdef __CUDACC__
+__device__ inline int build_wide_list(const TemplateMeta* meta, int batch, int p, int* s_list, int* s_cnt) {
+  for (int t = threadIdx.x; t < batch; t += blockDim.x) s_cnt[t] = __popc(meta[t].wide_mask);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int run = 0;
+    for (int t = 0; t < batch; ++t) { const int v = s_cnt[t]; s_cnt[t] = run; run += v; }
+    s_cnt[batch] = run;
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < batch; t += blockDim.x) {
+    unsigned m = meta[t].wide_mask;
+    int o = s_cnt[t];
+    while (m) { const int l = __ffs(m) - 1; m &= m - 1; s_list[o++] = t * p + l; }
+  }
+  __syncthreads();
+  return s_cnt[batch];
+}
+#endif
+constexpr int kMaxBatch = 64;    // templates per launch (bounds the shared-memory band list)
 
 template <typename T>
 inline T* ws_ptr(Ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }

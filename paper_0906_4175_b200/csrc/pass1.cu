@@ -25,7 +25,7 @@ struct P1Args {
   int p;
   int log_n;
   int n1;
-  int skip_narrow;            // generic kernel: leave bands of <= 32 rows to k_pass1_narrow
+  int batch;                  // templates in this launch
 };
 
 __device__ __forceinline__ float2 cis_frac(unsigned num, int log_n) {
@@ -43,110 +43,152 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
   constexpr int NGROUPS = NA / GA;
   constexpr int C = kColsPerCta;
   constexpr int SROW = NB * C + C;              // padded stride of S[m][..] in float2
+  constexpr int TILES = kN2 / C;
 
   extern __shared__ float2 smem[];
   float2* S = smem;                             // [FR][SROW]
   float2* A = S + FR * SROW;                    // [FR][C]   e^{2 pi i ja k2/n}
   float2* Bt = A + FR * C;                      // [NB][C]   e^{2 pi i NA jb k2/n}
+  __shared__ int s_list[DENSE ? 1 : kMaxBatch * kMaxBands];
+  __shared__ int s_cnt[kMaxBatch + 1];
+
+  // work list: the wide bands of the batch (DENSE: the one dense transform); every CTA builds the same list
+  int n_list = 1;
+  if constexpr (!DENSE) n_list = build_wide_list(a.meta, a.batch, a.p, s_list, s_cnt);
 
   const int tid = threadIdx.x;
   const int x = tid >> 3, c = tid & 7;
-  const int k2 = blockIdx.x * C + c;
-  const int l = blockIdx.y;
-  const int tb = blockIdx.z / G, r = blockIdx.z % G;
   const unsigned nmask = (1u << a.log_n) - 1u;
   const int n1 = a.n1;
+  const int n_items = n_list * TILES * G;
 
-  int e_lo, e_hi;
-  double c0 = 0, c2 = 0, c3 = 0, c4 = 0;
-  if constexpr (DENSE) {
-    e_lo = 0;
-    e_hi = 1 << a.log_n;
-  } else {
-    const TemplateMeta* m = a.meta + tb;
-    e_lo = m->edges[l];
-    e_hi = m->edges[l + 1];
-    c0 = m->c0; c2 = m->c2; c3 = m->c3; c4 = m->c4;
-  }
-  // rows and a-range touched by the band (uniform over the CTA)
-  const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
-  const int a_lo = row_lo / NB, a_hi = (e_hi > e_lo) ? row_hi / NB : -1;
-  if constexpr (!DENSE && NB == 32) {
-    // bands of at most 32 rows (and empty bands) belong to k_pass1_narrow
-    if (a.skip_narrow && (e_hi <= e_lo || row_hi - row_lo + 1 <= 32)) return;
-  }
-
-  if (x < FR) A[x * C + c] = cis_frac(((unsigned)((G * x + r) * k2)) & nmask, a.log_n);
-  if (x < NB) Bt[x * C + c] = cis_frac(((unsigned)(NA * x) * (unsigned)k2) & nmask, a.log_n);
-  __syncthreads();
-
-  // ------------------------------------------------------------------ stage 1: thread (b = x, c)
-  if (x < NB) {
-    const int b = x;
-    float2 acc[FR];
-#pragma unroll
-    for (int m = 0; m < FR; ++m) acc[m] = make_float2(0.f, 0.f);
 #pragma unroll 1
-    for (int g = 0; g < NGROUPS; ++g) {
-      const int a_base = GA * g;
-      if (a_base > a_hi || a_base + GA - 1 < a_lo) continue;
-      float2 xin[FR];
+  for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const int tile = item % TILES, r = (item / TILES) % G;
+    const int band_index = DENSE ? 0 : s_list[item / (TILES * G)];      // tb * p + l
+    const int k2 = tile * C + c;
+
+    int e_lo, e_hi;
+    double c0 = 0, c2 = 0, c3 = 0, c4 = 0;
+    if constexpr (DENSE) {
+      e_lo = 0;
+      e_hi = 1 << a.log_n;
+    } else {
+      const int tb = band_index / a.p, l = band_index - tb * a.p;
+      const TemplateMeta* m = a.meta + tb;
+      e_lo = m->edges[l];
+      e_hi = m->edges[l + 1];
+      c0 = m->c0; c2 = m->c2; c3 = m->c3; c4 = m->c4;
+    }
+    // rows and a-range touched by the band (uniform over the CTA)
+    const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
+    const int a_lo = row_lo / NB, a_hi = (e_hi > e_lo) ? row_hi / NB : -1;
+
+    if (x < FR) A[x * C + c] = cis_frac(((unsigned)((G * x + r) * k2)) & nmask, a.log_n);
+    if (x < NB) Bt[x * C + c] = cis_frac(((unsigned)(NA * x) * (unsigned)k2) & nmask, a.log_n);
+    __syncthreads();
+
+    // ---------------------------------------------------------------- stage 1: thread (b = x, c)
+    if (x < NB) {
+      const int b = x;
+      float2 acc[FR];
 #pragma unroll
-      for (int ap = 0; ap < FR; ++ap) {
-        float2 q = make_float2(0.f, 0.f);
-        if (ap < GA) {
-          const int aa = a_base + ap;
-          const int k = ((NB * aa + b) << kLogN2) + k2;
-          if (aa >= a_lo && aa <= a_hi && k >= e_lo && k < e_hi) {
-            if constexpr (DENSE) {
-              q = a.dense_in[k];
-            } else {
-              // correlate: template phasor times weighted data bin (Eq. 1 integrand)
-              const double u = a.u_tab[k];
-              double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
-              t -= rint(t);
-              float sn, cs;
-              sincospif(2.0f * (float)t, &sn, &cs);
-              q = cmul(a.wq[k], make_float2(cs, sn));
-            }
-            if constexpr (G > 1) {
-              if (r > 0) q = cmul(q, a.tw_n1[(r * ap * NB) % n1]);       // w_NA^{r a'}
+      for (int m = 0; m < FR; ++m) acc[m] = make_float2(0.f, 0.f);
+#pragma unroll 1
+      for (int g = 0; g < NGROUPS; ++g) {
+        const int a_base = GA * g;
+        if (a_base > a_hi || a_base + GA - 1 < a_lo) continue;
+        float2 xin[FR];
+#pragma unroll
+        for (int ap = 0; ap < FR; ++ap) {
+          float2 q = make_float2(0.f, 0.f);
+          if (ap < GA) {
+            const int aa = a_base + ap;
+            const int k = ((NB * aa + b) << kLogN2) + k2;
+            if (aa >= a_lo && aa <= a_hi && k >= e_lo && k < e_hi) {
+              if constexpr (DENSE) {
+                q = a.dense_in[k];
+              } else {
+                // correlate: template phasor times weighted data bin (Eq. 1 integrand)
+                const double u = a.u_tab[k];
+                double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
+                t -= rint(t);
+                float sn, cs;
+                sincospif(2.0f * (float)t, &sn, &cs);
+                q = cmul(a.wq[k], make_float2(cs, sn));
+              }
+              if constexpr (G > 1) {
+                if (r > 0) q = cmul(q, a.tw_n1[(r * ap * NB) % n1]);       // w_NA^{r a'}
+              }
             }
           }
+          xin[ap] = q;
         }
-        xin[ap] = q;
+        fft_dif<FR>(xin);
+#pragma unroll
+        for (int m = 0; m < FR; ++m) {
+          float2 v = xin[brev<FR>(m)];
+          if constexpr (NGROUPS > 1) {
+            if (g > 0) v = cmul(v, a.tw_n1[(a_base * (G * m + r) * NB) % n1]);   // w_NA^{a_base ja}
+          }
+          acc[m] = cadd(acc[m], v);
+        }
       }
-      fft_dif<FR>(xin);
 #pragma unroll
       for (int m = 0; m < FR; ++m) {
-        float2 v = xin[brev<FR>(m)];
-        if constexpr (NGROUPS > 1) {
-          if (g > 0) v = cmul(v, a.tw_n1[(a_base * (G * m + r) * NB) % n1]);   // w_NA^{a_base ja}
-        }
-        acc[m] = cadd(acc[m], v);
+        const int ja = G * m + r;
+        const float2 tw = cmul(a.tw_n1[(ja * b) % n1], A[m * C + c]);   // e^{2 pi i ja (1024 b + k2)/n}
+        S[m * SROW + b * C + c] = cmul(acc[m], tw);
       }
     }
-#pragma unroll
-    for (int m = 0; m < FR; ++m) {
-      const int ja = G * m + r;
-      const float2 tw = cmul(a.tw_n1[(ja * b) % n1], A[m * C + c]);   // e^{2 pi i ja (1024 b + k2)/n}
-      S[m * SROW + b * C + c] = cmul(acc[m], tw);
-    }
-  }
-  __syncthreads();
+    __syncthreads();
 
-  // ------------------------------------------------------------------ stage 2: thread (m = x, c)
-  if (x < FR) {
-    const int m = x;
-    float2 v[NB];
+    // ---------------------------------------------------------------- stage 2: thread (m = x, c)
+    if (x < FR) {
+      const int m = x;
+      float2 v[NB];
 #pragma unroll
-    for (int b = 0; b < NB; ++b) v[b] = S[m * SROW + b * C + c];
-    fft_dif<NB>(v);
-    const int band_index = DENSE ? 0 : (tb * a.p + l);
-    float2* out = a.y + ((size_t)band_index * n1 + (size_t)(G * m + r)) * kN2 + k2;
+      for (int b = 0; b < NB; ++b) v[b] = S[m * SROW + b * C + c];
+      fft_dif<NB>(v);
+      float2* out = a.y + ((size_t)band_index * n1 + (size_t)(G * m + r)) * kN2 + k2;
 #pragma unroll
-    for (int jb = 0; jb < NB; ++jb)
-      out[(size_t)jb * NA * kN2] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
+      for (int jb = 0; jb < NB; ++jb)
+        out[(size_t)jb * NA * kN2] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
+    }
+    __syncthreads();                            // S, A, Bt are rewritten by the next item
+  }
+}
+
+
+// ---------------------------------------------------------------------------------------------------
+// Row stage for the rows written by k_pass1 in the plain layout Y[j1][k2]: first 32-point stage of the
+// 1024-point row transform plus its twiddle, in place,
+//     A[j1][c][jm] = e^{2 pi i jm c/1024} sum_m e^{2 pi i jm m/32} Y[j1][32 m + c],
+// which is the layout pass 2 reads (k_pass1_narrow writes it directly).  One warp per row; only the
+// bands in the wide list (or every band if use_mask == 0: small n, dense transform) are touched.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const float2* __restrict__ tw_p2,
+                                                  const TemplateMeta* __restrict__ meta, int batch, int p, int log_n1,
+                                                  int n_bands_all, int use_mask) {
+  __shared__ int s_list[kMaxBatch * kMaxBands];
+  __shared__ int s_cnt[kMaxBatch + 1];
+  const int n_list = use_mask ? build_wide_list(meta, batch, p, s_list, s_cnt) : n_bands_all;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long total_rows = (long long)n_list << log_n1;
+  for (long long row = (long long)blockIdx.x * 8 + warp; row < total_rows; row += (long long)gridDim.x * 8) {
+    const int w = (int)(row >> log_n1), j1 = (int)(row & ((1 << log_n1) - 1));
+    const int band = use_mask ? s_list[w] : w;
+    float2* Y = y + (((size_t)band << log_n1) + (size_t)j1) * kN2;
+    float2 x[32];
+#pragma unroll
+    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = Y[32 * m + lane];       // lane = c
+    fft_dit<32>(x);                                                        // over m -> jm
+#pragma unroll
+    for (int jm = 0; jm < 32; ++jm) x[jm] = cmul(x[jm], tw_p2[jm * 32 + lane]);
+    __syncwarp();                                                          // the whole row is in registers
+    float4* out = reinterpret_cast<float4*>(Y + 32 * lane);
+#pragma unroll
+    for (int jm = 0; jm < 32; jm += 2) out[jm >> 1] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
   }
 }
 
@@ -257,9 +299,8 @@ static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
 }
 
 template <int NA, int NB, bool DENSE>
-static cudaError_t launch_p1(Ctx* c, const P1Args& args, int batch, int bands) {
+static cudaError_t launch_p1(Ctx* c, const P1Args& args) {
   constexpr int FR = NA >= 32 ? 32 : NA;
-  constexpr int G = NA / FR;
   constexpr int SROW = NB * kColsPerCta + kColsPerCta;
   const size_t smem = (size_t)(FR * SROW + FR * kColsPerCta + NB * kColsPerCta) * sizeof(float2);
   static bool configured = false;
@@ -268,27 +309,34 @@ static cudaError_t launch_p1(Ctx* c, const P1Args& args, int batch, int bands) {
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid(kN2 / kColsPerCta, bands, batch * G);
-  k_pass1<NA, NB, DENSE><<<grid, 256, smem, c->stream>>>(args);
+  // persistent over the work list; a CTA with nothing to do exits after building the (empty) list
+  k_pass1<NA, NB, DENSE><<<2 * c->n_sms, 256, smem, c->stream>>>(args);
   c->launches++;
   return cudaGetLastError();
 }
 
 template <bool DENSE>
-static cudaError_t dispatch_p1(Ctx* c, const P1Args& args, int batch, int bands) {
+static cudaError_t dispatch_p1(Ctx* c, const P1Args& args) {
   switch (c->na) {
     case 1:
-      if (c->nb == 16) return launch_p1<1, 16, DENSE>(c, args, batch, bands);
-      return launch_p1<1, 32, DENSE>(c, args, batch, bands);
-    case 2: return launch_p1<2, 32, DENSE>(c, args, batch, bands);
-    case 4: return launch_p1<4, 32, DENSE>(c, args, batch, bands);
-    case 8: return launch_p1<8, 32, DENSE>(c, args, batch, bands);
-    case 16: return launch_p1<16, 32, DENSE>(c, args, batch, bands);
-    case 32: return launch_p1<32, 32, DENSE>(c, args, batch, bands);
-    case 64: return launch_p1<64, 32, DENSE>(c, args, batch, bands);
-    case 128: return launch_p1<128, 32, DENSE>(c, args, batch, bands);
+      if (c->nb == 16) return launch_p1<1, 16, DENSE>(c, args);
+      return launch_p1<1, 32, DENSE>(c, args);
+    case 2: return launch_p1<2, 32, DENSE>(c, args);
+    case 4: return launch_p1<4, 32, DENSE>(c, args);
+    case 8: return launch_p1<8, 32, DENSE>(c, args);
+    case 16: return launch_p1<16, 32, DENSE>(c, args);
+    case 32: return launch_p1<32, 32, DENSE>(c, args);
+    case 64: return launch_p1<64, 32, DENSE>(c, args);
+    case 128: return launch_p1<128, 32, DENSE>(c, args);
   }
   return cudaErrorInvalidValue;
+}
+
+static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, int batch, int n_bands_all, int use_mask) {
+  k_rowstage<<<4 * c->n_sms, 256, 0, c->stream>>>(y, ws_ptr<float2>(c, c->lay.tw_p2), meta, batch, c->prm.p,
+                                                  c->log_n - kLogN2, n_bands_all, use_mask);
+  c->launches++;
+  return cudaGetLastError();
 }
 
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
@@ -302,11 +350,10 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
   args.p = c->prm.p;
   args.log_n = c->log_n;
   args.n1 = c->n1;
-  args.skip_narrow = 0;
+  args.batch = count;
+  cudaError_t e;
   if (c->nb == 32) {
-    // narrow bands first (most of the work), then the wide bands; each kernel skips the other's bands
-    args.skip_narrow = 1;
-    cudaError_t e;
+    // narrow bands (most of the work); the wide ones follow through the generic kernel + row stage
     switch (c->na) {
       case 1: e = launch_narrow<1>(c, args, count); break;
       case 2: e = launch_narrow<2>(c, args, count); break;
@@ -317,7 +364,10 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
     }
     if (e != cudaSuccess) return e;
   }
-  return dispatch_p1<false>(c, args, count, c->prm.p);
+  e = dispatch_p1<false>(c, args);
+  if (e != cudaSuccess) return e;
+  // TRANSITION: the narrow kernel still writes the plain layout, so every band goes through the row stage
+  return launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 0);
 }
 
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
@@ -331,8 +381,10 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.p = 1;
   args.log_n = c->log_n;
   args.n1 = c->n1;
-  args.skip_narrow = 0;
-  return dispatch_p1<true>(c, args, 1, 1);
+  args.batch = 1;
+  return dispatch_p1<true>(c, args);
 }
+
+cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid) { return launch_rowstage(c, d_mid, nullptr, 1, 1, 0); }
 
 }  // namespace gwmf

@@ -1,11 +1,14 @@
-// pass2.cu -- second pass of the band inverse FFTs fused with the statistics and the trigger maxima
-// (second half of step a3, steps a4 and a5).
+// pass2.cu -- last 32-point stage of the band inverse FFTs fused with the statistics and the trigger
+// maxima (end of step a3, steps a4 and a5).
 //
-// One warp owns one output residue j1 and walks over the p bands.  For each band the contiguous
-// 1024-point row Y_l[j1][0..1023] (8 KB) is brought into the warp's shared-memory buffer by one TMA bulk
-// copy (cp.async.bulk + mbarrier), issued one band ahead so that HBM latency hides behind the previous
-// band's arithmetic; the warp transforms it in registers (32 x 32, one transpose through the same
-// buffer, re-read with row stride 33) and accumulates, per output sample it owns,
+// Index algebra (see pass1.cu): sample j = j1 + n1 (jm + 32 jc); pass 1 leaves, per band l and row j1,
+//     A_l[j1][c][jm] = e^{2 pi i jm c/1024} sum_m e^{2 pi i jm m/32} Y_l[j1][32 m + c]        (8 KB, contiguous)
+// so that        z_l[j1 + n1 (jm + 32 jc)] = sum_c e^{2 pi i jc c/32} A_l[j1][c][jm]
+// is ONE 32-point transform per thread with lane = jm: no twiddles, no transpose, no shared-memory
+// exchange.  Warps are persistent: a warp walks over rows (template, j1) and, within a row, over the p
+// bands; every 8 KB row is brought into the warp's ring of shared-memory buffers by one TMA bulk copy
+// (cp.async.bulk + mbarrier), issued kP2Ring rows ahead across band AND row boundaries, so HBM latency is
+// hidden by the ring, not by occupancy.  Per owned output sample the warp accumulates
 //     z   = sum_l z_l            (Sigma_l z_l = z: no separate full-band transform)
 //     q   = sum_l |z_l|^2
 // so that rho^2 = |z|^2 / sigma^2 (Eq. 3) and chi^2 = (p/sigma^2)(q - |z|^2/p), which is Eq. 5
@@ -19,8 +22,7 @@
 namespace gwmf {
 
 struct P2Args {
-  const float2* y;            // [batch][p][n1][1024]
-  const float2* tw_p2;        // [32][32] e^{2 pi i jm c/1024}
+  const float2* y;            // A layout: [batch][p][n1][c = 32][jm = 32]
   const TemplateMeta* meta;   // offset to first template of the batch
   Slot* slots;                // offset to first template of the batch; nullptr = do not update
   float* series_rho;          // optional: n floats (batch must be 1)
@@ -31,6 +33,7 @@ struct P2Args {
   int log_n1;
   int log_w;                  // log2(window)
   int n_windows;
+  int n_rows;                 // rows (template, j1) of this launch = batch * n1
   float thresh;
 };
 
@@ -87,69 +90,80 @@ __device__ __forceinline__ void bulk_load_row(void* dst, const void* src, unsign
 }
 
 constexpr int kRowBytes = kN2 * (int)sizeof(float2);      // 8 KB
-constexpr int kBufElems = 32 * 33;                        // row buffer, also the stride-33 transpose tile
+constexpr int kP2Ring = 3;                                // row buffers per warp
 
-// Shared memory: [tw 32x32][warp 0: buf0, buf1][warp 1: ...]...[mbarriers 2 per warp].
-// A warp's current input buffer doubles as its transpose tile (row stride 33 -> conflict-free both ways).
+// Shared memory: [warp 0: ring of kP2Ring rows][warp 1: ...]...[mbarriers, kP2Ring per warp].
 template <bool STORE>
-__global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
+__global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
   extern __shared__ __align__(128) float2 smem2[];
-  float2* tw_s = smem2;                                   // [32][32]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float2* bufs = smem2 + 1024 + warp * (2 * kBufElems);   // two row buffers
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * 2 * kBufElems) + 2 * warp;
+  float2* bufs = smem2 + warp * (kP2Ring * kN2);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + kP2Warps * kP2Ring * kN2) + kP2Ring * warp;
 
-  const int j1 = blockIdx.x * kP2Warps + warp;
-  const int tb = blockIdx.y;
   const int p = a.p;
-  const float2* row0 = a.y + ((size_t)(tb * p) * a.n1 + j1) * kN2;
+  const int total_warps = gridDim.x * kP2Warps;
+  const int first_row = blockIdx.x * kP2Warps + warp;
+  if (first_row >= a.n_rows) return;                                  // warps are independent: no CTA barrier below
+  const int my_rows = (a.n_rows - first_row + total_warps - 1) / total_warps;
+  const int n_items = my_rows * p;                                    // (row, band) pairs, band fastest
   const size_t band_stride = (size_t)a.n1 * kN2;
+  const int n1_mask = a.n1 - 1;
 
   unsigned long long policy;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
-  if (lane == 0) {
-    mbar_init(&bars[0], 1);
-    mbar_init(&bars[1], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+
+  // prefetch cursor (next item to request)
+  int pf_item = 0, pf_l = 0, pf_row = first_row;
+  auto prefetch = [&]() {
+    // caller: lane 0 only, and only after every lane has consumed the buffer being refilled
+    const int tb = pf_row >> a.log_n1, j1 = pf_row & n1_mask;
+    const float2* src = a.y + ((size_t)(tb * p + pf_l) * a.n1 + j1) * kN2;
+    const int b = pf_item % kP2Ring;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    mbar_expect_tx(&bars[0], kRowBytes);
-    bulk_load_row(bufs, row0, kRowBytes, &bars[0], policy);
+    mbar_expect_tx(&bars[b], kRowBytes);
+    bulk_load_row(bufs + b * kN2, src, kRowBytes, &bars[b], policy);
+  };
+  auto advance = [&]() {
+    ++pf_item;
+    if (++pf_l == p) { pf_l = 0; pf_row += total_warps; }
+  };
+  if (lane == 0) {
+#pragma unroll
+    for (int b = 0; b < kP2Ring; ++b) mbar_init(&bars[b], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
-  __syncthreads();
+  __syncwarp();
+#pragma unroll 1
+  for (int b = 0; b < kP2Ring && pf_item < n_items; ++b) {
+    if (lane == 0) prefetch();
+    advance();
+  }
 
   float2 az[32];
   float aq[32];
 #pragma unroll
   for (int i = 0; i < 32; ++i) { az[i] = make_float2(0.f, 0.f); aq[i] = 0.f; }
 
+  int l = 0, row = first_row;
 #pragma unroll 1
-  for (int l = 0; l < p; ++l) {
-    float2* cur = bufs + (l & 1) * kBufElems;
-    if (l + 1 < p && lane == 0) {
-      // the other buffer was last touched (generic proxy) in iteration l-1: order that before the async write
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(&bars[(l + 1) & 1], kRowBytes);
-      bulk_load_row(bufs + ((l + 1) & 1) * kBufElems, row0 + (size_t)(l + 1) * band_stride, kRowBytes, &bars[(l + 1) & 1], policy);
-    }
-    mbar_wait(&bars[l & 1], (l >> 1) & 1);
+  for (int item = 0; item < n_items; ++item) {
+    const int b = item % kP2Ring;
+    const float2* cur = bufs + b * kN2;
+    mbar_wait(&bars[b], (item / kP2Ring) & 1);
     float2 x[32];
 #pragma unroll
-    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cur[32 * m + lane];     // k2 = 32 m + lane
-    __syncwarp();
-    fft_dit<32>(x);                                                       // over m -> jm
-#pragma unroll
-    for (int jm = 0; jm < 32; ++jm)
-      cur[jm * 33 + lane] = cmul(x[jm], tw_s[jm * 32 + lane]);   // times e^{2 pi i jm c/1024}
-    __syncwarp();
-#pragma unroll
-    for (int cc = 0; cc < 32; ++cc) x[brev<32>(cc)] = cur[lane * 33 + cc];   // now lane = jm, index = c
-    __syncwarp();
+    for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cur[32 * c + lane];     // lane = jm
     fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
+    __syncwarp();                                                         // every lane holds its 32 values
+    if (pf_item < n_items) {
+      if (lane == 0) prefetch();
+      advance();
+    }
     if constexpr (STORE) {
 #pragma unroll
       for (int jc = 0; jc < 32; ++jc)
-        a.dense_out[(size_t)j1 + ((size_t)(lane + 32 * jc) << a.log_n1)] = x[jc];
+        a.dense_out[(size_t)row + ((size_t)(lane + 32 * jc) << a.log_n1)] = x[jc];
+      row += total_warps;
     } else {
 #pragma unroll
       for (int jc = 0; jc < 32; ++jc) {
@@ -157,35 +171,40 @@ __global__ void __launch_bounds__(kP2Warps * 32) k_pass2(P2Args a) {
         az[jc] = cadd(az[jc], z);
         aq[jc] = fmaf(z.x, z.x, fmaf(z.y, z.y, aq[jc]));
       }
-    }
-  }
-
-  if constexpr (!STORE) {
-    const TemplateMeta* m = a.meta + tb;
-    const float scale = m->scale_rho2;
-    const float fp = (float)p, inv_p = 1.0f / (float)p;
-    const float thr2 = a.thresh * a.thresh;
+      if (++l == p) {
+        // ---- epilogue of one row: rho, chi^2 and the trigger slots (steps a4, a5) ----
+        const int tb = row >> a.log_n1, j1 = row & n1_mask;
+        const TemplateMeta* m = a.meta + tb;
+        const float scale = m->scale_rho2;
+        const float fp = (float)p, inv_p = 1.0f / (float)p;
+        const float thr2 = a.thresh * a.thresh;
 #pragma unroll
-    for (int jc = 0; jc < 32; ++jc) {
-      const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
-      const float rho2 = z2 * scale;                                        // Eq. 3 squared
-      const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * (fp * scale);     // Eq. 5
-      const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
-      if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
-      if (a.series_chi) a.series_chi[j] = chi;
-      if (a.slots && rho2 > thr2 * 0.999f) {
-        const float rho = sqrtf(rho2);
-        if (rho > a.thresh) {
-          Slot* s = a.slots + (size_t)tb * a.n_windows + (j >> a.log_w);
-          slot_max(s, ((unsigned long long)__float_as_uint(rho) << 32) | (unsigned long long)(0xFFFFFFFFu - j),
-                   (unsigned long long)__float_as_uint(chi));
+        for (int jc = 0; jc < 32; ++jc) {
+          const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
+          const float rho2 = z2 * scale;                                        // Eq. 3 squared
+          const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * (fp * scale);     // Eq. 5
+          const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
+          if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
+          if (a.series_chi) a.series_chi[j] = chi;
+          if (a.slots && rho2 > thr2 * 0.999f) {
+            const float rho = sqrtf(rho2);
+            if (rho > a.thresh) {
+              Slot* s = a.slots + (size_t)tb * a.n_windows + (j >> a.log_w);
+              slot_max(s, ((unsigned long long)__float_as_uint(rho) << 32) | (unsigned long long)(0xFFFFFFFFu - j),
+                       (unsigned long long)__float_as_uint(chi));
+            }
+          }
+          az[jc] = make_float2(0.f, 0.f);
+          aq[jc] = 0.f;
         }
+        l = 0;
+        row += total_warps;
       }
     }
   }
 }
 
-constexpr size_t kP2Smem = (1024 + kP2Warps * 2 * kBufElems) * sizeof(float2) + kP2Warps * 2 * sizeof(unsigned long long);
+constexpr size_t kP2Smem = (size_t)kP2Warps * kP2Ring * kN2 * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
 
 static cudaError_t p2_configure() {
   static bool done = false;
@@ -196,10 +215,14 @@ static cudaError_t p2_configure() {
   return e;
 }
 
+static int p2_grid(const Ctx* c, int n_rows) {
+  const int want = (n_rows + kP2Warps - 1) / kP2Warps;
+  return want < c->n_sms ? want : c->n_sms;               // persistent: at most one CTA per SM
+}
+
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi) {
   P2Args a;
   a.y = ws_ptr<float2>(c, c->lay.y);
-  a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   a.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
   a.slots = update_slots ? ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows : nullptr;
   a.series_rho = series_rho;
@@ -212,11 +235,11 @@ cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots,
   while ((1 << lw) < c->prm.window) ++lw;
   a.log_w = lw;
   a.n_windows = c->n_windows;
+  a.n_rows = count * c->n1;
   a.thresh = (float)c->prm.rho_thresh;
-  dim3 grid(c->n1 / kP2Warps, count);
   cudaError_t e = p2_configure();
   if (e != cudaSuccess) return e;
-  k_pass2<false><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  k_pass2<false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
   c->launches++;
   return cudaGetLastError();
 }
@@ -224,7 +247,6 @@ cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots,
 cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
   P2Args a;
   a.y = d_mid;
-  a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   a.meta = nullptr;
   a.slots = nullptr;
   a.series_rho = nullptr;
@@ -235,11 +257,11 @@ cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
   a.log_n1 = c->log_n - kLogN2;
   a.log_w = 0;
   a.n_windows = 0;
+  a.n_rows = c->n1;
   a.thresh = 0.f;
-  dim3 grid(c->n1 / kP2Warps, 1);
   cudaError_t e = p2_configure();
   if (e != cudaSuccess) return e;
-  k_pass2<true><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  k_pass2<true><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
   c->launches++;
   return cudaGetLastError();
 }

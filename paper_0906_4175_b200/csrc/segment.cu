@@ -139,7 +139,7 @@ cudaError_t launch_segment_prepare(Ctx* c) {
 // One thread per template; the edges are binary searches in the monotone fp64 table.
 // ---------------------------------------------------------------------------------------------------
 __global__ void k_bank_setup(TemplateMeta* __restrict__ meta, const double* __restrict__ c_tab, int n_templates,
-                             int p, int k_low, int half_n, double four_df) {
+                             int p, int k_low, int half_n, double four_df, int all_wide) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n_templates) return;
   TemplateMeta m = meta[t];
@@ -159,13 +159,21 @@ __global__ void k_bank_setup(TemplateMeta* __restrict__ meta, const double* __re
   }
   m.edges[p] = m.k_high;
   for (int l = p + 1; l <= kMaxBands; ++l) m.edges[l] = m.k_high;
+  // bands for the generic pass-1 kernel: more than 32 input rows (or every band when n1 < 32)
+  unsigned mask = 0u;
+  for (int l = 0; l < p; ++l) {
+    const int e_lo = m.edges[l], e_hi = m.edges[l + 1];
+    const int rows = e_hi > e_lo ? ((e_hi - 1) >> kLogN2) - (e_lo >> kLogN2) + 1 : 0;
+    if (all_wide || rows > 32) mask |= 1u << l;
+  }
+  m.wide_mask = mask;
   meta[t] = m;
 }
 
 cudaError_t launch_bank_setup(Ctx* c) {
   k_bank_setup<<<(c->n_templates + 127) / 128, 128, 0, c->stream>>>(
       ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<double>(c, c->lay.c_tab), c->n_templates, c->prm.p, c->k_low,
-      (int)(c->n / 2), 4.0 * c->df);
+      (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1);
   c->launches++;
   return cudaGetLastError();
 }
