@@ -66,6 +66,7 @@ Layout make_layout(const gwmf_params* p) {
   L.series_rho = take(n * sizeof(float));
   L.series_chi = take(n * sizeof(float));
   L.flags = take(256);
+  L.q = take((size_t)L.batch * half * sizeof(float2));
   size_t yb = (size_t)L.batch * (size_t)p->p * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;

@@ -20,6 +20,8 @@ struct P1Args {
   const float2* wq;           // weighted spectrum, n/2
   const double* u_tab;        // f^(-1/3), n/2
   const float2* tw_n1;        // e^{2 pi i m/n1}
+  const float2* tw_p2;        // [32][32] e^{2 pi i a b/1024}
+  const float2* q;            // [batch][n/2] correlated spectrum Q_I[k] (k_correlate)
   const float2* dense_in;     // DENSE only: n complex inputs
   float2* y;                  // [batch][p][n1][1024]
   int p;
@@ -68,8 +70,7 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
     const int band_index = DENSE ? 0 : s_list[item / (TILES * G)];      // tb * p + l
     const int k2 = tile * C + c;
 
-    int e_lo, e_hi;
-    double c0 = 0, c2 = 0, c3 = 0, c4 = 0;
+    int e_lo, e_hi, tb_q = 0;
     if constexpr (DENSE) {
       e_lo = 0;
       e_hi = 1 << a.log_n;
@@ -78,7 +79,7 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
       const TemplateMeta* m = a.meta + tb;
       e_lo = m->edges[l];
       e_hi = m->edges[l + 1];
-      c0 = m->c0; c2 = m->c2; c3 = m->c3; c4 = m->c4;
+      tb_q = tb;
     }
     // rows and a-range touched by the band (uniform over the CTA)
     const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
@@ -109,13 +110,7 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
               if constexpr (DENSE) {
                 q = a.dense_in[k];
               } else {
-                // correlate: template phasor times weighted data bin (Eq. 1 integrand)
-                const double u = a.u_tab[k];
-                double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
-                t -= rint(t);
-                float sn, cs;
-                sincospif(2.0f * (float)t, &sn, &cs);
-                q = cmul(a.wq[k], make_float2(cs, sn));
+                q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + k];      // Q_I[k] from k_correlate
               }
               if constexpr (G > 1) {
                 if (r > 0) q = cmul(q, a.tw_n1[(r * ap * NB) % n1]);       // w_NA^{r a'}
@@ -194,106 +189,149 @@ __global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const 
 
 
 // ---------------------------------------------------------------------------------------------------
-// Narrow bands (at most 32 input rows; 15 of the 16 bands of a typical template).  With so few rows
-// stage 1 degenerates: every b = k1 mod 32 has at most one non-zero a, so V[ja][b] is a single product
-// Q[k] e^{2 pi i ja k/n} and needs neither a transform over a nor a shared-memory exchange.  A thread
-// owns (ja, column): it forms its <= 32 stage-2 inputs from the band's rows (staged once per CTA in
-// shared memory, where the template phasor is evaluated), runs the 32-point transform over b in
-// registers with the tail of zero inputs pruned at compile time, and streams out its 32 rows.
-// The rows are rotated so that the band's first row sits at b' = 0; the rotation factor
-// w_32^{jb b0} is folded into the output twiddle table.
-// CTA = CJ values of ja x CC = 256/CJ columns.
+// Correlate (step a2): Q_I[k] = w[k] e^{i Psi0_I(f_k)} for k_low <= k < k_high, once per (template, bin).
+// The phase is evaluated in fp64 (Horner in u = f^(-1/3), coefficients in turns), reduced to one turn in
+// fp64, and only then rounded to fp32 for sincospif.  Q (4 MiB per template at n = 2^20) is written once and
+// read by every ja-slice of pass 1 out of L2.
 // ---------------------------------------------------------------------------------------------------
-template <int RMAX, int CC>
-__device__ __forceinline__ void narrow_body(const P1Args& a, const float2* __restrict__ E, const float2* __restrict__ Bt,
-                                            float2 A, int R, int row_lo, int ja, int c, float2* __restrict__ out,
-                                            size_t row_stride) {
+__global__ void __launch_bounds__(256) k_correlate(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wq,
+                                                   const double* __restrict__ u_tab, float2* __restrict__ q, int half_n) {
+  const TemplateMeta* m = meta + blockIdx.y;
+  const int k = blockIdx.x * 256 + threadIdx.x;
+  if (k < m->edges[0] || k >= m->k_high) return;
+  // correlate: template phasor times weighted data bin (Eq. 1 integrand)
+  const double u = u_tab[k];
+  double t = fma(fma(fma(fma(m->c0, u * u, m->c2), u, m->c3), u, m->c4), u, -0.125);   // Psi0 / 2 pi, turns
+  t -= rint(t);
+  float sn, cs;
+  sincospif(2.0f * (float)t, &sn, &cs);
+  q[(size_t)blockIdx.y * half_n + k] = cmul(wq[k], make_float2(cs, sn));
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Narrow bands (at most 32 input rows: 99 % of the bands of the headline bank).  n1 = NA * 32, output row
+// j1 = ja + NA jb, input row k1 = 32 a + b.  With so few rows every residue b has at most one non-zero
+// input, so the transform over a degenerates to the single product Q[k] e^{2 pi i ja k/n}, and the band's
+// rows, rotated so that the first one sits at b' = 0, feed a 32-point transform over b whose zero tail is
+// pruned at compile time (RMAX = 4, 8, 16, 32).
+//
+// A CTA owns one ja and the 256 columns k2 = 32 m + c, m = 0..31, c = 8 cg .. 8 cg + 7, and runs both the
+// column transform and the first stage of the row transform (over m), so that what reaches HBM is already
+//     A[j1][c][jm] = e^{2 pi i jm c/1024} sum_m e^{2 pi i jm m/32} Y[j1][32 m + c],
+// the layout pass 2 consumes with a single 32-point transform per thread:
+//   phase 1, thread (m, ci):  v[jb] = FFT32_b( Q[k] e^{2 pi i ja k/n} ),  tile[jb][m][ci] = v[jb] e^{2 pi i jb m/1024}
+//   phase 2, thread (jb, ci): x[m] = tile[jb][m][ci] S,  S = e^{2 pi i jb (c + 1024 b0)/32768}  (the rest of the
+//                             column twiddle e^{2 pi i NA jb k2/n} and the rotation w_32^{jb b0});
+//                             X[jm] = FFT32_m(x) e^{2 pi i jm c/1024};  staged as [jb][ci][jm]
+//   store: per jb one contiguous 2 KB piece of row j1, by TMA bulk copy shared -> global.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kTileStride = 257;      // float2 per jb row of the exchange tile (conflict-free both ways)
+constexpr int kStageStride = 258;     // float2 per jb row of the store staging (16-byte aligned rows)
+
+template <int RMAX>
+__device__ __forceinline__ void narrow_phase1(const P1Args& a, const float2* __restrict__ qrow, float2* __restrict__ tile,
+                                              float2 Aja, int R, int row_lo, int e_lo, int e_hi, int ja, int k2, int m, int ci) {
   float2 v[32];
   const int n1m = a.n1 - 1;
 #pragma unroll
   for (int i = 0; i < RMAX; ++i) {
-    float2 q = make_float2(0.f, 0.f);
-    if (i < R) {
-      const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], A);        // e^{2 pi i ja k/n}, k = 1024 k1 + k2
-      q = cmul(E[i * CC + c], t);
+    float2 val = make_float2(0.f, 0.f);
+    const int k = ((row_lo + i) << kLogN2) + k2;
+    if (i < R && k >= e_lo && k < e_hi) {
+      const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], Aja);      // e^{2 pi i ja k/n}, k = 1024 k1 + k2
+      val = cmul(qrow[k], t);
     }
-    v[brev<32>(i)] = q;
+    v[brev<32>(i)] = val;
   }
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
 #pragma unroll
-  for (int jb = 0; jb < 32; ++jb) out[(size_t)jb * row_stride] = cmul(v[jb], Bt[jb * CC + c]);
+  for (int jb = 0; jb < 32; ++jb)
+    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], __ldg(&a.tw_p2[jb * 32 + m]));
 }
 
-template <int CJ>
 __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
-  constexpr int CC = 256 / CJ;
-  extern __shared__ float2 smem[];
-  float2* Bt = smem;              // [32][CC]  e^{2 pi i (NA jb k2/n + jb b0/32)}
-  float2* E = smem + 32 * CC;     // [R][CC]   Q of the band's rows, this column tile
+  extern __shared__ __align__(128) float2 smem[];
+  float2* tile = smem;                          // [32][kStageStride] (phase 1 uses stride kTileStride)
+  float2* T3 = smem + 32 * kStageStride;        // [8][32]  e^{2 pi i jm c/1024}
 
   const int tid = threadIdx.x;
-  const int c = tid % CC, x = tid / CC;
-  const int tiles = kN2 / CC;
-  const int tile = blockIdx.x % tiles, jblk = blockIdx.x / tiles;
-  const int l = blockIdx.y, tb = blockIdx.z;
   const int na = a.n1 >> 5;
-  const int ja = jblk * CJ + x;
-  const int k2 = tile * CC + c;
+  const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
+  const int l = blockIdx.y, tb = blockIdx.z;
+  const int band_index = tb * a.p + l;
   const unsigned nmask = (1u << a.log_n) - 1u;
 
-  const TemplateMeta* m = a.meta + tb;
-  const int e_lo = m->edges[l], e_hi = m->edges[l + 1];
-  float2* out = a.y + ((size_t)(tb * a.p + l) * a.n1 + (size_t)ja) * kN2 + k2;
+  const TemplateMeta* mt = a.meta + tb;
+  const int e_lo = mt->edges[l], e_hi = mt->edges[l + 1];
+  float2* out0 = a.y + ((size_t)band_index * a.n1 + (size_t)ja) * kN2 + cg * 256;   // row jb adds jb * na * 1024
   const size_t row_stride = (size_t)na * kN2;
   if (e_hi <= e_lo) {             // empty band: z_l = 0
-#pragma unroll
-    for (int jb = 0; jb < 32; ++jb) out[(size_t)jb * row_stride] = make_float2(0.f, 0.f);
+#pragma unroll 4
+    for (int jb = 0; jb < 32; ++jb) out0[(size_t)jb * row_stride + tid] = make_float2(0.f, 0.f);
     return;
   }
   const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
-  if (R > 32) return;             // wide band: k_pass1
+  if (R > 32) return;             // wide band: k_pass1 + k_rowstage
 
-  const unsigned rot = (unsigned)(row_lo & 31) << (a.log_n - 5);           // b0 * n/32
-  for (int idx = tid; idx < 32 * CC; idx += 256) {
-    const unsigned jb = idx / CC, kk2 = tile * CC + idx % CC;
-    Bt[idx] = cis_frac(((unsigned)na * jb * kk2 + jb * rot) & nmask, a.log_n);
+  {
+    const int ci = tid >> 5, jm = tid & 31;
+    T3[tid] = __ldg(&a.tw_p2[jm * 32 + 8 * cg + ci]);
   }
-  const double c0 = m->c0, c2 = m->c2, c3 = m->c3, c4 = m->c4;
-  for (int idx = tid; idx < R * CC; idx += 256) {
-    const int k = ((row_lo + idx / CC) << kLogN2) + tile * CC + idx % CC;
-    float2 q = make_float2(0.f, 0.f);
-    if (k >= e_lo && k < e_hi) {
-      // correlate: template phasor times weighted data bin (Eq. 1 integrand)
-      const double u = a.u_tab[k];
-      double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
-      t -= rint(t);
-      float sn, cs;
-      sincospif(2.0f * (float)t, &sn, &cs);
-      q = cmul(a.wq[k], make_float2(cs, sn));
-    }
-    E[idx] = q;
+  // ---- phase 1: thread (m, ci), column k2
+  {
+    const int ci = tid & 7, m = tid >> 3;
+    const int k2 = 32 * m + 8 * cg + ci;
+    const float2 Aja = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
+    const float2* qrow = a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
+    if (R <= 4) narrow_phase1<4>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    else if (R <= 8) narrow_phase1<8>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    else if (R <= 16) narrow_phase1<16>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    else narrow_phase1<32>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
   }
   __syncthreads();
-  const float2 A = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
-  if (R <= 4) narrow_body<4, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
-  else if (R <= 8) narrow_body<8, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
-  else if (R <= 16) narrow_body<16, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
-  else narrow_body<32, CC>(a, E, Bt, A, R, row_lo, ja, c, out, row_stride);
+  // ---- phase 2: thread (jb = lane, ci = warp)
+  {
+    const int jb = tid & 31, ci = tid >> 5;
+    const int c = 8 * cg + ci;
+    float sn, cs;
+    const unsigned num = ((unsigned)jb * (unsigned)(c + 1024 * (row_lo & 31))) & 32767u;
+    sincospif((float)num * (1.0f / 16384.0f), &sn, &cs);
+    const float2 S = make_float2(cs, sn);
+    float2 x[32];
+#pragma unroll
+    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cmul(tile[jb * kTileStride + m * 8 + ci], S);
+    fft_dit<32>(x);                                   // over m -> jm
+    __syncthreads();                                  // the tile has been read by everyone: reuse it as staging
+    float4* st = reinterpret_cast<float4*>(tile + jb * kStageStride + ci * 32);
+#pragma unroll
+    for (int jm = 0; jm < 32; jm += 2) {
+      const float2 u0 = cmul(x[jm], T3[ci * 32 + jm]), u1 = cmul(x[jm + 1], T3[ci * 32 + jm + 1]);
+      st[jm >> 1] = make_float4(u0.x, u0.y, u1.x, u1.y);
+    }
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic writes -> visible to the bulk copy engine
+  __syncthreads();
+  if (tid < 32) {
+    const unsigned src = (unsigned)__cvta_generic_to_shared(tile + tid * kStageStride);
+    float2* dst = out0 + (size_t)tid * row_stride;
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], 2048;" ::"l"(dst), "r"(src) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the copy's reads
+  }
 }
 
-template <int CJ>
+constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 256) * sizeof(float2);
+
 static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
-  constexpr int CC = 256 / CJ;
-  const size_t smem = (size_t)(64 * CC) * sizeof(float2);
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass1_narrow<CJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNarrowSmem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid((kN2 / CC) * (c->na / CJ), c->prm.p, batch);
-  k_pass1_narrow<CJ><<<grid, 256, smem, c->stream>>>(args);
+  dim3 grid(4 * c->na, c->prm.p, batch);
+  k_pass1_narrow<<<grid, 256, kNarrowSmem, c->stream>>>(args);
   c->launches++;
   return cudaGetLastError();
 }
@@ -351,23 +389,22 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = count;
-  cudaError_t e;
+  args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
+  args.q = ws_ptr<float2>(c, c->lay.q);
+  const int half = (int)(c->n / 2);
+  k_correlate<<<dim3(half / 256, count), 256, 0, c->stream>>>(args.meta, args.wq, args.u_tab, ws_ptr<float2>(c, c->lay.q), half);
+  c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
   if (c->nb == 32) {
-    // narrow bands (most of the work); the wide ones follow through the generic kernel + row stage
-    switch (c->na) {
-      case 1: e = launch_narrow<1>(c, args, count); break;
-      case 2: e = launch_narrow<2>(c, args, count); break;
-      case 4: e = launch_narrow<4>(c, args, count); break;
-      case 8: e = launch_narrow<8>(c, args, count); break;
-      case 16: e = launch_narrow<16>(c, args, count); break;
-      default: e = launch_narrow<32>(c, args, count); break;
-    }
+    // narrow bands (almost all of the work) write the A layout directly
+    e = launch_narrow(c, args, count);
     if (e != cudaSuccess) return e;
   }
+  // wide bands (every band if n1 < 32): generic kernel in the plain layout, then the row stage in place
   e = dispatch_p1<false>(c, args);
   if (e != cudaSuccess) return e;
-  // TRANSITION: the narrow kernel still writes the plain layout, so every band goes through the row stage
-  return launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 0);
+  return launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 1);
 }
 
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
@@ -376,6 +413,8 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.wq = nullptr;
   args.u_tab = nullptr;
   args.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
+  args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
+  args.q = nullptr;
   args.dense_in = d_in;
   args.y = d_mid;
   args.p = 1;
