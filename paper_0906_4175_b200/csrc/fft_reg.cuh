@@ -53,6 +53,12 @@ __device__ __forceinline__ pk2 mul2(pk2 a, pk2 b) { pk2 r; asm("mul.rn.f32x2 %0,
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return unpk(fma2(pk(b.y, b.y), pk(-a.y, a.x), mul2(pk(b.x, b.x), pk(a))));
 }
+// Twiddle in broadcast form (w.x, w.x), (w.y, w.y): a * w is then two packed instructions with no
+// negation or move left over (the half swap and the sign of -a.y are operand modifiers).
+struct tw4 { pk2 xx, yy; };
+__device__ __forceinline__ tw4 make_tw4(float2 w) { tw4 t; t.xx = pk(w.x, w.x); t.yy = pk(w.y, w.y); return t; }
+__device__ __forceinline__ tw4 make_tw4(float4 w) { tw4 t; t.xx = pk(w.x, w.y); t.yy = pk(w.z, w.w); return t; }   // table entry {x, x, y, y}
+__device__ __forceinline__ float2 cmul_tw(float2 a, tw4 w) { return unpk(fma2(pk(-a.y, a.x), w.yy, mul2(w.xx, pk(a)))); }
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return unpk(add2(pk(a), pk(b))); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return unpk(sub2(pk(a), pk(b))); }
 

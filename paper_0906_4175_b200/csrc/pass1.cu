@@ -157,8 +157,8 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
 
 // ---------------------------------------------------------------------------------------------------
 // Row stage for the rows written by k_pass1 in the plain layout Y[j1][k2]: first 32-point stage of the
-// 1024-point row transform plus its twiddle, in place,
-//     A[j1][c][jm] = e^{2 pi i jm c/1024} sum_m e^{2 pi i jm m/32} Y[j1][32 m + c],
+// 1024-point row transform, in place,
+//     A[j1][c][jm] = sum_m e^{2 pi i jm m/32} Y[j1][32 m + c],
 // which is the layout pass 2 reads (k_pass1_narrow writes it directly).  One warp per row; only the
 // bands in the wide list (or every band if use_mask == 0: small n, dense transform) are touched.
 // ---------------------------------------------------------------------------------------------------
@@ -178,8 +178,6 @@ __global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const 
 #pragma unroll
     for (int m = 0; m < 32; ++m) x[brev<32>(m)] = Y[32 * m + lane];       // lane = c
     fft_dit<32>(x);                                                        // over m -> jm
-#pragma unroll
-    for (int jm = 0; jm < 32; ++jm) x[jm] = cmul(x[jm], tw_p2[jm * 32 + lane]);
     __syncwarp();                                                          // the whole row is in registers
     float4* out = reinterpret_cast<float4*>(Y + 32 * lane);
 #pragma unroll
@@ -217,20 +215,21 @@ __global__ void __launch_bounds__(256) k_correlate(const TemplateMeta* __restric
 //
 // A CTA owns one ja and the 256 columns k2 = 32 m + c, m = 0..31, c = 8 cg .. 8 cg + 7, and runs both the
 // column transform and the first stage of the row transform (over m), so that what reaches HBM is already
-//     A[j1][c][jm] = e^{2 pi i jm c/1024} sum_m e^{2 pi i jm m/32} Y[j1][32 m + c],
-// the layout pass 2 consumes with a single 32-point transform per thread:
+//     A[j1][c][jm] = sum_m e^{2 pi i jm m/32} Y[j1][32 m + c],
+// the layout pass 2 consumes with one twiddle and one 32-point transform per thread:
 //   phase 1, thread (m, ci):  v[jb] = FFT32_b( Q[k] e^{2 pi i ja k/n} ),  tile[jb][m][ci] = v[jb] e^{2 pi i jb m/1024}
 //   phase 2, thread (jb, ci): x[m] = tile[jb][m][ci] S,  S = e^{2 pi i jb (c + 1024 b0)/32768}  (the rest of the
 //                             column twiddle e^{2 pi i NA jb k2/n} and the rotation w_32^{jb b0});
-//                             X[jm] = FFT32_m(x) e^{2 pi i jm c/1024};  staged as [jb][ci][jm]
+//                             X[jm] = FFT32_m(x);  staged as [jb][ci][jm]
 //   store: per jb one contiguous 2 KB piece of row j1, by TMA bulk copy shared -> global.
 // ---------------------------------------------------------------------------------------------------
 constexpr int kTileStride = 257;      // float2 per jb row of the exchange tile (conflict-free both ways)
 constexpr int kStageStride = 258;     // float2 per jb row of the store staging (16-byte aligned rows)
 
 template <int RMAX>
-__device__ __forceinline__ void narrow_phase1(const P1Args& a, const float2* __restrict__ qrow, float2* __restrict__ tile,
-                                              float2 Aja, int R, int row_lo, int e_lo, int e_hi, int ja, int k2, int m, int ci) {
+__device__ __forceinline__ void narrow_phase1(const P1Args& a, const float2* __restrict__ qrow, const float2* __restrict__ T1,
+                                              float2* __restrict__ tile, float2 Aja, int R, int row_lo, int e_lo, int e_hi,
+                                              int ja, int k2, int m, int ci) {
   float2 v[32];
   const int n1m = a.n1 - 1;
 #pragma unroll
@@ -246,13 +245,13 @@ __device__ __forceinline__ void narrow_phase1(const P1Args& a, const float2* __r
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
 #pragma unroll
   for (int jb = 0; jb < 32; ++jb)
-    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], __ldg(&a.tw_p2[jb * 32 + m]));
+    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], T1[jb * 32 + m]);
 }
 
 __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   extern __shared__ __align__(128) float2 smem[];
   float2* tile = smem;                          // [32][kStageStride] (phase 1 uses stride kTileStride)
-  float2* T3 = smem + 32 * kStageStride;        // [8][32]  e^{2 pi i jm c/1024}
+  float2* T1 = smem + 32 * kStageStride;        // [32 jb][32 m]  e^{2 pi i jb m/1024}
 
   const int tid = threadIdx.x;
   const int na = a.n1 >> 5;
@@ -274,20 +273,19 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   const int R = row_hi - row_lo + 1;
   if (R > 32) return;             // wide band: k_pass1 + k_rowstage
 
-  {
-    const int ci = tid >> 5, jm = tid & 31;
-    T3[tid] = __ldg(&a.tw_p2[jm * 32 + 8 * cg + ci]);
-  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) T1[tid + 256 * i] = __ldg(&a.tw_p2[tid + 256 * i]);
+  __syncthreads();
   // ---- phase 1: thread (m, ci), column k2
   {
     const int ci = tid & 7, m = tid >> 3;
     const int k2 = 32 * m + 8 * cg + ci;
     const float2 Aja = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
     const float2* qrow = a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
-    if (R <= 4) narrow_phase1<4>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
-    else if (R <= 8) narrow_phase1<8>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
-    else if (R <= 16) narrow_phase1<16>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
-    else narrow_phase1<32>(a, qrow, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    if (R <= 4) narrow_phase1<4>(a, qrow, T1, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    else if (R <= 8) narrow_phase1<8>(a, qrow, T1, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    else if (R <= 16) narrow_phase1<16>(a, qrow, T1, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
+    else narrow_phase1<32>(a, qrow, T1, tile, Aja, R, row_lo, e_lo, e_hi, ja, k2, m, ci);
   }
   __syncthreads();
   // ---- phase 2: thread (jb = lane, ci = warp)
@@ -297,18 +295,15 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
     float sn, cs;
     const unsigned num = ((unsigned)jb * (unsigned)(c + 1024 * (row_lo & 31))) & 32767u;
     sincospif((float)num * (1.0f / 16384.0f), &sn, &cs);
-    const float2 S = make_float2(cs, sn);
+    const tw4 S = make_tw4(make_float2(cs, sn));
     float2 x[32];
 #pragma unroll
-    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cmul(tile[jb * kTileStride + m * 8 + ci], S);
+    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cmul_tw(tile[jb * kTileStride + m * 8 + ci], S);
     fft_dit<32>(x);                                   // over m -> jm
     __syncthreads();                                  // the tile has been read by everyone: reuse it as staging
     float4* st = reinterpret_cast<float4*>(tile + jb * kStageStride + ci * 32);
 #pragma unroll
-    for (int jm = 0; jm < 32; jm += 2) {
-      const float2 u0 = cmul(x[jm], T3[ci * 32 + jm]), u1 = cmul(x[jm + 1], T3[ci * 32 + jm + 1]);
-      st[jm >> 1] = make_float4(u0.x, u0.y, u1.x, u1.y);
-    }
+    for (int jm = 0; jm < 32; jm += 2) st[jm >> 1] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic writes -> visible to the bulk copy engine
   __syncthreads();
@@ -321,7 +316,7 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   }
 }
 
-constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 256) * sizeof(float2);
+constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 1024) * sizeof(float2);
 
 static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
   static bool configured = false;

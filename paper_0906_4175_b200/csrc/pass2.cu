@@ -2,10 +2,10 @@
 // maxima (end of step a3, steps a4 and a5).
 //
 // Index algebra (see pass1.cu): sample j = j1 + n1 (jm + 32 jc); pass 1 leaves, per band l and row j1,
-//     A_l[j1][c][jm] = e^{2 pi i jm c/1024} sum_m e^{2 pi i jm m/32} Y_l[j1][32 m + c]        (8 KB, contiguous)
-// so that        z_l[j1 + n1 (jm + 32 jc)] = sum_c e^{2 pi i jc c/32} A_l[j1][c][jm]
-// is ONE 32-point transform per thread with lane = jm: no twiddles, no transpose, no shared-memory
-// exchange.  Warps are persistent: a warp walks over rows (template, j1) and, within a row, over the p
+//     A_l[j1][c][jm] = sum_m e^{2 pi i jm m/32} Y_l[j1][32 m + c]                              (8 KB, contiguous)
+// so that        z_l[j1 + n1 (jm + 32 jc)] = sum_c e^{2 pi i jc c/32} e^{2 pi i jm c/1024} A_l[j1][c][jm]
+// is ONE twiddle multiply (table in shared memory, same for every row and band) and ONE 32-point
+// transform per thread with lane = jm: no transpose, no shared-memory exchange.  Warps are persistent: a warp walks over rows (template, j1) and, within a row, over the p
 // bands; every 8 KB row is brought into the warp's ring of shared-memory buffers by one TMA bulk copy
 // (cp.async.bulk + mbarrier), issued kP2Ring rows ahead across band AND row boundaries, so HBM latency is
 // hidden by the ring, not by occupancy.  Per owned output sample the warp accumulates
@@ -23,6 +23,7 @@ namespace gwmf {
 
 struct P2Args {
   const float2* y;            // A layout: [batch][p][n1][c = 32][jm = 32]
+  const float2* tw_p2;        // [32][32] e^{2 pi i c jm/1024}
   const TemplateMeta* meta;   // offset to first template of the batch
   Slot* slots;                // offset to first template of the batch; nullptr = do not update
   float* series_rho;          // optional: n floats (batch must be 1)
@@ -92,13 +93,16 @@ __device__ __forceinline__ void bulk_load_row(void* dst, const void* src, unsign
 constexpr int kRowBytes = kN2 * (int)sizeof(float2);      // 8 KB
 constexpr int kP2Ring = 3;                                // row buffers per warp
 
-// Shared memory: [warp 0: ring of kP2Ring rows][warp 1: ...]...[mbarriers, kP2Ring per warp].
+// Shared memory: [twiddles 32x32][warp 0: ring of kP2Ring rows][warp 1: ...]...[mbarriers, kP2Ring per warp].
 template <bool STORE>
 __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
   extern __shared__ __align__(128) float2 smem2[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float2* bufs = smem2 + warp * (kP2Ring * kN2);
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + kP2Warps * kP2Ring * kN2) + kP2Ring * warp;
+  float2* tw_s = smem2;                                               // [c][jm]
+  float2* bufs = smem2 + 1024 + warp * (kP2Ring * kN2);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * kP2Ring * kN2) + kP2Ring * warp;
+  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
+  __syncthreads();                                                    // the only CTA-wide barrier
 
   const int p = a.p;
   const int total_warps = gridDim.x * kP2Warps;
@@ -152,7 +156,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
     mbar_wait(&bars[b], (item / kP2Ring) & 1);
     float2 x[32];
 #pragma unroll
-    for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cur[32 * c + lane];     // lane = jm
+    for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(cur[32 * c + lane], tw_s[32 * c + lane]);     // lane = jm
     fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
     __syncwarp();                                                         // every lane holds its 32 values
     if (pf_item < n_items) {
@@ -204,7 +208,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
   }
 }
 
-constexpr size_t kP2Smem = (size_t)kP2Warps * kP2Ring * kN2 * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
+constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
 
 static cudaError_t p2_configure() {
   static bool done = false;
@@ -223,6 +227,7 @@ static int p2_grid(const Ctx* c, int n_rows) {
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi) {
   P2Args a;
   a.y = ws_ptr<float2>(c, c->lay.y);
+  a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   a.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
   a.slots = update_slots ? ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows : nullptr;
   a.series_rho = series_rho;
@@ -247,6 +252,7 @@ cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots,
 cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
   P2Args a;
   a.y = d_mid;
+  a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   a.meta = nullptr;
   a.slots = nullptr;
   a.series_rho = nullptr;
