@@ -66,7 +66,7 @@ Layout make_layout(const gwmf_params* p) {
   L.series_rho = take(n * sizeof(float));
   L.series_chi = take(n * sizeof(float));
   L.flags = take(256);
-  L.q = take((size_t)L.batch * half * sizeof(float2));
+  L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
   size_t yb = (size_t)L.batch * (size_t)p->p * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;
@@ -154,15 +154,29 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->have_bank = c->have_segment = false;
   c->launches = 0;
   c->h_meta = nullptr;
+  c->side = nullptr;
+  c->ev_fork = c->ev_join = nullptr;
+  {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);
+    if (cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, hi) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+      if (c->side) cudaStreamDestroy(c->side);
+      if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+      delete c;
+      return GWMF_E_CUDA;
+    }
+  }
   if (cudaMallocHost((void**)&c->h_meta, sizeof(TemplateMeta) * (size_t)params->max_templates) != cudaSuccess) {
-    delete c;
+    c->h_meta = nullptr;
+    gwmf_destroy(reinterpret_cast<gwmf_ctx*>(c));
     return GWMF_E_CUDA;
   }
   cudaError_t e = launch_tables(c);
   if (e == cudaSuccess) e = launch_reset_slots(c, 0, params->max_templates);
   if (e != cudaSuccess) {
-    cudaFreeHost(c->h_meta);
-    delete c;
+    gwmf_destroy(reinterpret_cast<gwmf_ctx*>(c));
     return GWMF_E_CUDA;
   }
   *out = reinterpret_cast<gwmf_ctx*>(c);
@@ -173,6 +187,9 @@ void gwmf_destroy(gwmf_ctx* ctx) {
   if (!ctx) return;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
   cudaStreamSynchronize(c->stream);
+  if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
   if (c->h_meta) cudaFreeHost(c->h_meta);
   delete c;
 }
@@ -221,9 +238,12 @@ int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates) {
   if (first_template < 0 || n_templates < 0 || first_template + n_templates > c->n_templates) return GWMF_E_ARG;
   if (n_templates == 0) return GWMF_OK;
   CU(launch_reset_slots(c, first_template, n_templates));
-  for (int done = 0; done < n_templates; done += c->lay.batch) {
-    int cnt = n_templates - done < c->lay.batch ? n_templates - done : c->lay.batch;
-    CU(launch_pass1_filter(c, first_template + done, cnt));
+  int parity = 0;
+  for (int done = 0; done < n_templates; done += c->lay.batch, parity ^= 1) {
+    const int cnt = n_templates - done < c->lay.batch ? n_templates - done : c->lay.batch;
+    const int rest = n_templates - done - cnt;
+    const int next = rest < c->lay.batch ? rest : c->lay.batch;
+    CU(launch_pass1_filter(c, first_template + done, cnt, first_template + done + cnt, next, parity, done > 0));
     CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
   }
   return GWMF_OK;
@@ -242,8 +262,10 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
   for (int b = 0; b < nb; ++b) {
     int done = b * c->lay.batch;
     int cnt = n_templates - done < c->lay.batch ? n_templates - done : c->lay.batch;
+    const int rest = n_templates - done - cnt;
+    const int next = rest < c->lay.batch ? rest : c->lay.batch;
     CU(cudaEventRecord(ev[3 * b], c->stream));
-    CU(launch_pass1_filter(c, first_template + done, cnt));
+    CU(launch_pass1_filter(c, first_template + done, cnt, first_template + done + cnt, next, b & 1, b > 0));
     CU(cudaEventRecord(ev[3 * b + 1], c->stream));
     CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
     CU(cudaEventRecord(ev[3 * b + 2], c->stream));
@@ -334,7 +356,7 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
   if (rc != GWMF_OK) return rc;
   float* d_rho = ws_ptr<float>(c, c->lay.series_rho);
   float* d_chi = ws_ptr<float>(c, c->lay.series_chi);
-  CU(launch_pass1_filter(c, template_id, 1));
+  CU(launch_pass1_filter(c, template_id, 1, 0, 0, 0, false));
   CU(launch_pass2_filter(c, template_id, 1, false, d_rho, d_chi));
   if (host_rho)
     CU(cudaMemcpyAsync(host_rho, d_rho, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));

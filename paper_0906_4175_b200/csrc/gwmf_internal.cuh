@@ -53,6 +53,8 @@ struct Ctx {
   Layout lay;
   char* ws;
   cudaStream_t stream;
+  cudaStream_t side;             // high-priority side stream for the low-volume pass-1 kernels
+  cudaEvent_t ev_fork, ev_join;
   int n_templates;
   bool have_bank, have_segment;
   int64_t launches;
@@ -64,7 +66,7 @@ struct Ctx {
 cudaError_t launch_tables(Ctx* c);
 cudaError_t launch_segment_prepare(Ctx* c);                       // after s/Sn are on the device
 cudaError_t launch_bank_setup(Ctx* c);
-cudaError_t launch_pass1_filter(Ctx* c, int first, int count);
+cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready);
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
 cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid);
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,

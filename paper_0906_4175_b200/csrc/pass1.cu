@@ -332,7 +332,7 @@ static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
 }
 
 template <int NA, int NB, bool DENSE>
-static cudaError_t launch_p1(Ctx* c, const P1Args& args) {
+static cudaError_t launch_p1(Ctx* c, const P1Args& args, cudaStream_t st) {
   constexpr int FR = NA >= 32 ? 32 : NA;
   constexpr int SROW = NB * kColsPerCta + kColsPerCta;
   const size_t smem = (size_t)(FR * SROW + FR * kColsPerCta + NB * kColsPerCta) * sizeof(float2);
@@ -343,36 +343,51 @@ static cudaError_t launch_p1(Ctx* c, const P1Args& args) {
     configured = true;
   }
   // persistent over the work list; a CTA with nothing to do exits after building the (empty) list
-  k_pass1<NA, NB, DENSE><<<2 * c->n_sms, 256, smem, c->stream>>>(args);
+  k_pass1<NA, NB, DENSE><<<2 * c->n_sms, 256, smem, st>>>(args);
   c->launches++;
   return cudaGetLastError();
 }
 
 template <bool DENSE>
-static cudaError_t dispatch_p1(Ctx* c, const P1Args& args) {
+static cudaError_t dispatch_p1(Ctx* c, const P1Args& args, cudaStream_t st) {
   switch (c->na) {
     case 1:
-      if (c->nb == 16) return launch_p1<1, 16, DENSE>(c, args);
-      return launch_p1<1, 32, DENSE>(c, args);
-    case 2: return launch_p1<2, 32, DENSE>(c, args);
-    case 4: return launch_p1<4, 32, DENSE>(c, args);
-    case 8: return launch_p1<8, 32, DENSE>(c, args);
-    case 16: return launch_p1<16, 32, DENSE>(c, args);
-    case 32: return launch_p1<32, 32, DENSE>(c, args);
-    case 64: return launch_p1<64, 32, DENSE>(c, args);
-    case 128: return launch_p1<128, 32, DENSE>(c, args);
+      if (c->nb == 16) return launch_p1<1, 16, DENSE>(c, args, st);
+      return launch_p1<1, 32, DENSE>(c, args, st);
+    case 2: return launch_p1<2, 32, DENSE>(c, args, st);
+    case 4: return launch_p1<4, 32, DENSE>(c, args, st);
+    case 8: return launch_p1<8, 32, DENSE>(c, args, st);
+    case 16: return launch_p1<16, 32, DENSE>(c, args, st);
+    case 32: return launch_p1<32, 32, DENSE>(c, args, st);
+    case 64: return launch_p1<64, 32, DENSE>(c, args, st);
+    case 128: return launch_p1<128, 32, DENSE>(c, args, st);
   }
   return cudaErrorInvalidValue;
 }
 
-static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, int batch, int n_bands_all, int use_mask) {
-  k_rowstage<<<4 * c->n_sms, 256, 0, c->stream>>>(y, ws_ptr<float2>(c, c->lay.tw_p2), meta, batch, c->prm.p,
+static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, int batch, int n_bands_all, int use_mask,
+                                   cudaStream_t st) {
+  k_rowstage<<<4 * c->n_sms, 256, 0, st>>>(y, ws_ptr<float2>(c, c->lay.tw_p2), meta, batch, c->prm.p,
                                                   c->log_n - kLogN2, n_bands_all, use_mask);
   c->launches++;
   return cudaGetLastError();
 }
 
-cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
+static cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+  const int half = (int)(c->n / 2);
+  k_correlate<<<dim3(half / 256, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, ws_ptr<float2>(c, c->lay.wq),
+                                                      ws_ptr<double>(c, c->lay.u_tab),
+                                                      ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half, half);
+  c->launches++;
+  return cudaGetLastError();
+}
+
+// Pass 1 of one batch.  The narrow-band kernel (almost all of the work) runs on the context's stream; the
+// low-volume kernels -- the generic kernel and the row stage for the wide bands, and the correlate kernel
+// of the NEXT batch (next_count > 0) into the other half of the double-buffered Q -- run beside it on a
+// high-priority side stream between a fork and a join event.  q_ready: this batch's Q was already produced
+// by the previous call.
+cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready) {
   P1Args args;
   args.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
   args.wq = ws_ptr<float2>(c, c->lay.wq);
@@ -385,21 +400,32 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count) {
   args.n1 = c->n1;
   args.batch = count;
   args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
-  args.q = ws_ptr<float2>(c, c->lay.q);
-  const int half = (int)(c->n / 2);
-  k_correlate<<<dim3(half / 256, count), 256, 0, c->stream>>>(args.meta, args.wq, args.u_tab, ws_ptr<float2>(c, c->lay.q), half);
-  c->launches++;
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
+  args.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
+  cudaError_t e;
+  if (!q_ready) {
+    e = launch_correlate(c, first, count, parity, c->stream);
+    if (e != cudaSuccess) return e;
+  }
+  // fork: everything enqueued so far on the main stream (this batch's Q, the previous batch's pass 2, which
+  // read the band buffer) precedes the side work
+  if ((e = cudaEventRecord(c->ev_fork, c->stream)) != cudaSuccess) return e;
+  if ((e = cudaStreamWaitEvent(c->side, c->ev_fork, 0)) != cudaSuccess) return e;
   if (c->nb == 32) {
-    // narrow bands (almost all of the work) write the A layout directly
+    // narrow bands write the A layout directly
     e = launch_narrow(c, args, count);
     if (e != cudaSuccess) return e;
   }
   // wide bands (every band if n1 < 32): generic kernel in the plain layout, then the row stage in place
-  e = dispatch_p1<false>(c, args);
+  e = dispatch_p1<false>(c, args, c->side);
   if (e != cudaSuccess) return e;
-  return launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 1);
+  e = launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 1, c->side);
+  if (e != cudaSuccess) return e;
+  if (next_count > 0) {
+    e = launch_correlate(c, next_first, next_count, parity ^ 1, c->side);
+    if (e != cudaSuccess) return e;
+  }
+  if ((e = cudaEventRecord(c->ev_join, c->side)) != cudaSuccess) return e;
+  return cudaStreamWaitEvent(c->stream, c->ev_join, 0);
 }
 
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
@@ -416,9 +442,9 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = 1;
-  return dispatch_p1<true>(c, args);
+  return dispatch_p1<true>(c, args, c->stream);
 }
 
-cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid) { return launch_rowstage(c, d_mid, nullptr, 1, 1, 0); }
+cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid) { return launch_rowstage(c, d_mid, nullptr, 1, 1, 0, c->stream); }
 
 }  // namespace gwmf

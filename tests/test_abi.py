@@ -48,7 +48,7 @@ def test_workspace_bytes_host_only(lib):
     b = gwmf.workspace_bytes(1 << 20, 16, 4096, 1024)
     # band intermediate: batch(8) * p * n * 8 B = 1 GiB, plus the correlated spectra (batch * 4 MiB),
     # tables / slots / staging
-    assert (1 << 30) + (32 << 20) < b < (1 << 30) + (96 << 20)
+    assert (1 << 30) + (64 << 20) < b < (1 << 30) + (128 << 20)
     assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (320 << 20)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
