@@ -241,8 +241,9 @@ def run_gpu(args):
     gbs = bytes_per_launch / (avg_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak()
     dom = int(np.argmax(k_ms))
-    names = ["k_pass1 (template+correlate+FFT pass 1, writes p*N*8 B/template)",
-             "k_pass2 (FFT pass 2 + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"]
+    names = ["pass 1: k_pass1_narrow (pruned column FFT + first row stage, writes p*N*8 B/template) with the "
+             "low-volume kernels (k_correlate, k_pass1 generic, k_rowstage) beside it on the side stream; timed fork to join",
+             "pass 2: k_pass2 (last FFT stage + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"]
 
     # end to end through the C ABI with host buffers
     s_pin = torch.from_numpy(s32).pin_memory()
@@ -306,9 +307,9 @@ def run_gpu(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of
-# each kernel (profiles/), index 0 = k_pass1, 1 = k_pass2; None until a capture exists.
-TRAFFIC_BYTES = {0: None, 1: None}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (8 templates) from the committed `ncu --set full`
+# capture (profiles/r1_v11_*.md): index 0 = k_pass1_narrow (0.0041 + 1.0147 GB), 1 = k_pass2 (1.0738 + 0.0038 GB).
+TRAFFIC_BYTES = {0: 1.0188e9, 1: 1.0777e9}
 
 
 def main():

@@ -1,15 +1,18 @@
-// pass1.cu -- first pass of the band inverse FFTs (step a2 + first half of a3), with the correlate
-// fused in: the input Q[k] = w[k] f_k^(-7/6) e^{i Psi0(f_k)} is GENERATED per bin (template phase in fp64,
-// reduced to turns, then fp32 sincospi) and never stored.
+// pass1.cu -- correlate (step a2) and the first pass of the band inverse FFTs (first half of a3).
 //
-// Index algebra.  n = n1 * 1024.  Input bin k = 1024 k1 + k2, output sample j = j1 + n1 j2.
-//   z_l[j1 + n1 j2] = sum_{k2} e^{2 pi i j2 k2/1024} Y_l[j1][k2]                               (pass 2)
-//   Y_l[j1][k2]     = e^{2 pi i j1 k2/n} sum_{k1 in band l} Q[1024 k1 + k2] e^{2 pi i j1 k1/n1}  (this file)
+// Index algebra.  n = n1 * 1024.  Input bin k = 1024 k1 + k2, k2 = 32 m + c; output sample j = j1 + n1 j2,
+// j2 = jm + 32 jc.
+//   z_l[j1 + n1 (jm + 32 jc)] = sum_c e^{2 pi i jc c/32} e^{2 pi i jm c/1024} A_l[j1][c][jm]          (pass 2)
+//   A_l[j1][c][jm]  = sum_m e^{2 pi i jm m/32} Y_l[j1][32 m + c]                            (row stage, this file)
+//   Y_l[j1][k2]     = e^{2 pi i j1 k2/n} sum_{k1 in band l} Q[1024 k1 + k2] e^{2 pi i j1 k1/n1}  (column transform)
+// What this pass leaves in HBM is A_l (p * n complex per template): each row j1 is 8 KB, [c][jm].
 // The n1-point column transform is itself split n1 = NA * NB with k1 = NB a + b, j1 = ja + NA jb:
-//   stage 1 (thread = (b, column)):  V[ja][b] = sum_a Q[NB a + b] w_NA^{ja a}, times e^{2 pi i ja (1024 b + k2)/n}
-//   stage 2 (thread = (ja, column)): Y[ja + NA jb] = e^{2 pi i NA jb k2/n} sum_b w_NB^{jb b} V[ja][b]
-// A band is a contiguous run of bins, i.e. of rows k1, so stage 1 only touches the groups of `a` that
-// the band reaches (pruned input); for NA > 32 a CTA produces the 32 outputs ja = G m + r of one residue r.
+//   stage 1:  V[ja][b] = sum_a Q[NB a + b] w_NA^{ja a}, times e^{2 pi i ja (1024 b + k2)/n}
+//   stage 2:  Y[ja + NA jb] = e^{2 pi i NA jb k2/n} sum_b w_NB^{jb b} V[ja][b]
+// A band is a contiguous run of bins, i.e. of rows k1, so the transform is pruned to the rows the band touches.
+// Kernels:  k_correlate (Q once per template and bin), k_pass1_narrow (bands of <= 32 rows: column transform +
+// row stage in one CTA, writes A directly), k_pass1 (generic: wide bands and the dense transform, plain layout
+// Y) followed by k_rowstage (Y -> A in place).
 #include "fft_reg.cuh"
 #include "gwmf_internal.cuh"
 
@@ -23,7 +26,7 @@ struct P1Args {
   const float2* tw_p2;        // [32][32] e^{2 pi i a b/1024}
   const float2* q;            // [batch][n/2] correlated spectrum Q_I[k] (k_correlate)
   const float2* dense_in;     // DENSE only: n complex inputs
-  float2* y;                  // [batch][p][n1][1024]
+  float2* y;                  // [batch][p][n1][1024]: row j1 of band l, A layout [c][jm] (generic kernel: plain Y[k2])
   int p;
   int log_n;
   int n1;
