@@ -228,6 +228,7 @@ __global__ void __launch_bounds__(256) k_correlate(const TemplateMeta* __restric
 // ---------------------------------------------------------------------------------------------------
 constexpr int kTileStride = 257;      // float2 per jb row of the exchange tile (conflict-free both ways)
 constexpr int kStageStride = 258;     // float2 per jb row of the store staging (16-byte aligned rows)
+constexpr int kT1Stride = 34;         // float2 per row of the shared twiddle table (16-byte aligned, conflict-free LDS.128)
 
 template <int RMAX>
 __device__ __forceinline__ void narrow_phase1(const P1Args& a, const float2* __restrict__ qrow, const float2* __restrict__ T1,
@@ -246,15 +247,20 @@ __device__ __forceinline__ void narrow_phase1(const P1Args& a, const float2* __r
     v[brev<32>(i)] = val;
   }
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
+  // T1 is symmetric: row m holds e^{2 pi i jb m/1024} for consecutive jb, read two at a time
+  const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
 #pragma unroll
-  for (int jb = 0; jb < 32; ++jb)
-    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], T1[jb * 32 + m]);
+  for (int jb = 0; jb < 32; jb += 2) {
+    const float4 w = t1[jb >> 1];
+    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], make_float2(w.x, w.y));
+    tile[(jb + 1) * kTileStride + m * 8 + ci] = cmul(v[jb + 1], make_float2(w.z, w.w));
+  }
 }
 
 __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   extern __shared__ __align__(128) float2 smem[];
   float2* tile = smem;                          // [32][kStageStride] (phase 1 uses stride kTileStride)
-  float2* T1 = smem + 32 * kStageStride;        // [32 jb][32 m]  e^{2 pi i jb m/1024}
+  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i jb m/1024}
 
   const int tid = threadIdx.x;
   const int na = a.n1 >> 5;
@@ -277,7 +283,7 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   if (R > 32) return;             // wide band: k_pass1 + k_rowstage
 
 #pragma unroll
-  for (int i = 0; i < 4; ++i) T1[tid + 256 * i] = __ldg(&a.tw_p2[tid + 256 * i]);
+  for (int i = 0; i < 4; ++i) T1[(tid >> 5) * kT1Stride + 8 * i * kT1Stride + (tid & 31)] = __ldg(&a.tw_p2[tid + 256 * i]);
   __syncthreads();
   // ---- phase 1: thread (m, ci), column k2
   {
@@ -319,7 +325,7 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   }
 }
 
-constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 1024) * sizeof(float2);
+constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 32 * kT1Stride) * sizeof(float2);
 
 static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
   static bool configured = false;
