@@ -271,8 +271,8 @@ def run_gpu(args):
 
     if rank == 0:
         line = base_line(args, w, value, ms / args.steps, "f32")
-        line["config"]["l2"] = ("no flush: every launch streams a band intermediate of batch*p*N*8 B = 1 GiB, "
-                                "8x the 126 MB L2, so nothing survives from one launch to the next")
+        line["config"]["l2"] = ("no flush: every launch streams a band intermediate of batch*p*N*8 B = 2 GiB, "
+                                "16x the 126 MB L2, through pass 1 (write) and pass 2 (read)")
         line["config"]["batch_templates_per_launch"] = float(batch_templates[0])
         line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(s32.nbytes + Sn.nbytes),
                        "d2h_bytes_per_step": int(12 + trig.nbytes), "ms_per_step": ms_e2e / args.steps}
@@ -281,7 +281,7 @@ def run_gpu(args):
         line["triggers_per_step"] = int(len(trig))
         line["roofline"] = {
             "bound": "hbm", "kernel": names[dom], "achieved": float(gbs[dom]), "peak": peak, "unit": "GB/s",
-            "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": TRAFFIC_BYTES.get(dom),
+            "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": TRAFFIC_BYTES_PER_TEMPLATE[dom] * float(batch_templates[dom]),
             "bytes_per_launch": float(bytes_per_launch[dom]), "avg_launch_ms": float(avg_ms[dom]),
             "kernels": {"k_pass1": {"avg_launch_ms": float(avg_ms[0]), "GB/s": float(gbs[0]), "frac": float(gbs[0] / peak),
                                     "share_of_step": float(k_ms[0] / k_ms.sum())},
@@ -307,9 +307,10 @@ def run_gpu(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch (8 templates) from the committed `ncu --set full`
-# capture (profiles/r1_v11_*.md): index 0 = k_pass1_narrow (0.0041 + 1.0147 GB), 1 = k_pass2 (1.0738 + 0.0038 GB).
-TRAFFIC_BYTES = {0: 1.0188e9, 1: 1.0777e9}
+# dram__bytes_read.sum + dram__bytes_write.sum PER TEMPLATE from the committed `ncu --set full` capture
+# (profiles/r1_v11_*.md, 8 templates per launch): index 0 = k_pass1_narrow ((0.0041 + 1.0147) GB / 8),
+# 1 = k_pass2 ((1.0738 + 0.0038) GB / 8); scaled by the templates per launch of the run.
+TRAFFIC_BYTES_PER_TEMPLATE = {0: 1.0188e9 / 8, 1: 1.0777e9 / 8}
 
 
 def main():

@@ -29,10 +29,11 @@ bool params_ok(const gwmf_params* p) {
 }
 
 int default_batch(const gwmf_params* p) {
-  // keep the band intermediate (batch * p * n * 8 B) near 1 GiB: several waves of CTAs per launch
-  // without holding more than ~1% of the 180 GB HBM
+  // keep the band intermediate (batch * p * n * 8 B) near 2 GiB: many waves of CTAs per launch (kernel
+  // tails and launch gaps amortised; measured 16 > 8 > 4 templates per launch at n = 2^20) while holding
+  // about 1% of the 180 GB HBM
   double per = (double)p->p * (double)p->n * 8.0;
-  int b = (int)(1073741824.0 / per);
+  int b = (int)(2147483648.0 / per);
   if (b < 1) b = 1;
   if (b > kMaxBatch) b = kMaxBatch;
   if (b > p->max_templates) b = p->max_templates;

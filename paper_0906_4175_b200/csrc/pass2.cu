@@ -117,7 +117,9 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
 
   // prefetch cursor (next item to request)
-  int pf_item = 0, pf_l = 0, pf_row = first_row;
+  // Rows are walked from the END of the band buffer: what pass 1 wrote last is still in L2.
+  const int last_row = a.n_rows - 1 - first_row;
+  int pf_item = 0, pf_l = 0, pf_row = last_row;
   auto prefetch = [&]() {
     // caller: lane 0 only, and only after every lane has consumed the buffer being refilled
     const int tb = pf_row >> a.log_n1, j1 = pf_row & n1_mask;
@@ -129,7 +131,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
   };
   auto advance = [&]() {
     ++pf_item;
-    if (++pf_l == p) { pf_l = 0; pf_row += total_warps; }
+    if (++pf_l == p) { pf_l = 0; pf_row -= total_warps; }
   };
   if (lane == 0) {
 #pragma unroll
@@ -148,7 +150,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 #pragma unroll
   for (int i = 0; i < 32; ++i) { az[i] = make_float2(0.f, 0.f); aq[i] = 0.f; }
 
-  int l = 0, row = first_row;
+  int l = 0, row = last_row;
 #pragma unroll 1
   for (int item = 0; item < n_items; ++item) {
     const int b = item % kP2Ring;
@@ -167,7 +169,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 #pragma unroll
       for (int jc = 0; jc < 32; ++jc)
         a.dense_out[(size_t)row + ((size_t)(lane + 32 * jc) << a.log_n1)] = x[jc];
-      row += total_warps;
+      row -= total_warps;
     } else {
 #pragma unroll
       for (int jc = 0; jc < 32; ++jc) {
@@ -202,7 +204,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
           aq[jc] = 0.f;
         }
         l = 0;
-        row += total_warps;
+        row -= total_warps;
       }
     }
   }

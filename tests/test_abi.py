@@ -46,9 +46,9 @@ def test_workspace_bytes_host_only(lib):
     assert gwmf.workspace_bytes(1 << 23, 4, 4096, 1) == 0
     assert gwmf.workspace_bytes(1 << 14, 33, 4096, 1) == 0
     b = gwmf.workspace_bytes(1 << 20, 16, 4096, 1024)
-    # band intermediate: batch(8) * p * n * 8 B = 1 GiB, plus the correlated spectra (batch * 4 MiB),
-    # tables / slots / staging
-    assert (1 << 30) + (64 << 20) < b < (1 << 30) + (128 << 20)
+    # band intermediate: batch(16) * p * n * 8 B = 2 GiB, plus the double-buffered correlated spectra
+    # (2 * batch * 4 MiB), tables / slots / staging
+    assert (2 << 30) + (128 << 20) < b < (2 << 30) + (192 << 20)
     assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (320 << 20)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
