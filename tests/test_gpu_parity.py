@@ -208,6 +208,28 @@ def test_p_extremes_and_covariance(gw):
     assert f2.sigma()[0] == pytest.approx(f1.sigma()[0] / math.sqrt(c), rel=1e-12)
 
 
+def test_empty_bands_and_few_bins(gw):
+    # a template that spans only a few dozen bins: with p = 32 most bands hold one bin and several are
+    # empty (coinciding edges) -- their z_l must be exactly 0 in both pass-1 paths
+    for log_n in (14, 15):           # n1 = 16: generic kernel only; n1 = 32: narrow kernel's empty-band path
+        n = 1 << log_n
+        masses = [(50.0, 50.0), (48.0, 45.0), (8.0, 8.0)]       # f_ISCO = 44.0 Hz, 47.3 Hz, 275 Hz
+        s = inputs.time_series(inputs.noise_spectrum(n, 77) + inputs.injection_spectrum(n, 50.0, 50.0, 9.0, n // 2), n)
+        s = s.astype(np.float32)
+        Sn = inputs.psd_array(n)
+        w = inputs.Workload(config=-1, n=n, p=32, rho_thresh=4.0, window=2048, masses=masses, seed=0)
+        f = _run_gpu(gw, w, s, Sn)
+        out = oracle.filter_bank(s.astype(np.float64), Sn, masses, 32, 2048, 4.0)
+        parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
+        e = np.asarray(out["edges"])
+        assert np.any(e[0, 1:] == e[0, :-1]), "this case is meant to have empty bands"
+        for t, (m1, m2) in enumerate(masses):
+            rho_o, chi_o, _, _ = oracle.filter_template(s.astype(np.float64), Sn, m1, m2, 32)
+            rho_g, chi_g = f.series(t)
+            parity.assert_series(rho_g, chi_g, rho_o, chi_o, 32, f"few-bin template {t}, n=2^{log_n}")
+        parity.assert_triggers(f.triggers(), out, 4.0, 2048, 32)
+
+
 def test_determinism_and_refilter(gw):
     w = inputs.workload(0)
     s = inputs.segment(w)
