@@ -163,6 +163,41 @@ def test_config4_long_segment_sampled(gw):
     _sampled_config(gw, 4, ids)
 
 
+def test_long_segment_p16_sampled(gw):
+    # SURVEY 8(f)-3 / PAPER.md:119,194: N = 4 x 2^20 segments with the headline p = 16 (the paper's "another
+    # factor of 2" shape): config 4's segment and bank, 16 bands
+    w = inputs.workload(4, 48)
+    s = inputs.segment(w).astype(np.float32)
+    Sn = w.psd
+    f = _run_gpu(gw, w, s, Sn, p=16)
+    ids = [0, 17, 47]
+    s64 = s.astype(np.float64)
+    out = oracle.filter_bank(s64, Sn, [w.masses[i] for i in ids], 16, w.window, w.rho_thresh)
+    parity.assert_sigma_edges(f.sigma()[ids], f.band_edges()[ids], out["sigma"], out["edges"])
+    parity.assert_triggers(f.triggers(), out, w.rho_thresh, w.window, 16, template_ids=ids)
+    rho_o, chi_o, _, _ = oracle.filter_template(s64, Sn, *w.masses[17], 16)
+    rho_g, chi_g = f.series(17)
+    parity.assert_series(rho_g, chi_g, rho_o, chi_o, 16, "N=2^22, p=16, template 17")
+
+
+def test_snr_only_mode_is_p1(gw):
+    # SURVEY 8(f)-2 / PAPER.md:164 (the pipeline without chi^2): p = 1 is one band = the whole template, i.e.
+    # one inverse FFT per template; rho and the triggers must equal those of the p = 16 run, chi^2 == 0
+    w = inputs.workload(1, 24)
+    s = inputs.segment(w).astype(np.float32)
+    f16 = _run_gpu(gw, w, s, w.psd)
+    f1 = _run_gpu(gw, w, s, w.psd, p=1)
+    t16, t1 = f16.triggers(), f1.triggers()
+    out = oracle.filter_bank(s.astype(np.float64), w.psd, w.masses, 1, w.window, w.rho_thresh)
+    parity.assert_triggers(t1, out, w.rho_thresh, w.window, 1)
+    assert np.all(t1["chisq"] == 0.0)
+    k16 = {(int(t["template_id"]), int(t["sample"])): float(t["rho"]) for t in t16}
+    k1 = {(int(t["template_id"]), int(t["sample"])): float(t["rho"]) for t in t1}
+    common = set(k16) & set(k1)
+    assert len(common) >= 0.9 * max(len(k16), 1)          # cells within 1e-3 of threshold / a rival peak may differ
+    assert all(abs(k16[c] - k1[c]) <= 1e-3 + 1e-4 * k16[c] for c in common)
+
+
 def test_config3_stream_segments_sampled(gw):
     w = inputs.workload(3)
     x = inputs.stream(w).astype(np.float32)
