@@ -37,6 +37,28 @@ from paper_0906_4175_b200 import inputs  # noqa: E402
 
 METRIC = "template-segments/sec at N=2^20, p=16 (SNR+chi^2)"
 UNIT = "template-segments/s"
+
+# --workload: the default is the headline config; the others are the "next" rows of SURVEY.md 8(f), measured
+# with the same protocol (their lines are context, not the contract's metric).
+WORKLOADS = {
+    "headline": dict(config=2, p=None, templates=None, metric=METRIC,
+                     text="BASELINE.json:configs[2]: N=2^20 (256 s at 4096 Hz), 1024 templates (total mass 2-34 Msun, "
+                          "grid uniform in eta and chirp mass), p=16, threshold 6, window 4096; Eq. 2 coloured Gaussian "
+                          "noise + 10 injections, seed 2 (+rank)"),
+    "snr_only": dict(config=2, p=1, templates=None, metric="template-segments/sec at N=2^20, p=1 (SNR only, PAPER.md:164)",
+                     text="SURVEY.md 8(f)-2: configs[2]'s segment and bank with p=1 (one inverse FFT per template, no chi^2)"),
+    "long16": dict(config=4, p=16, templates=None, metric="template-segments/sec at N=2^22, p=16 (SNR+chi^2)",
+                   text="SURVEY.md 8(f)-3: configs[4]'s segment (N=2^22, 1024 s) and bank (512 templates, m1,m2 in [1,2] "
+                        "Msun) with the headline p=16, threshold 5.5"),
+}
+
+
+def load_workload(name):
+    spec = WORKLOADS[name]
+    w = inputs.workload(spec["config"], spec["templates"])
+    if spec["p"] is not None:
+        w.p = spec["p"]
+    return w, spec
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback, only if MEASURED_PEAKS.json is absent
 
 
@@ -135,12 +157,10 @@ def oracle_rate(w, s64, Sn, n_templates: int, threads: int):
 
 def base_line(args, w, value, ms_per_step, dtype):
     return {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "metric": WORKLOADS[args.workload]["metric"], "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": dtype, "data": "synthetic",
-        "config": {"workload": "BASELINE.json:configs[2]: N=2^20 (256 s at 4096 Hz), 1024 templates "
-                               "(total mass 2-34 Msun, grid uniform in eta and chirp mass), p=16, threshold 6, "
-                               "window 4096; Eq. 2 coloured Gaussian noise + 10 injections, seed 2 (+rank)",
+        "config": {"workload": WORKLOADS[args.workload]["text"],
                    "n": w.n, "templates": len(w.masses), "p": w.p, "window": w.window,
                    "rho_thresh": w.rho_thresh, "units_per_step": len(w.masses) * args.gpus},
     }
@@ -150,7 +170,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = inputs.workload(2)
+    w, _ = load_workload(args.workload)
     s64 = inputs.segment(w).astype(np.float32).astype(np.float64)
     Sn = w.psd
     cores = min(host_cores(), 32)
@@ -163,7 +183,7 @@ def run_reference(args):
         t_total += dt
     value = per_step * args.steps / t_total
     line = base_line(args, w, value, 1e3 * t_total / args.steps, "f64")
-    sample = f"{per_step} of the 1024 templates per step (evenly spread over the bank), full N=2^20 segment, p=16"
+    sample = f"{per_step} of the {len(w.masses)} templates per step (evenly spread over the bank), full N={w.n} segment, p={w.p}"
     line["impl"] = "reference"
     line["config"]["units_per_step"] = per_step
     line["config"]["sample"] = sample
@@ -194,7 +214,7 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    w = inputs.workload(2)
+    w, _ = load_workload(args.workload)
     seed_off, first, count = shard_plan(world, rank, len(w.masses))
     w.seed += seed_off
     s32 = inputs.segment(w).astype(np.float32)
@@ -271,8 +291,9 @@ def run_gpu(args):
 
     if rank == 0:
         line = base_line(args, w, value, ms / args.steps, "f32")
-        line["config"]["l2"] = ("no flush: every launch streams a band intermediate of batch*p*N*8 B = 2 GiB, "
-                                "16x the 126 MB L2, through pass 1 (write) and pass 2 (read)")
+        line["config"]["l2"] = ("no flush: every launch streams a band intermediate of batch*p*N*8 B = %.2f GiB, "
+                                "%.0fx the 126 MB L2, through pass 1 (write) and pass 2 (read)"
+                                % (bytes_per_launch[0] / 2**30, bytes_per_launch[0] / 126e6))
         line["config"]["batch_templates_per_launch"] = float(batch_templates[0])
         line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(s32.nbytes + Sn.nbytes),
                        "d2h_bytes_per_step": int(12 + trig.nbytes), "ms_per_step": ms_e2e / args.steps}
@@ -281,7 +302,8 @@ def run_gpu(args):
         line["triggers_per_step"] = int(len(trig))
         line["roofline"] = {
             "bound": "hbm", "kernel": names[dom], "achieved": float(gbs[dom]), "peak": peak, "unit": "GB/s",
-            "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": TRAFFIC_BYTES_PER_TEMPLATE[dom] * float(batch_templates[dom]),
+            "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": (TRAFFIC_BYTES_PER_TEMPLATE[dom] * float(batch_templates[dom])
+                                                                  if args.workload == "headline" else None),
             "bytes_per_launch": float(bytes_per_launch[dom]), "avg_launch_ms": float(avg_ms[dom]),
             "kernels": {"k_pass1": {"avg_launch_ms": float(avg_ms[0]), "GB/s": float(gbs[0]), "frac": float(gbs[0] / peak),
                                     "share_of_step": float(k_ms[0] / k_ms.sum())},
@@ -297,8 +319,8 @@ def run_gpu(args):
             nt = cores * (2 if cores <= 16 else 1)
             rate, dt = oracle_rate(w, s32.astype(np.float64), Sn, nt, cores)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": f"{nt} of the 1024 templates (evenly spread), full N=2^20 segment, "
-                                              f"p=16, {dt:.1f} s wall",
+                                    "sample": f"{nt} of the {T} templates (evenly spread), full N={w.n} segment, "
+                                              f"p={w.p}, {dt:.1f} s wall",
                                     "context": "paper: 16x total speed-up, GeForce 8800 Ultra vs one 2.5 GHz Q9300 core "
                                                "(PAPER.md:5) -- other hardware, context only"}
         print(json.dumps(line), flush=True)
@@ -320,6 +342,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="gwmf", choices=["gwmf", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="headline", choices=sorted(WORKLOADS))
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
