@@ -41,11 +41,9 @@ __device__ __forceinline__ float2 cis_frac(unsigned num, int log_n) {
 }
 
 template <int NA, int NB, bool DENSE>
-__global__ void __launch_bounds__(256) k_pass1(P1Args a) {
+__global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
   constexpr int FR = NA >= 32 ? 32 : NA;        // stage-1 transform length = ja outputs per CTA
   constexpr int G = NA / FR;                    // residues r of ja = G m + r
-  constexpr int GA = NA >= 32 ? 16 : NA;        // inputs a per group
-  constexpr int NGROUPS = NA / GA;
   constexpr int C = kColsPerCta;
   constexpr int SROW = NB * C + C;              // padded stride of S[m][..] in float2
   constexpr int TILES = kN2 / C;
@@ -93,50 +91,39 @@ __global__ void __launch_bounds__(256) k_pass1(P1Args a) {
     __syncthreads();
 
     // ---------------------------------------------------------------- stage 1: thread (b = x, c)
+    // V[ja][b] = sum_a Q[NB a + b] w_NA^{ja a} with ja = G m + r, a = a' + FR g:  w_NA^{ja a} = w_FR^{m a'} w_NA^{r a},
+    // so the G inputs that share a' are combined first and ONE FR-point transform over a' follows.
     if (x < NB) {
       const int b = x;
-      float2 acc[FR];
+      float2 xin[FR];
 #pragma unroll
-      for (int m = 0; m < FR; ++m) acc[m] = make_float2(0.f, 0.f);
-#pragma unroll 1
-      for (int g = 0; g < NGROUPS; ++g) {
-        const int a_base = GA * g;
-        if (a_base > a_hi || a_base + GA - 1 < a_lo) continue;
-        float2 xin[FR];
+      for (int ap = 0; ap < FR; ++ap) {
+        float2 sum = make_float2(0.f, 0.f);
 #pragma unroll
-        for (int ap = 0; ap < FR; ++ap) {
-          float2 q = make_float2(0.f, 0.f);
-          if (ap < GA) {
-            const int aa = a_base + ap;
-            const int k = ((NB * aa + b) << kLogN2) + k2;
-            if (aa >= a_lo && aa <= a_hi && k >= e_lo && k < e_hi) {
-              if constexpr (DENSE) {
-                q = a.dense_in[k];
-              } else {
-                q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + k];      // Q_I[k] from k_correlate
-              }
-              if constexpr (G > 1) {
-                if (r > 0) q = cmul(q, a.tw_n1[(r * ap * NB) % n1]);       // w_NA^{r a'}
-              }
+        for (int g = 0; g < G; ++g) {
+          const int aa = ap + FR * g;
+          const int k = ((NB * aa + b) << kLogN2) + k2;
+          if (aa >= a_lo && aa <= a_hi && k >= e_lo && k < e_hi) {
+            float2 q;
+            if constexpr (DENSE) {
+              q = a.dense_in[k];
+            } else {
+              q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + k];      // Q_I[k] from k_correlate
             }
+            if constexpr (G > 1) {
+              if (r > 0) q = cmul(q, a.tw_n1[(r * aa * NB) % n1]);         // w_NA^{r a}
+            }
+            sum = cadd(sum, q);
           }
-          xin[ap] = q;
         }
-        fft_dif<FR>(xin);
-#pragma unroll
-        for (int m = 0; m < FR; ++m) {
-          float2 v = xin[brev<FR>(m)];
-          if constexpr (NGROUPS > 1) {
-            if (g > 0) v = cmul(v, a.tw_n1[(a_base * (G * m + r) * NB) % n1]);   // w_NA^{a_base ja}
-          }
-          acc[m] = cadd(acc[m], v);
-        }
+        xin[ap] = sum;
       }
+      fft_dif<FR>(xin);
 #pragma unroll
       for (int m = 0; m < FR; ++m) {
         const int ja = G * m + r;
         const float2 tw = cmul(a.tw_n1[(ja * b) % n1], A[m * C + c]);   // e^{2 pi i ja (1024 b + k2)/n}
-        S[m * SROW + b * C + c] = cmul(acc[m], tw);
+        S[m * SROW + b * C + c] = cmul(xin[brev<FR>(m)], tw);
       }
     }
     __syncthreads();
