@@ -60,6 +60,15 @@ __device__ __forceinline__ void slot_max(Slot* s, unsigned long long key, unsign
   }
 }
 
+// Rare path of the epilogue, kept out of line so that the 32-fold unrolled epilogue stays small (at p = 1
+// it runs on every 8 KB row and must not thrash the instruction cache).
+__device__ __noinline__ void emit_candidate(Slot* slots_t, unsigned j, float rho2, float chi, float thresh, int log_w) {
+  const float rho = sqrtf(rho2);
+  if (rho > thresh)
+    slot_max(slots_t + (j >> log_w), ((unsigned long long)__float_as_uint(rho) << 32) | (unsigned long long)(0xFFFFFFFFu - j),
+             (unsigned long long)__float_as_uint(chi));
+}
+
 // ---- TMA (bulk async copy) + mbarrier helpers --------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
@@ -94,7 +103,7 @@ constexpr int kRowBytes = kN2 * (int)sizeof(float2);      // 8 KB
 constexpr int kP2Ring = 3;                                // row buffers per warp
 
 // Shared memory: [twiddles 32x32][warp 0: ring of kP2Ring rows][warp 1: ...]...[mbarriers, kP2Ring per warp].
-template <bool STORE>
+template <bool STORE, bool SERIES>
 __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
   extern __shared__ __align__(128) float2 smem2[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -180,26 +189,21 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
       if (++l == p) {
         // ---- epilogue of one row: rho, chi^2 and the trigger slots (steps a4, a5) ----
         const int tb = row >> a.log_n1, j1 = row & n1_mask;
-        const TemplateMeta* m = a.meta + tb;
-        const float scale = m->scale_rho2;
-        const float fp = (float)p, inv_p = 1.0f / (float)p;
-        const float thr2 = a.thresh * a.thresh;
+        const float scale = __ldg(&a.meta[tb].scale_rho2);
+        const float fp_scale = (float)p * scale, inv_p = 1.0f / (float)p;
+        const float thr2 = a.thresh * a.thresh * 0.999f;
+        Slot* slots_t = a.slots ? a.slots + (size_t)tb * a.n_windows : nullptr;
 #pragma unroll
         for (int jc = 0; jc < 32; ++jc) {
           const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
           const float rho2 = z2 * scale;                                        // Eq. 3 squared
-          const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * (fp * scale);     // Eq. 5
+          const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * fp_scale;         // Eq. 5
           const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
-          if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
-          if (a.series_chi) a.series_chi[j] = chi;
-          if (a.slots && rho2 > thr2 * 0.999f) {
-            const float rho = sqrtf(rho2);
-            if (rho > a.thresh) {
-              Slot* s = a.slots + (size_t)tb * a.n_windows + (j >> a.log_w);
-              slot_max(s, ((unsigned long long)__float_as_uint(rho) << 32) | (unsigned long long)(0xFFFFFFFFu - j),
-                       (unsigned long long)__float_as_uint(chi));
-            }
+          if constexpr (SERIES) {
+            if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
+            if (a.series_chi) a.series_chi[j] = chi;
           }
+          if (rho2 > thr2 && slots_t) emit_candidate(slots_t, j, rho2, chi, a.thresh, a.log_w);
           az[jc] = make_float2(0.f, 0.f);
           aq[jc] = 0.f;
         }
@@ -215,8 +219,9 @@ constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(fl
 static cudaError_t p2_configure() {
   static bool done = false;
   if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(k_pass2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  cudaError_t e = cudaFuncSetAttribute(k_pass2<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   done = (e == cudaSuccess);
   return e;
 }
@@ -246,7 +251,8 @@ cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots,
   a.thresh = (float)c->prm.rho_thresh;
   cudaError_t e = p2_configure();
   if (e != cudaSuccess) return e;
-  k_pass2<false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  if (series_rho || series_chi) k_pass2<false, true><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  else k_pass2<false, false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
   c->launches++;
   return cudaGetLastError();
 }
@@ -269,7 +275,7 @@ cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
   a.thresh = 0.f;
   cudaError_t e = p2_configure();
   if (e != cudaSuccess) return e;
-  k_pass2<true><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  k_pass2<true, false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
   c->launches++;
   return cudaGetLastError();
 }
