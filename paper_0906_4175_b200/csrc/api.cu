@@ -61,6 +61,7 @@ Layout make_layout(const gwmf_params* p) {
   L.tw_p2 = take(1024 * sizeof(float2));
   L.meta = take(T * sizeof(TemplateMeta));
   L.slots = take(T * nw * sizeof(Slot));
+  L.masks = take(T * sizeof(uint32_t));
   L.counts = take(T * sizeof(int));
   L.offsets = take((T + 1) * sizeof(long long));
   L.trig_out = take(T * nw * sizeof(gwmf_trigger));
@@ -155,16 +156,21 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->have_bank = c->have_segment = false;
   c->launches = 0;
   c->h_meta = nullptr;
+  c->h_masks = nullptr;
   c->side = nullptr;
-  c->ev_fork = c->ev_join = nullptr;
+  c->ev_fork = c->ev_join = c->ev_masks = nullptr;
   {
     int lo = 0, hi = 0;
     cudaDeviceGetStreamPriorityRange(&lo, &hi);
     if (cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, hi) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_masks, cudaEventDisableTiming) != cudaSuccess ||
+        cudaMallocHost((void**)&c->h_masks, sizeof(uint32_t) * (size_t)params->max_templates) != cudaSuccess) {
       if (c->side) cudaStreamDestroy(c->side);
       if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+      if (c->ev_join) cudaEventDestroy(c->ev_join);
+      if (c->ev_masks) cudaEventDestroy(c->ev_masks);
       delete c;
       return GWMF_E_CUDA;
     }
@@ -191,6 +197,8 @@ void gwmf_destroy(gwmf_ctx* ctx) {
   if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
+  if (c->ev_masks) cudaEventDestroy(c->ev_masks);
+  if (c->h_masks) cudaFreeHost(c->h_masks);
   if (c->h_meta) cudaFreeHost(c->h_meta);
   delete c;
 }

@@ -34,7 +34,7 @@ struct alignas(16) Slot {
 };
 
 struct Layout {                  // byte offsets into the caller's workspace
-  size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, slots, counts, offsets, trig_out,
+  size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, slots, counts, offsets, trig_out,
          series_rho, series_chi, flags, q, y, total;
   size_t y_bytes;
   int batch;
@@ -60,6 +60,8 @@ struct Ctx {
   int64_t launches;
   std::string cuda_err;
   TemplateMeta* h_meta;          // host staging of the bank (pinned)
+  uint32_t* h_masks;             // host mirror of TemplateMeta::wide_mask (pinned), valid once ev_masks has fired
+  cudaEvent_t ev_masks;
 };
 
 // ---- launchers (defined in the .cu files) --------------------------------------------------------

@@ -406,16 +406,27 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   // read the band buffer) precedes the side work
   if ((e = cudaEventRecord(c->ev_fork, c->stream)) != cudaSuccess) return e;
   if ((e = cudaStreamWaitEvent(c->side, c->ev_fork, 0)) != cudaSuccess) return e;
-  if (c->nb == 32) {
+  // which kernels have anything to do: host mirror of the wide-band masks (written by k_bank_setup; the event
+  // has normally fired long before the first filter call)
+  if ((e = cudaEventSynchronize(c->ev_masks)) != cudaSuccess) return e;
+  const uint32_t full = c->prm.p >= 32 ? 0xFFFFFFFFu : ((1u << c->prm.p) - 1u);
+  bool any_wide = false, any_narrow = false;
+  for (int t = first; t < first + count; ++t) {
+    any_wide |= c->h_masks[t] != 0u;
+    any_narrow |= c->h_masks[t] != full;
+  }
+  if (any_narrow) {
     // narrow bands write the A layout directly
     e = launch_narrow(c, args, count);
     if (e != cudaSuccess) return e;
   }
-  // wide bands (every band if n1 < 32): generic kernel in the plain layout, then the row stage in place
-  e = dispatch_p1<false>(c, args, c->side);
-  if (e != cudaSuccess) return e;
-  e = launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 1, c->side);
-  if (e != cudaSuccess) return e;
+  if (any_wide) {
+    // wide bands (every band if n1 < 32): generic kernel in the plain layout, then the row stage in place
+    e = dispatch_p1<false>(c, args, c->side);
+    if (e != cudaSuccess) return e;
+    e = launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 1, c->side);
+    if (e != cudaSuccess) return e;
+  }
   if (next_count > 0) {
     e = launch_correlate(c, next_first, next_count, parity ^ 1, c->side);
     if (e != cudaSuccess) return e;

@@ -138,8 +138,8 @@ cudaError_t launch_segment_prepare(Ctx* c) {
 //   sigma^2 = 4 df C[k_high-1];  e_0 = k_low;  e_l = 1 + min{k : C[k] >= (l/p) C[k_high-1]};  e_p = k_high.
 // One thread per template; the edges are binary searches in the monotone fp64 table.
 // ---------------------------------------------------------------------------------------------------
-__global__ void k_bank_setup(TemplateMeta* __restrict__ meta, const double* __restrict__ c_tab, int n_templates,
-                             int p, int k_low, int half_n, double four_df, int all_wide) {
+__global__ void k_bank_setup(TemplateMeta* __restrict__ meta, uint32_t* __restrict__ masks, const double* __restrict__ c_tab,
+                             int n_templates, int p, int k_low, int half_n, double four_df, int all_wide) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n_templates) return;
   TemplateMeta m = meta[t];
@@ -167,15 +167,22 @@ __global__ void k_bank_setup(TemplateMeta* __restrict__ meta, const double* __re
     if (all_wide || rows > 32) mask |= 1u << l;
   }
   m.wide_mask = mask;
+  masks[t] = mask;
   meta[t] = m;
 }
 
 cudaError_t launch_bank_setup(Ctx* c) {
   k_bank_setup<<<(c->n_templates + 127) / 128, 128, 0, c->stream>>>(
-      ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<double>(c, c->lay.c_tab), c->n_templates, c->prm.p, c->k_low,
-      (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1);
+      ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<uint32_t>(c, c->lay.masks), ws_ptr<double>(c, c->lay.c_tab),
+      c->n_templates, c->prm.p, c->k_low, (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1);
   c->launches++;
-  return cudaGetLastError();
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  // host mirror of the wide-band masks: lets gwmf_filter skip kernels that would find nothing to do
+  e = cudaMemcpyAsync(c->h_masks, ws_ptr<uint32_t>(c, c->lay.masks), sizeof(uint32_t) * (size_t)c->n_templates,
+                      cudaMemcpyDeviceToHost, c->stream);
+  if (e != cudaSuccess) return e;
+  return cudaEventRecord(c->ev_masks, c->stream);
 }
 
 }  // namespace gwmf
