@@ -127,6 +127,13 @@ int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges);
  * touch trigger slots.  syncs. */
 int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host_chisq);
 
+/* Debug/parity: the correlate step alone (Eq. 1 integrand).  host_q receives n/2 interleaved
+ * complex fp32 values Q[k] = (4/n) D[k] f_k^(-7/6) e^{+i Psi0(f_k)} / (S_n[k] sigma_ref) for k_low <= k < k_high of
+ * template `template_id` and 0 elsewhere, with D the forward DFT of the loaded segment and
+ * sigma_ref^2 = 4 df sum_{k_low <= k < n/2} f_k^(-7/3)/S_n[k] (the library's internal normalisation, which
+ * cancels in rho and chi^2).  HOST array of n floats.  Needs a bank and a segment.  syncs. */
+int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q);
+
 /* Debug/parity: the library's batched complex FFT alone.  X[k] = sum_j x[j] e^{+2 pi i jk/n}
  * (unnormalised inverse transform, the e^{2 pi i f t} of Eq. 1).  in/out: DEVICE arrays of n
  * interleaved complex fp32 (re, im), n = params.n; in != out.  async. */

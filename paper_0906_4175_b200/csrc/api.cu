@@ -375,6 +375,22 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
   return GWMF_OK;
 }
 
+int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q) {
+  if (!ctx || !host_q) return GWMF_E_ARG;
+  Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
+  if (template_id < 0 || template_id >= c->n_templates) return GWMF_E_ARG;
+  int rc = check_flags(c);
+  if (rc != GWMF_OK) return rc;
+  const size_t half = (size_t)(c->n / 2);
+  float2* d_q = ws_ptr<float2>(c, c->lay.q);
+  CU(cudaMemsetAsync(d_q, 0, half * sizeof(float2), c->stream));      // bins outside [k_low, k_high) are not written
+  CU(launch_correlate(c, template_id, 1, 0, c->stream));
+  CU(cudaMemcpyAsync(host_q, d_q, half * sizeof(float2), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return GWMF_OK;
+}
+
 int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out) {
   if (!ctx || !d_in || !d_out || d_in == d_out) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);

@@ -69,6 +69,7 @@ cudaError_t launch_tables(Ctx* c);
 cudaError_t launch_segment_prepare(Ctx* c);                       // after s/Sn are on the device
 cudaError_t launch_bank_setup(Ctx* c);
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready);
+cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st);
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
 cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid);
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,

@@ -369,7 +369,7 @@ static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, 
   return cudaGetLastError();
 }
 
-static cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   const int half = (int)(c->n / 2);
   k_correlate<<<dim3(half / 256, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, ws_ptr<float2>(c, c->lay.wq),
                                                       ws_ptr<double>(c, c->lay.u_tab),

@@ -19,7 +19,8 @@ OK, E_ARG, E_EMPTY_TEMPLATE, E_STATE, E_CAPACITY, E_CUDA, E_WORKSPACE = 0, -1, -
 
 EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
-    "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_series", "gwmf_fft_inverse",
+    "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_series", "gwmf_correlate",
+    "gwmf_fft_inverse",
     "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
 
@@ -67,6 +68,7 @@ def load_library():
     L.gwmf_sigma.argtypes = [C.c_void_p, C.c_void_p]
     L.gwmf_band_edges.argtypes = [C.c_void_p, C.c_void_p]
     L.gwmf_series.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    L.gwmf_correlate.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     L.gwmf_fft_inverse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.gwmf_launch_count.argtypes = [C.c_void_p]
     L.gwmf_launch_count.restype = C.c_int64
@@ -212,6 +214,11 @@ class Filter:
         self._check(self._L.gwmf_series(self._h, int(template_id), rho.ctypes.data_as(C.c_void_p),
                                         chi.ctypes.data_as(C.c_void_p)))
         return rho, chi
+
+    def correlate(self, template_id) -> np.ndarray:
+        q = np.empty(self.n // 2, dtype=np.complex64)
+        self._check(self._L.gwmf_correlate(self._h, int(template_id), q.ctypes.data_as(C.c_void_p)))
+        return q
 
     def fft_inverse(self, x):
         """x: torch complex64 device tensor of n points -> unnormalised e^{+2 pi i jk/n} transform."""

@@ -54,6 +54,44 @@ def test_fft_inverse_alone(gw, log_n):
     assert np.max(np.abs(T - tone)) < 2e-6
 
 
+# ----------------------------------------------------------------------------- the correlate step alone
+@pytest.mark.parametrize("log_n,masses", [(14, (8.0, 8.0)), (18, (1.0, 1.0)), (20, (1.4, 1.4))])
+def test_correlate_alone(gw, log_n, masses):
+    # Q[k] = (4/n) D[k] f^(-7/6) e^{i Psi0} / (S_n sigma_ref) against the oracle's template and data spectrum.
+    # (1,1) Msun at 40 Hz carries Psi0 = 6.7e3 rad: a phase evaluated in fp32 would be off by 1e-3 rad.
+    n = 1 << log_n
+    m1, m2 = masses
+    s = inputs.time_series(inputs.noise_spectrum(n, 300 + log_n), n).astype(np.float32)
+    Sn = inputs.psd_array(n)
+    f = gw.Filter(n, 4, 4096, 1)
+    f.make_bank([masses])
+    f.load_segment(s, Sn)
+    q = f.correlate(0).astype(np.complex128)
+    D = oracle.data_spectrum(s.astype(np.float64))[: n // 2]
+    h = oracle.template(m1, m2, n)                        # f^(-7/6) e^{i Psi0} on [k_low, k_high), 0 elsewhere
+    Ctab = oracle.power_table(Sn, n)
+    df = inputs.FS / n
+    sigma_ref = math.sqrt(4.0 * df * Ctab[n // 2 - 1])
+    inv_sn = np.zeros(n // 2)
+    k_low = int(math.ceil(inputs.F_LOW / df))
+    inv_sn[k_low:] = 1.0 / Sn[k_low:n // 2]
+    want = (4.0 / n) * D * h * inv_sn / sigma_ref
+    scale = np.sqrt(np.mean(np.abs(want[np.abs(want) > 0]) ** 2))
+    assert np.count_nonzero(want) > 100
+    assert np.all(q[want == 0] == 0)
+    # the library's data spectrum comes from its fp32 FFT: absolute error ~ 1e-6 * rms(D) in every bin, carried
+    # into Q by the bin's weight; the template phasor and the fp32 products add ~1e-6 relative
+    weight = np.abs((4.0 / n) * h * inv_sn / sigma_ref)
+    rms_d = np.sqrt(np.mean(np.abs(D[k_low:]) ** 2))
+    err = np.abs(q - want) - (3e-6 * np.abs(want) + 4e-6 * rms_d * weight)
+    assert np.max(err) <= 0, (int(np.argmax(err)), q[int(np.argmax(err))], want[int(np.argmax(err))], scale)
+    # phase alone, bin by bin, on the bins at or above the rms (there the fp32 FFT of the data contributes
+    # ~1e-6 rad, the fp64-reduced template phase 4e-7, the fp32 products 1e-7)
+    big = (np.abs(D) > rms_d) & (np.abs(want) > 0)
+    dphi = np.angle(q[big] / want[big])
+    assert np.max(np.abs(dphi)) < 4e-6, np.max(np.abs(dphi))
+
+
 # ----------------------------------------------------------------------------- config 0, everything
 def test_config0_full(gw):
     w = inputs.workload(0)
