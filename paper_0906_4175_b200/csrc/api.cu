@@ -62,6 +62,7 @@ Layout make_layout(const gwmf_params* p) {
   L.meta = take(T * sizeof(TemplateMeta));
   L.slots = take(T * nw * sizeof(Slot));
   L.masks = take(T * sizeof(uint32_t));
+  L.prefix_totals = take(1024 * sizeof(double));
   L.counts = take(T * sizeof(int));
   L.offsets = take((T + 1) * sizeof(long long));
   L.trig_out = take(T * nw * sizeof(gwmf_trigger));

@@ -34,7 +34,7 @@ struct alignas(16) Slot {
 };
 
 struct Layout {                  // byte offsets into the caller's workspace
-  size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, slots, counts, offsets, trig_out,
+  size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
          series_rho, series_chi, flags, q, y, total;
   size_t y_bytes;
   int batch;

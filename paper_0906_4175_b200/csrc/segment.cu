@@ -64,26 +64,42 @@ __global__ void k_power_terms(const double* __restrict__ sn, const double* __res
   g[k] = v;
 }
 
-// Inclusive fp64 prefix sum C[k] = sum_{k' <= k} g[k'] with a fixed summation order: one CTA of 1024
-// threads, thread t sums the contiguous chunk [t*L, (t+1)*L) sequentially, chunk totals are scanned
-// sequentially by thread 0, then every thread rewrites its chunk.  (Once per segment; 4 MiB.)
-__global__ void __launch_bounds__(1024) k_prefix(const double* __restrict__ g, double* __restrict__ c_tab,
-                                                 int half_n) {
-  __shared__ double part[1024];
-  int t = threadIdx.x;
-  int L = (half_n + 1023) / 1024;
-  int lo = t * L, hi = min(lo + L, half_n);
-  double acc = 0.0;
-  for (int k = lo; k < hi; ++k) acc += g[k];
-  part[t] = acc;
-  __syncthreads();
-  if (t == 0) {
-    double run = 0.0;
-    for (int i = 0; i < 1024; ++i) { double v = part[i]; part[i] = run; run += v; }
+// Inclusive fp64 prefix sum C[k] = sum_{k' <= k} g[k'] with a FIXED summation order (so that sigma and the band
+// edges are bit-reproducible): the table is cut into 1024 contiguous chunks of L entries; a chunk is summed
+// sequentially, the chunk totals are scanned sequentially, and every chunk is then re-summed from its offset.
+// One warp per chunk: coalesced loads into shared memory, one lane walks the chunk (the dependent chain of L
+// fp64 adds is ~2 us), coalesced stores.  (Once per segment; 4 MiB.)
+constexpr int kPrefixChunks = 1024;
+
+__global__ void __launch_bounds__(32) k_prefix_totals(const double* __restrict__ g, double* __restrict__ totals, int half_n, int L) {
+  extern __shared__ double sh[];
+  const int lo = blockIdx.x * L, hi = min(lo + L, half_n);
+  for (int k = lo + threadIdx.x; k < hi; k += 32) sh[k - lo] = g[k];
+  __syncwarp();
+  if (threadIdx.x == 0) {
+    double acc = 0.0;
+    for (int k = 0; k < hi - lo; ++k) acc += sh[k];
+    totals[blockIdx.x] = acc;
   }
-  __syncthreads();
-  acc = part[t];
-  for (int k = lo; k < hi; ++k) { acc += g[k]; c_tab[k] = acc; }
+}
+
+__global__ void k_prefix_scan(double* __restrict__ totals) {      // exclusive, sequential
+  double run = 0.0;
+  for (int i = 0; i < kPrefixChunks; ++i) { const double v = totals[i]; totals[i] = run; run += v; }
+}
+
+__global__ void __launch_bounds__(32) k_prefix_write(const double* __restrict__ g, const double* __restrict__ offsets,
+                                                     double* __restrict__ c_tab, int half_n, int L) {
+  extern __shared__ double sh[];
+  const int lo = blockIdx.x * L, hi = min(lo + L, half_n);
+  for (int k = lo + threadIdx.x; k < hi; k += 32) sh[k - lo] = g[k];
+  __syncwarp();
+  if (threadIdx.x == 0) {
+    double acc = offsets[blockIdx.x];
+    for (int k = 0; k < hi - lo; ++k) { acc += sh[k]; sh[k] = acc; }
+  }
+  __syncwarp();
+  for (int k = lo + threadIdx.x; k < hi; k += 32) c_tab[k] = sh[k - lo];
 }
 
 // wq[k] = (4/n) conj(Z[k]) f_k^(-7/6) / S_n[k] / sigma_ref for k_low <= k < n/2, else 0, where
@@ -125,7 +141,16 @@ cudaError_t launch_segment_prepare(Ctx* c) {
   cudaMemsetAsync(flags, 0, sizeof(int), c->stream);
   k_power_terms<<<(half + 255) / 256, 256, 0, c->stream>>>(ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab),
                                                            ws_ptr<double>(c, c->lay.g_tab), flags, c->k_low, half);
-  k_prefix<<<1, 1024, 0, c->stream>>>(ws_ptr<double>(c, c->lay.g_tab), ws_ptr<double>(c, c->lay.c_tab), half);
+  {
+    const int L = (half + kPrefixChunks - 1) / kPrefixChunks;
+    const size_t sm = (size_t)L * sizeof(double);
+    double* totals = ws_ptr<double>(c, c->lay.prefix_totals);
+    k_prefix_totals<<<kPrefixChunks, 32, sm, c->stream>>>(ws_ptr<double>(c, c->lay.g_tab), totals, half, L);
+    k_prefix_scan<<<1, 1, 0, c->stream>>>(totals);
+    k_prefix_write<<<kPrefixChunks, 32, sm, c->stream>>>(ws_ptr<double>(c, c->lay.g_tab), totals,
+                                                         ws_ptr<double>(c, c->lay.c_tab), half, L);
+    c->launches += 2;
+  }
   k_weighted_spectrum<<<(half + 255) / 256, 256, 0, c->stream>>>(
       Z, ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab), ws_ptr<double>(c, c->lay.c_tab),
       ws_ptr<float2>(c, c->lay.wq), c->k_low, half, 4.0 / (double)c->n, 4.0 * c->df);
@@ -136,43 +161,58 @@ cudaError_t launch_segment_prepare(Ctx* c) {
 // ---------------------------------------------------------------------------------------------------
 // sigma and band edges of every template (Eq. 4; equal-power bands):
 //   sigma^2 = 4 df C[k_high-1];  e_0 = k_low;  e_l = 1 + min{k : C[k] >= (l/p) C[k_high-1]};  e_p = k_high.
-// One thread per template; the edges are binary searches in the monotone fp64 table.
+// One thread per (template, edge); the edges are binary searches in the monotone fp64 table.
 // ---------------------------------------------------------------------------------------------------
-__global__ void k_bank_setup(TemplateMeta* __restrict__ meta, uint32_t* __restrict__ masks, const double* __restrict__ c_tab,
-                             int n_templates, int p, int k_low, int half_n, double four_df, int all_wide) {
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= n_templates) return;
-  TemplateMeta m = meta[t];
-  double total = c_tab[m.k_high - 1];
-  double ref = c_tab[half_n - 1];
-  m.sigma = sqrt(four_df * total);
-  m.scale_rho2 = (float)(ref / total);
-  m.edges[0] = k_low;
-  for (int l = 1; l < p; ++l) {
-    double target = ((double)l / (double)p) * total;
-    int lo = k_low, hi = m.k_high - 1;          // smallest k in [lo, hi] with C[k] >= target
-    while (lo < hi) {
-      int mid = (lo + hi) >> 1;
-      if (c_tab[mid] >= target) hi = mid; else lo = mid + 1;
+__global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ meta, uint32_t* __restrict__ masks,
+                                                    const double* __restrict__ c_tab, int n_templates, int p, int k_low,
+                                                    int half_n, double four_df, int all_wide) {
+  // thread (l = threadIdx.x, template = 8 blockIdx.x + threadIdx.y): one band edge each, then the wide-band mask
+  __shared__ int s_edges[8][kMaxBands + 1];
+  const int l = threadIdx.x, ty = threadIdx.y;
+  const int t = blockIdx.x * 8 + ty;
+  const bool live = t < n_templates;
+  int k_high = 0;
+  double total = 0.0;
+  if (live) {
+    k_high = meta[t].k_high;
+    total = c_tab[k_high - 1];
+    int e;
+    if (l == 0) e = k_low;
+    else if (l >= p) e = k_high;
+    else {
+      const double target = ((double)l / (double)p) * total;
+      int lo = k_low, hi = k_high - 1;          // smallest k in [lo, hi] with C[k] >= target
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (c_tab[mid] >= target) hi = mid; else lo = mid + 1;
+      }
+      e = lo + 1;
     }
-    m.edges[l] = lo + 1;
+    s_edges[ty][l] = e;
+    if (l == 0) s_edges[ty][kMaxBands] = k_high;
   }
-  m.edges[p] = m.k_high;
-  for (int l = p + 1; l <= kMaxBands; ++l) m.edges[l] = m.k_high;
+  __syncthreads();
+  if (!live) return;
   // bands for the generic pass-1 kernel: more than 32 input rows (or every band when n1 < 32)
-  unsigned mask = 0u;
-  for (int l = 0; l < p; ++l) {
-    const int e_lo = m.edges[l], e_hi = m.edges[l + 1];
+  bool wide = false;
+  if (l < p) {
+    const int e_lo = s_edges[ty][l], e_hi = s_edges[ty][l + 1];
     const int rows = e_hi > e_lo ? ((e_hi - 1) >> kLogN2) - (e_lo >> kLogN2) + 1 : 0;
-    if (all_wide || rows > 32) mask |= 1u << l;
+    wide = all_wide || rows > 32;
   }
-  m.wide_mask = mask;
-  masks[t] = mask;
-  meta[t] = m;
+  const unsigned mask = __ballot_sync(0xFFFFFFFFu, wide);
+  meta[t].edges[l] = s_edges[ty][l];
+  if (l == 0) {
+    meta[t].edges[kMaxBands] = k_high;
+    meta[t].sigma = sqrt(four_df * total);
+    meta[t].scale_rho2 = (float)(c_tab[half_n - 1] / total);
+    meta[t].wide_mask = mask;
+    masks[t] = mask;
+  }
 }
 
 cudaError_t launch_bank_setup(Ctx* c) {
-  k_bank_setup<<<(c->n_templates + 127) / 128, 128, 0, c->stream>>>(
+  k_bank_setup<<<(c->n_templates + 7) / 8, dim3(32, 8), 0, c->stream>>>(
       ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<uint32_t>(c, c->lay.masks), ws_ptr<double>(c, c->lay.c_tab),
       c->n_templates, c->prm.p, c->k_low, (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1);
   c->launches++;
