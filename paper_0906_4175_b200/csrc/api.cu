@@ -307,13 +307,15 @@ int gwmf_triggers(gwmf_ctx* ctx, gwmf_trigger* host_out, int64_t capacity, int64
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
   *n_out = 0;
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
-  int rc = check_flags(c);
-  if (rc != GWMF_OK) return rc;
+  // compaction first, then ONE synchronisation for the input-check flag and the event count
   CU(launch_compact(c));
+  int flag = 0;
   long long total = 0;
+  CU(cudaMemcpyAsync(&flag, ws_ptr<int>(c, c->lay.flags), sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU(cudaMemcpyAsync(&total, ws_ptr<long long>(c, c->lay.offsets) + c->n_templates, sizeof(long long),
                      cudaMemcpyDeviceToHost, c->stream));
   CU(cudaStreamSynchronize(c->stream));
+  if (flag) return GWMF_E_ARG;
   *n_out = total;
   long long take = total < capacity ? total : capacity;
   if (take > 0) {

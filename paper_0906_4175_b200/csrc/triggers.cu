@@ -10,13 +10,18 @@ __global__ void k_reset_slots(Slot* __restrict__ slots, size_t count) {
   if (i < count) { slots[i].key = 0ull; slots[i].aux = 0ull; }
 }
 
-__global__ void k_count(const Slot* __restrict__ slots, int* __restrict__ counts, int n_templates, int n_windows) {
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
+// one warp per template: lanes look at 32 consecutive windows at a time
+__global__ void __launch_bounds__(256) k_count(const Slot* __restrict__ slots, int* __restrict__ counts, int n_templates,
+                                               int n_windows) {
+  const int t = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (t >= n_templates) return;
   const Slot* s = slots + (size_t)t * n_windows;
   int c = 0;
-  for (int w = 0; w < n_windows; ++w) c += (s[w].key != 0ull);
-  counts[t] = c;
+  for (int w0 = 0; w0 < n_windows; w0 += 32) {
+    const bool hit = (w0 + lane < n_windows) && s[w0 + lane].key != 0ull;
+    c += __popc(__ballot_sync(0xFFFFFFFFu, hit));
+  }
+  if (lane == 0) counts[t] = c;
 }
 
 // offsets[t] = sum_{t' < t} counts[t'], offsets[n_templates] = total (as long long in offsets64[0])
@@ -40,25 +45,31 @@ __global__ void __launch_bounds__(1024) k_scan(const int* __restrict__ counts, l
   for (int i = lo; i < hi; ++i) { offsets[i] = acc; acc += counts[i]; }
 }
 
-__global__ void k_emit(const Slot* __restrict__ slots, const long long* __restrict__ offsets,
-                       gwmf_trigger* __restrict__ out, long long capacity, int n_templates, int n_windows) {
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
+// one warp per template; within a template events keep window order (ballot + prefix popcount)
+__global__ void __launch_bounds__(256) k_emit(const Slot* __restrict__ slots, const long long* __restrict__ offsets,
+                                              gwmf_trigger* __restrict__ out, long long capacity, int n_templates,
+                                              int n_windows) {
+  const int t = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (t >= n_templates) return;
   const Slot* s = slots + (size_t)t * n_windows;
   long long o = offsets[t];
-  for (int w = 0; w < n_windows; ++w) {
-    unsigned long long key = s[w].key;
-    if (key != 0ull) {
-      if (o < capacity) {
-        gwmf_trigger g;
-        g.template_id = t;
-        g.sample = (int32_t)(0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull));
-        g.rho = __uint_as_float((unsigned)(key >> 32));
-        g.chisq = __uint_as_float((unsigned)(s[w].aux & 0xFFFFFFFFull));
-        out[o] = g;
-      }
-      ++o;
+  for (int w0 = 0; w0 < n_windows; w0 += 32) {
+    const int w = w0 + lane;
+    Slot sl;
+    sl.key = 0ull; sl.aux = 0ull;
+    if (w < n_windows) sl = s[w];
+    const bool hit = sl.key != 0ull;
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, hit);
+    const long long pos = o + __popc(b & ((1u << lane) - 1u));
+    if (hit && pos < capacity) {
+      gwmf_trigger g;
+      g.template_id = t;
+      g.sample = (int32_t)(0xFFFFFFFFu - (unsigned)(sl.key & 0xFFFFFFFFull));
+      g.rho = __uint_as_float((unsigned)(sl.key >> 32));
+      g.chisq = __uint_as_float((unsigned)(sl.aux & 0xFFFFFFFFull));
+      out[pos] = g;
     }
+    o += __popc(b);
   }
 }
 
@@ -77,9 +88,9 @@ cudaError_t launch_compact(Ctx* c) {
   long long* offsets = ws_ptr<long long>(c, c->lay.offsets);
   int T = c->n_templates;
   long long cap = (long long)c->prm.max_templates * c->n_windows;
-  k_count<<<(T + 127) / 128, 128, 0, c->stream>>>(slots, counts, T, c->n_windows);
+  k_count<<<(T + 7) / 8, 256, 0, c->stream>>>(slots, counts, T, c->n_windows);
   k_scan<<<1, 1024, 0, c->stream>>>(counts, offsets, T);
-  k_emit<<<(T + 127) / 128, 128, 0, c->stream>>>(slots, offsets, ws_ptr<gwmf_trigger>(c, c->lay.trig_out), cap, T,
+  k_emit<<<(T + 7) / 8, 256, 0, c->stream>>>(slots, offsets, ws_ptr<gwmf_trigger>(c, c->lay.trig_out), cap, T,
                                                  c->n_windows);
   c->launches += 3;
   return cudaGetLastError();
