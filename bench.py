@@ -330,9 +330,9 @@ def run_gpu(args):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum PER TEMPLATE from the committed `ncu --set full` capture
-# (profiles/r1_v11_*.md, 8 templates per launch): index 0 = k_pass1_narrow ((0.0041 + 1.0147) GB / 8),
-# 1 = k_pass2 ((1.0738 + 0.0038) GB / 8); scaled by the templates per launch of the run.
-TRAFFIC_BYTES_PER_TEMPLATE = {0: 1.0188e9 / 8, 1: 1.0777e9 / 8}
+# (profiles/r1_v13_final.md, 16 templates per launch): index 0 = k_pass1_narrow ((0.0070 + 2.0882) GB / 16),
+# 1 = k_pass2 ((2.1475 + 0.0036) GB / 16); scaled by the templates per launch of the run.
+TRAFFIC_BYTES_PER_TEMPLATE = {0: 2.0952e9 / 16, 1: 2.1511e9 / 16}
 
 
 def main():
