@@ -201,6 +201,25 @@ def test_config4_long_segment_sampled(gw):
     _sampled_config(gw, 4, ids)
 
 
+def test_noise_statistics_at_full_size(gw):
+    # in stationary Gaussian noise rho^2 is chi^2 with 2 degrees of freedom and the veto
+    # statistic chi^2 with 2p - 2, whatever the template: properties that hold at any size, checked at the
+    # headline shape (N = 2^20, p = 16) in the launch configuration bench.py times (SURVEY pin P9)
+    w = inputs.workload(2)
+    s = inputs.segment(w, inject=False).astype(np.float32)
+    f = _run_gpu(gw, w, s, w.psd)
+    n_eff = w.n / 8.0                                    # neighbouring samples are correlated
+    for t in (0, 517, 1023):
+        rho, chi = f.series(t)
+        r2 = rho.astype(np.float64) ** 2
+        assert abs(r2.mean() - 2.0) < 3 * 2.0 / math.sqrt(n_eff), (t, r2.mean())
+        nu = 2 * w.p - 2
+        assert abs(chi.mean() - nu) < 3 * math.sqrt(2 * nu / n_eff) + 0.02 * nu, (t, chi.mean())
+        assert abs(chi.astype(np.float64).var() - 2 * nu) < 0.15 * 2 * nu, (t, chi.var())
+    # exceedances of the threshold: P(rho > 6) = e^-18 per sample -> ~16 samples over the whole bank
+    assert len(f.triggers()) < 200
+
+
 def test_long_segment_p16_sampled(gw):
     # SURVEY 8(f)-3 / PAPER.md:119,194: N = 4 x 2^20 segments with the headline p = 16 (the paper's "another
     # factor of 2" shape): config 4's segment and bank, 16 bands
