@@ -336,6 +336,24 @@ def test_determinism_and_refilter(gw):
     assert f.triggers().tobytes() == a.tobytes()
 
 
+def test_batching_invariance(gw):
+    # the result must not depend on how the bank is cut into launches (double-buffered Q, side stream,
+    # ragged last batch, partial filter calls)
+    n = 1 << 17
+    w1 = inputs.workload(1, 37)
+    masses = w1.masses
+    s = inputs.time_series(inputs.noise_spectrum(n, 5) + inputs.injection_spectrum(n, *masses[11], 10.0, 4242), n).astype(np.float32)
+    Sn = inputs.psd_array(n)
+    w = inputs.Workload(config=-1, n=n, p=16, rho_thresh=5.0, window=4096, masses=masses, seed=0)
+    ref = _run_gpu(gw, w, s, Sn, batch=37).triggers().tobytes()
+    for batch in (1, 5, 8, 36):
+        f = _run_gpu(gw, w, s, Sn, batch=batch)
+        assert f.triggers().tobytes() == ref, f"batch {batch}"
+    f.filter(3, 20)                 # partial re-filter in ragged batches keeps the other templates' events
+    f.filter(30, 7)
+    assert f.triggers().tobytes() == ref
+
+
 def test_error_codes(gw):
     assert gw.workspace_bytes(1000, 4, 8, 1) == 0             # n not a power of two
     assert gw.workspace_bytes(1 << 14, 0, 4096, 1) == 0       # p < 1
