@@ -64,8 +64,9 @@ typedef struct {
   double  rho_thresh;    /* SNR threshold, strict '>'                                             */
   int32_t window;        /* W: trigger window in samples, power of two, divides n                 */
   int32_t max_templates; /* capacity of the bank                                                  */
-  int32_t batch;         /* templates filtered per kernel launch, 0 .. 64 (0 = library default); sizes
-                            the band-intermediate buffer: batch * p * n * 8 bytes                  */
+  int32_t batch;         /* templates filtered per kernel launch, 0 .. 64 (0 = library default: about
+                            2 GiB of band intermediate); sizes the band-intermediate buffer,
+                            batch * p * n * 8 bytes, and the correlated spectra, 2 * batch * n * 4 bytes */
 } gwmf_params;
 
 /* Bytes of DEVICE memory the caller must provide to gwmf_create (0 if params are invalid). */
@@ -97,7 +98,9 @@ int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_t
  * to later work on that stream).  async for device sources. */
 int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn);
 
-/* Matched-filter templates [first_template, first_template + n_templates) against the loaded segment:
+/* Matched-filter templates [first_template, first_template + n_templates) against the loaded segment
+ * (the host may wait here for the segment preparation to finish: the call reads back which bands of which
+ * templates need the wide-band kernels):
  * p band inverse FFTs, rho and chi^2 at every sample (Eq. 3, 5) and the per-window
  * maxima above threshold.  Trigger slots of those templates are reset first.  async. */
 int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
