@@ -3,6 +3,7 @@
 // beyond a handful of scalars per template.
 #include <math.h>
 #include <new>
+#include <stdlib.h>
 #include <string.h>
 #include <vector>
 
@@ -155,6 +156,10 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->stream = (cudaStream_t)cuda_stream;
   c->n_templates = 0;
   c->have_bank = c->have_segment = false;
+  {
+    const char* f = getenv("GWMF_FUSED");
+    c->fused = f && f[0] == '1';
+  }
   c->launches = 0;
   c->h_meta = nullptr;
   c->h_masks = nullptr;
@@ -254,7 +259,8 @@ int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates) {
     const int rest = n_templates - done - cnt;
     const int next = rest < c->lay.batch ? rest : c->lay.batch;
     CU(launch_pass1_filter(c, first_template + done, cnt, first_template + done + cnt, next, parity, done > 0));
-    CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
+    if (c->fused) CU(launch_fused_filter(c, first_template + done, cnt, parity, true, nullptr, nullptr));
+    else CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
   }
   return GWMF_OK;
 }
@@ -277,7 +283,8 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
     CU(cudaEventRecord(ev[3 * b], c->stream));
     CU(launch_pass1_filter(c, first_template + done, cnt, first_template + done + cnt, next, b & 1, b > 0));
     CU(cudaEventRecord(ev[3 * b + 1], c->stream));
-    CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
+    if (c->fused) CU(launch_fused_filter(c, first_template + done, cnt, b & 1, true, nullptr, nullptr));
+    else CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
     CU(cudaEventRecord(ev[3 * b + 2], c->stream));
   }
   CU(cudaStreamSynchronize(c->stream));
@@ -369,7 +376,8 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
   float* d_rho = ws_ptr<float>(c, c->lay.series_rho);
   float* d_chi = ws_ptr<float>(c, c->lay.series_chi);
   CU(launch_pass1_filter(c, template_id, 1, 0, 0, 0, false));
-  CU(launch_pass2_filter(c, template_id, 1, false, d_rho, d_chi));
+  if (c->fused) CU(launch_fused_filter(c, template_id, 1, 0, false, d_rho, d_chi));
+  else CU(launch_pass2_filter(c, template_id, 1, false, d_rho, d_chi));
   if (host_rho)
     CU(cudaMemcpyAsync(host_rho, d_rho, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
   if (host_chisq)

@@ -57,6 +57,7 @@ struct Ctx {
   cudaEvent_t ev_fork, ev_join;
   int n_templates;
   bool have_bank, have_segment;
+  bool fused;                    // EXPERIMENTAL (env GWMF_FUSED=1): spill-free kernel instead of narrow pass 1 + pass 2
   int64_t launches;
   std::string cuda_err;
   TemplateMeta* h_meta;          // host staging of the bank (pinned)
@@ -73,6 +74,8 @@ cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStrea
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
 cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid);
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,
+                                float* series_chi);
+cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool update_slots, float* series_rho,
                                 float* series_chi);
 cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out);
 inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, float2* d_out) {

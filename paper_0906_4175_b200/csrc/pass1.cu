@@ -415,7 +415,7 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
     any_wide |= c->h_masks[t] != 0u;
     any_narrow |= c->h_masks[t] != full;
   }
-  if (any_narrow) {
+  if (any_narrow && !c->fused) {
     // narrow bands write the A layout directly
     e = launch_narrow(c, args, count);
     if (e != cudaSuccess) return e;

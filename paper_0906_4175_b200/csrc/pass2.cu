@@ -69,6 +69,14 @@ __device__ __noinline__ void emit_candidate(Slot* slots_t, unsigned j, float rho
              (unsigned long long)__float_as_uint(chi));
 }
 
+__device__ __forceinline__ float2 cis_frac_p2(unsigned num, int log_n) {
+  // e^{2 pi i num / 2^log_n}; num is reduced mod 2^log_n first so that 2 num / n is exact in fp32
+  num &= (1u << log_n) - 1u;
+  float s, c;
+  sincospif(2.0f * (float)num / (float)(1u << log_n), &s, &c);
+  return make_float2(c, s);
+}
+
 // ---- TMA (bulk async copy) + mbarrier helpers --------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
@@ -212,6 +220,191 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
       }
     }
   }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// EXPERIMENTAL spill-free path: narrow bands never reach HBM.  A CTA owns 8 consecutive rows j1 of one
+// template (one per warp) and walks the p bands.  For a narrow band (<= 32 input rows) the row of Y is
+// formed directly from the correlated spectrum, Y_l[j1][k2] = e^{2 pi i j1 k2/n} sum_i Q[1024 k1_i + k2]
+// e^{2 pi i j1 k1_i/n1} (R complex MACs per sample with row-constant twiddles; the band's rows are staged in
+// shared memory once per CTA), then both 32-point stages of the row transform run in the warp.  Wide bands
+// come from the band buffer (generic pass-1 kernel + row stage) through a TMA load, as in k_pass2.
+// ---------------------------------------------------------------------------------------------------
+struct FArgs {
+  P2Args b;
+  const float2* q;            // [batch][n/2] correlated spectra of the batch
+  const float2* tw_n1;        // e^{2 pi i m/n1}
+  int log_n;
+  int n_groups;               // batch * n1 / 8
+};
+
+constexpr int kFRows = 8;                       // input rows staged per chunk
+constexpr int kFTile = 32 * 33;                 // per-warp tile (float2): padded transpose tile / TMA landing buffer
+
+template <bool SERIES>
+__global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
+  const P2Args& a = fa.b;
+  extern __shared__ __align__(128) float2 smem2[];
+  float2* tw_s = smem2;                                   // [c][jm] e^{2 pi i c jm/1024}
+  float2* Qs = smem2 + 1024;                              // [kFRows][1024]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  float2* buf = Qs + kFRows * 1024 + warp * kFTile;
+  float2* beta = Qs + kFRows * 1024 + 8 * kFTile + warp * 32;
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(Qs + kFRows * 1024 + 8 * kFTile + 8 * 32) + warp;
+  for (int i = tid; i < 1024; i += 256) tw_s[i] = a.tw_p2[i];
+  if (lane == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  unsigned long long policy;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+
+  const int p = a.p;
+  const int n1 = a.n1, n1m = n1 - 1;
+  const int groups_per_t = n1 >> 3;
+  const size_t half = (size_t)1 << (fa.log_n - 1);
+  unsigned tma_phase = 0;
+
+#pragma unroll 1
+  for (int g = blockIdx.x; g < fa.n_groups; g += gridDim.x) {
+    const int tb = g / groups_per_t, j1 = ((g - tb * groups_per_t) << 3) + warp;
+    const TemplateMeta* mt = a.meta + tb;
+    const unsigned wide_mask = mt->wide_mask;
+    const float2* qrow = fa.q + (size_t)tb * half;
+    // row twiddles: e^{2 pi i j1 k2/n} = alpha_lane * beta^m with k2 = 32 m + lane
+    beta[lane] = cis_frac_p2(((unsigned)j1 * 32u * (unsigned)lane), fa.log_n);
+    const float2 alpha = cis_frac_p2((unsigned)j1 * (unsigned)lane, fa.log_n);
+    __syncwarp();
+
+    float2 az[32];
+    float aq[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) { az[i] = make_float2(0.f, 0.f); aq[i] = 0.f; }
+
+#pragma unroll 1
+    for (int l = 0; l < p; ++l) {
+      const int e_lo = mt->edges[l], e_hi = mt->edges[l + 1];
+      float2 x[32];
+      if ((wide_mask >> l) & 1u) {
+        // wide band: the A row was written by the generic pass-1 kernel + row stage
+        const float2* src = a.y + ((size_t)(tb * p + l) * n1 + j1) * kN2;
+        if (lane == 0) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          mbar_expect_tx(bar, kN2 * (unsigned)sizeof(float2));
+          bulk_load_row(buf, src, kN2 * (unsigned)sizeof(float2), bar, policy);
+        }
+        mbar_wait(bar, tma_phase & 1u);
+        ++tma_phase;
+#pragma unroll
+        for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(buf[32 * c + lane], tw_s[32 * c + lane]);
+        __syncwarp();
+      } else {
+        if (e_hi <= e_lo) continue;                    // empty band: z_l = 0
+        const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
+        const int R = row_hi - row_lo + 1;
+        float2 acc[32];
+#pragma unroll
+        for (int m = 0; m < 32; ++m) acc[m] = make_float2(0.f, 0.f);
+#pragma unroll 1
+        for (int r0 = 0; r0 < R; r0 += kFRows) {
+          const int rc = R - r0 < kFRows ? R - r0 : kFRows;
+          __syncthreads();                             // the previous chunk has been consumed by every warp
+          for (int idx = tid; idx < rc * 1024; idx += 256) {
+            const int k = ((row_lo + r0 + (idx >> 10)) << kLogN2) + (idx & 1023);
+            Qs[idx] = (k >= e_lo && k < e_hi) ? qrow[k] : make_float2(0.f, 0.f);
+          }
+          __syncthreads();
+#pragma unroll 1
+          for (int i = 0; i < rc; ++i) {
+            const tw4 r = make_tw4(cmul(fa.tw_n1[(j1 * (row_lo + r0 + i)) & n1m], alpha));   // e^{2 pi i j1 (k1/n1 + lane/n)}
+            const float2* qs = Qs + i * 1024 + lane;
+#pragma unroll
+            for (int m = 0; m < 32; ++m) {
+              const float2 qv = qs[32 * m];
+              acc[m] = unpk(fma2(pk(-qv.y, qv.x), r.yy, fma2(pk(qv), r.xx, pk(acc[m]))));
+            }
+          }
+        }
+        // first row stage (over m), lane = c
+#pragma unroll
+        for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cmul(acc[m], beta[m]);
+        fft_dit<32>(x);
+#pragma unroll
+        for (int jm = 0; jm < 32; ++jm) buf[lane * 33 + jm] = x[jm];
+        __syncwarp();
+#pragma unroll
+        for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(buf[c * 33 + lane], tw_s[32 * c + lane]);   // lane = jm
+        __syncwarp();
+      }
+      fft_dit<32>(x);                                   // over c -> jc
+#pragma unroll
+      for (int jc = 0; jc < 32; ++jc) {
+        const float2 z = x[jc];
+        az[jc] = cadd(az[jc], z);
+        aq[jc] = fmaf(z.x, z.x, fmaf(z.y, z.y, aq[jc]));
+      }
+    }
+    // ---- epilogue of one row: rho, chi^2 and the trigger slots (steps a4, a5) ----
+    {
+      const float scale = mt->scale_rho2;
+      const float fp_scale = (float)p * scale, inv_p = 1.0f / (float)p;
+      const float thr2 = a.thresh * a.thresh * 0.999f;
+      Slot* slots_t = a.slots ? a.slots + (size_t)tb * a.n_windows : nullptr;
+#pragma unroll
+      for (int jc = 0; jc < 32; ++jc) {
+        const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
+        const float rho2 = z2 * scale;                                        // Eq. 3 squared
+        const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * fp_scale;         // Eq. 5
+        const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
+        if constexpr (SERIES) {
+          if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
+          if (a.series_chi) a.series_chi[j] = chi;
+        }
+        if (rho2 > thr2 && slots_t) emit_candidate(slots_t, j, rho2, chi, a.thresh, a.log_w);
+      }
+    }
+    __syncwarp();
+  }
+}
+
+constexpr size_t kFusedSmem = (size_t)(1024 + kFRows * 1024 + 8 * kFTile + 8 * 32) * sizeof(float2) + 8 * sizeof(unsigned long long);
+
+cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool update_slots, float* series_rho, float* series_chi) {
+  static bool done = false;
+  if (!done) {
+    cudaError_t e = cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
+    if (e != cudaSuccess) return e;
+    done = true;
+  }
+  FArgs fa;
+  P2Args& a = fa.b;
+  a.y = ws_ptr<float2>(c, c->lay.y);
+  a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
+  a.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
+  a.slots = update_slots ? ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows : nullptr;
+  a.series_rho = series_rho;
+  a.series_chi = series_chi;
+  a.dense_out = nullptr;
+  a.p = c->prm.p;
+  a.n1 = c->n1;
+  a.log_n1 = c->log_n - kLogN2;
+  int lw = 0;
+  while ((1 << lw) < c->prm.window) ++lw;
+  a.log_w = lw;
+  a.n_windows = c->n_windows;
+  a.n_rows = count * c->n1;
+  a.thresh = (float)c->prm.rho_thresh;
+  fa.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
+  fa.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
+  fa.log_n = c->log_n;
+  fa.n_groups = count * (c->n1 / 8);
+  const int grid = fa.n_groups < c->n_sms ? fa.n_groups : c->n_sms;
+  if (series_rho || series_chi) k_fused<true><<<grid, 256, kFusedSmem, c->stream>>>(fa);
+  else k_fused<false><<<grid, 256, kFusedSmem, c->stream>>>(fa);
+  c->launches++;
+  return cudaGetLastError();
 }
 
 constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
