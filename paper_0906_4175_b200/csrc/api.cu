@@ -71,6 +71,7 @@ Layout make_layout(const gwmf_params* p) {
   L.series_chi = take(n * sizeof(float));
   L.flags = take(256);
   L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
+  L.qb = take(2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2));   // band-separated copy (k_fused)
   size_t yb = (size_t)L.batch * (size_t)p->p * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;

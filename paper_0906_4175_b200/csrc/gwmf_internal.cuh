@@ -23,6 +23,7 @@ struct TemplateMeta {
   int32_t k_high;                // first bin above the template
   int32_t edges[kMaxBands + 1];  // band l = bins [edges[l], edges[l+1])
   uint32_t wide_mask;            // bit l: band l goes through the generic pass-1 kernel (> 32 input rows)
+  uint16_t row_off[kMaxBands + 2];  // band-separated spectrum Qb: rows of narrow band l start at row_off[l] (k_fused)
 };
 
 // One (template, window) trigger slot, updated with a 128-bit compare-and-swap.
@@ -35,7 +36,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, y, total;
+         series_rho, series_chi, flags, q, qb, y, total;
   size_t y_bytes;
   int batch;
 };
@@ -71,6 +72,8 @@ cudaError_t launch_segment_prepare(Ctx* c);                       // after s/Sn 
 cudaError_t launch_bank_setup(Ctx* c);
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready);
 cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st);
+cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cudaStream_t st);
+inline int qb_rows_cap(const Ctx* c) { return c->n1 / 2 + kMaxBands + 2; }   // rows of Qb per template
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
 cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid);
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,

@@ -369,6 +369,46 @@ static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, 
   return cudaGetLastError();
 }
 
+// The same values, band by band: row r of template I holds the 1024 bins of input row k1 of the narrow band l
+// that owns compact row r (row_off[l] <= r < row_off[l+1]), with the bins outside the band set to 0, so that a
+// band's rows are contiguous and need no masking by the consumer (k_fused stages them with one bulk copy).
+__global__ void __launch_bounds__(256) k_correlate_bands(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wq,
+                                                         const double* __restrict__ u_tab, float2* __restrict__ qb, int p,
+                                                         int rows_cap) {
+  const TemplateMeta* m = meta + blockIdx.y;
+  const int r = blockIdx.x;
+  if (r >= m->row_off[p]) return;
+  int l = 0;
+  while (m->row_off[l + 1] <= r) ++l;
+  const int e_lo = m->edges[l], e_hi = m->edges[l + 1];
+  const int k1 = (e_lo >> kLogN2) + (r - m->row_off[l]);
+  float2* out = qb + ((size_t)blockIdx.y * rows_cap + r) * kN2;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int k2 = threadIdx.x + 256 * j;
+    const int k = (k1 << kLogN2) + k2;
+    float2 v = make_float2(0.f, 0.f);
+    if (k >= e_lo && k < e_hi) {
+      const double u = u_tab[k];
+      double t = fma(fma(fma(fma(m->c0, u * u, m->c2), u, m->c3), u, m->c4), u, -0.125);   // Psi0 / 2 pi, turns
+      t -= rint(t);
+      float sn, cs;
+      sincospif(2.0f * (float)t, &sn, &cs);
+      v = cmul(wq[k], make_float2(cs, sn));
+    }
+    out[k2] = v;
+  }
+}
+
+cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+  const int cap = qb_rows_cap(c);
+  k_correlate_bands<<<dim3(c->n1 / 2 + c->prm.p + 1, count), 256, 0, st>>>(
+      ws_ptr<TemplateMeta>(c, c->lay.meta) + first, ws_ptr<float2>(c, c->lay.wq), ws_ptr<double>(c, c->lay.u_tab),
+      ws_ptr<float2>(c, c->lay.qb) + (size_t)parity * c->lay.batch * cap * kN2, c->prm.p, cap);
+  c->launches++;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   const int half = (int)(c->n / 2);
   k_correlate<<<dim3(half / 256, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, ws_ptr<float2>(c, c->lay.wq),
@@ -400,7 +440,10 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   cudaError_t e;
   if (!q_ready) {
     e = launch_correlate(c, first, count, parity, c->stream);
+    if (e == cudaSuccess && c->fused) e = launch_correlate_bands(c, first, count, parity, c->stream);
     if (e != cudaSuccess) return e;
+    // (the side stream's correlates of an earlier call are complete: gwmf_triggers / any sync came in between,
+    // or they were ordered before this call's work through the previous join)
   }
   // fork: everything enqueued so far on the main stream (this batch's Q, the previous batch's pass 2, which
   // read the band buffer) precedes the side work
@@ -426,6 +469,18 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
     if (e != cudaSuccess) return e;
     e = launch_rowstage(c, args.y, args.meta, count, count * c->prm.p, 1, c->side);
     if (e != cudaSuccess) return e;
+  }
+  if (c->fused) {
+    // the spill-free kernel only waits for the wide bands; the next batch's correlates then run beside it
+    if ((e = cudaEventRecord(c->ev_join, c->side)) != cudaSuccess) return e;
+    if (next_count > 0) {
+      bool next_wide = false;
+      for (int t = next_first; t < next_first + next_count; ++t) next_wide |= c->h_masks[t] != 0u;
+      e = launch_correlate_bands(c, next_first, next_count, parity ^ 1, c->side);
+      if (e == cudaSuccess && next_wide) e = launch_correlate(c, next_first, next_count, parity ^ 1, c->side);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaStreamWaitEvent(c->stream, c->ev_join, 0);
   }
   if (next_count > 0) {
     e = launch_correlate(c, next_first, next_count, parity ^ 1, c->side);

@@ -232,13 +232,14 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 // ---------------------------------------------------------------------------------------------------
 struct FArgs {
   P2Args b;
-  const float2* q;            // [batch][n/2] correlated spectra of the batch
+  const float2* qb;           // [batch][rows_cap][1024] band-separated correlated spectra (k_correlate_bands)
   const float2* tw_n1;        // e^{2 pi i m/n1}
   int log_n;
   int n_groups;               // batch * n1 / 8
+  int rows_cap;
 };
 
-constexpr int kFRows = 8;                       // input rows staged per chunk
+constexpr int kFRows = 8;                       // input rows staged per chunk (64 KB)
 constexpr int kFTile = 32 * 33;                 // per-warp tile (float2): padded transpose tile / TMA landing buffer
 
 template <bool SERIES>
@@ -246,16 +247,18 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
   const P2Args& a = fa.b;
   extern __shared__ __align__(128) float2 smem2[];
   float2* tw_s = smem2;                                   // [c][jm] e^{2 pi i c jm/1024}
-  float2* Qs = smem2 + 1024;                              // [kFRows][1024]
+  float2* Qs = smem2 + 1024;                              // [2][kFRows][1024]: double-buffered chunk of band rows
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  float2* buf = Qs + kFRows * 1024 + warp * kFTile;
-  float2* beta = Qs + kFRows * 1024 + 8 * kFTile + warp * 32;
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(Qs + kFRows * 1024 + 8 * kFTile + 8 * 32) + warp;
+  float2* buf = Qs + 2 * kFRows * 1024 + warp * kFTile;
+  float2* beta = Qs + 2 * kFRows * 1024 + 8 * kFTile + warp * 32;
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Qs + 2 * kFRows * 1024 + 8 * kFTile + 8 * 32);
+  unsigned long long* bar = bars + warp;                  // this warp's TMA barrier (wide bands)
+  unsigned long long* full = bars + 8;                    // full[2]: chunk landed in Qs[b]
+  int* s_meta = reinterpret_cast<int*>(bars + 10);        // [0..33): edges, [40..74): row_off
   for (int i = tid; i < 1024; i += 256) tw_s[i] = a.tw_p2[i];
-  if (lane == 0) {
-    mbar_init(bar, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
+  if (lane == 0) mbar_init(bar, 1);
+  if (tid == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); }
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
   unsigned long long policy;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
@@ -263,19 +266,44 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
   const int p = a.p;
   const int n1 = a.n1, n1m = n1 - 1;
   const int groups_per_t = n1 >> 3;
-  const size_t half = (size_t)1 << (fa.log_n - 1);
-  unsigned tma_phase = 0;
+  unsigned tma_phase = 0;           // uses of this warp's barrier
+  unsigned use0 = 0, use1 = 0;      // uses of full[0], full[1] (uniform over the CTA)
+  int cidx = 0;                     // chunks consumed so far (buffer = cidx & 1)
 
 #pragma unroll 1
   for (int g = blockIdx.x; g < fa.n_groups; g += gridDim.x) {
     const int tb = g / groups_per_t, j1 = ((g - tb * groups_per_t) << 3) + warp;
     const TemplateMeta* mt = a.meta + tb;
+    __syncthreads();                                       // s_meta and both chunk buffers are free
+    if (tid <= p) { s_meta[tid] = mt->edges[tid]; s_meta[40 + tid] = mt->row_off[tid]; }
     const unsigned wide_mask = mt->wide_mask;
-    const float2* qrow = fa.q + (size_t)tb * half;
+    const float2* qb_t = fa.qb + (size_t)tb * fa.rows_cap * kN2;
     // row twiddles: e^{2 pi i j1 k2/n} = alpha_lane * beta^m with k2 = 32 m + lane
     beta[lane] = cis_frac_p2(((unsigned)j1 * 32u * (unsigned)lane), fa.log_n);
     const float2 alpha = cis_frac_p2((unsigned)j1 * (unsigned)lane, fa.log_n);
-    __syncwarp();
+    __syncthreads();
+    // chunk (l, r0) of the narrow bands: rows row_off[l] + r0 .. of Qb; issue() starts its bulk copy into Qs[b]
+    auto issue = [&](int l, int r0, int b) {
+      const int R = s_meta[40 + l + 1] - s_meta[40 + l];
+      const int rc = R - r0 < kFRows ? R - r0 : kFRows;
+      const unsigned bytes = (unsigned)rc * kN2 * (unsigned)sizeof(float2);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(&full[b], bytes);
+      bulk_load_row(Qs + b * kFRows * 1024, qb_t + (size_t)(s_meta[40 + l] + r0) * kN2, bytes, &full[b], policy);
+    };
+    auto next_chunk = [&](int& l, int& r0) -> bool {       // advance to the following chunk of this group
+      const int R = s_meta[40 + l + 1] - s_meta[40 + l];
+      if (r0 + kFRows < R) { r0 += kFRows; return true; }
+      for (int l2 = l + 1; l2 < p; ++l2)
+        if (s_meta[40 + l2 + 1] > s_meta[40 + l2]) { l = l2; r0 = 0; return true; }
+      return false;
+    };
+    {   // first chunk of the group
+      int l0 = -1;
+      for (int l2 = 0; l2 < p; ++l2)
+        if (s_meta[40 + l2 + 1] > s_meta[40 + l2]) { l0 = l2; break; }
+      if (l0 >= 0 && tid == 0) issue(l0, 0, cidx & 1);
+    }
 
     float2 az[32];
     float aq[32];
@@ -284,7 +312,6 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
 
 #pragma unroll 1
     for (int l = 0; l < p; ++l) {
-      const int e_lo = mt->edges[l], e_hi = mt->edges[l + 1];
       float2 x[32];
       if ((wide_mask >> l) & 1u) {
         // wide band: the A row was written by the generic pass-1 kernel + row stage
@@ -300,25 +327,29 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
         for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(buf[32 * c + lane], tw_s[32 * c + lane]);
         __syncwarp();
       } else {
-        if (e_hi <= e_lo) continue;                    // empty band: z_l = 0
-        const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
-        const int R = row_hi - row_lo + 1;
+        const int R = s_meta[40 + l + 1] - s_meta[40 + l];
+        if (R == 0) continue;                          // empty band: z_l = 0
+        const int row_lo = s_meta[l] >> kLogN2;
         float2 acc[32];
 #pragma unroll
         for (int m = 0; m < 32; ++m) acc[m] = make_float2(0.f, 0.f);
 #pragma unroll 1
         for (int r0 = 0; r0 < R; r0 += kFRows) {
           const int rc = R - r0 < kFRows ? R - r0 : kFRows;
-          __syncthreads();                             // the previous chunk has been consumed by every warp
-          for (int idx = tid; idx < rc * 1024; idx += 256) {
-            const int k = ((row_lo + r0 + (idx >> 10)) << kLogN2) + (idx & 1023);
-            Qs[idx] = (k >= e_lo && k < e_hi) ? qrow[k] : make_float2(0.f, 0.f);
+          const int b = cidx & 1;
+          __syncthreads();                             // every warp is done with the chunk that used Qs[b ^ 1]
+          if (tid == 0) {
+            int ln = l, rn = r0;
+            if (next_chunk(ln, rn)) issue(ln, rn, b ^ 1);
           }
-          __syncthreads();
+          mbar_wait(&full[b], (b ? use1 : use0) & 1u);
+          if (b) ++use1; else ++use0;
+          ++cidx;
+          const float2* qbase = Qs + b * kFRows * 1024 + lane;
 #pragma unroll 1
           for (int i = 0; i < rc; ++i) {
             const tw4 r = make_tw4(cmul(fa.tw_n1[(j1 * (row_lo + r0 + i)) & n1m], alpha));   // e^{2 pi i j1 (k1/n1 + lane/n)}
-            const float2* qs = Qs + i * 1024 + lane;
+            const float2* qs = qbase + i * 1024;
 #pragma unroll
             for (int m = 0; m < 32; ++m) {
               const float2 qv = qs[32 * m];
@@ -364,11 +395,11 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
         if (rho2 > thr2 && slots_t) emit_candidate(slots_t, j, rho2, chi, a.thresh, a.log_w);
       }
     }
-    __syncwarp();
   }
 }
 
-constexpr size_t kFusedSmem = (size_t)(1024 + kFRows * 1024 + 8 * kFTile + 8 * 32) * sizeof(float2) + 8 * sizeof(unsigned long long);
+constexpr size_t kFusedSmem = (size_t)(1024 + 2 * kFRows * 1024 + 8 * kFTile + 8 * 32) * sizeof(float2) +
+                              10 * sizeof(unsigned long long) + 80 * sizeof(int);
 
 cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool update_slots, float* series_rho, float* series_chi) {
   static bool done = false;
@@ -396,7 +427,8 @@ cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool u
   a.n_windows = c->n_windows;
   a.n_rows = count * c->n1;
   a.thresh = (float)c->prm.rho_thresh;
-  fa.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
+  fa.rows_cap = qb_rows_cap(c);
+  fa.qb = ws_ptr<float2>(c, c->lay.qb) + (size_t)parity * c->lay.batch * fa.rows_cap * kN2;
   fa.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
   fa.log_n = c->log_n;
   fa.n_groups = count * (c->n1 / 8);

@@ -195,12 +195,22 @@ __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ m
   if (!live) return;
   // bands for the generic pass-1 kernel: more than 32 input rows (or every band when n1 < 32)
   bool wide = false;
+  int rows = 0;
   if (l < p) {
     const int e_lo = s_edges[ty][l], e_hi = s_edges[ty][l + 1];
-    const int rows = e_hi > e_lo ? ((e_hi - 1) >> kLogN2) - (e_lo >> kLogN2) + 1 : 0;
+    rows = e_hi > e_lo ? ((e_hi - 1) >> kLogN2) - (e_lo >> kLogN2) + 1 : 0;
     wide = all_wide || rows > 32;
   }
   const unsigned mask = __ballot_sync(0xFFFFFFFFu, wide);
+  // rows of the narrow bands in the band-separated spectrum: exclusive prefix sum over the bands
+  int incl = wide ? 0 : rows;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (l >= d) incl += v;
+  }
+  meta[t].row_off[l + 1] = (uint16_t)incl;
+  if (l == 0) { meta[t].row_off[0] = 0; meta[t].row_off[kMaxBands + 1] = 0; }
   meta[t].edges[l] = s_edges[ty][l];
   if (l == 0) {
     meta[t].edges[kMaxBands] = k_high;

@@ -48,8 +48,8 @@ def test_workspace_bytes_host_only(lib):
     b = gwmf.workspace_bytes(1 << 20, 16, 4096, 1024)
     # band intermediate: batch(16) * p * n * 8 B = 2 GiB, plus the double-buffered correlated spectra
     # (2 * batch * 4 MiB), tables / slots / staging
-    assert (2 << 30) + (128 << 20) < b < (2 << 30) + (192 << 20)
-    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (320 << 20)
+    assert (2 << 30) + (128 << 20) < b < (2 << 30) + (384 << 20)
+    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (340 << 20)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
 
