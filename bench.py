@@ -62,6 +62,17 @@ def load_workload(name):
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback, only if MEASURED_PEAKS.json is absent
 
 
+def alu_peak():
+    """FP32 non-tensor peak in TFLOP/s: 148 SMs x 128 lanes x 2 flop x max SM clock."""
+    mhz, src = 1965.0, "B200 nominal max SM clock"
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            mhz, src = float(json.load(fh)["sm_max_mhz"]), "MEASURED_PEAKS.json sm_max_mhz"
+    except Exception:
+        pass
+    return 148 * 128 * 2 * mhz * 1e6 / 1e12, "148 SMs x 128 FP32 lanes x 2 flop x %.0f MHz (%s)" % (mhz, src)
+
+
 def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -222,7 +233,10 @@ def run_gpu(args):
     Sn = w.psd
     T = len(w.masses)
 
+    if args.path != "auto":
+        os.environ["GWMF_FUSED"] = "1" if args.path == "fused" else "0"
     f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}")
+    fused = f.uses_fused
     f.make_bank(w.masses)
     s_dev = torch.from_numpy(s32).to(dev)
     sn_dev = torch.from_numpy(Sn).to(dev)
@@ -265,6 +279,10 @@ def run_gpu(args):
     names = ["pass 1: k_pass1_narrow (pruned column FFT + first row stage, writes p*N*8 B/template) with the "
              "low-volume kernels (k_correlate, k_pass1 generic, k_rowstage) beside it on the side stream; timed fork to join",
              "pass 2: k_pass2 (last FFT stage + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"]
+    if fused:
+        names = ["wide bands only: k_pass1 generic + k_rowstage (side stream; the next batch's correlates run beside k_fused)",
+                 "k_fused (spill-free: narrow bands formed from the correlated spectrum, both row-transform stages, "
+                 "rho/chi^2/trigger epilogue; no band intermediate in HBM)"]
 
     # end to end through the C ABI with host buffers
     s_pin = torch.from_numpy(s32).pin_memory()
@@ -301,6 +319,11 @@ def run_gpu(args):
         line["gpu_launches"] = int(launches)
         line["clocks"] = clocks
         line["triggers_per_step"] = int(len(trig))
+        line["config"]["path"] = "spill-free (k_fused)" if fused else "two-pass (k_pass1_narrow + k_pass2)"
+        if fused:
+            line["config"]["l2"] = ("no flush: no band intermediate; per launch the kernel reads the batch's correlated "
+                                    "spectra (%.0f MiB, produced by the previous launch's side stream) out of L2"
+                                    % (batch_templates[1] * w.n * 4 / 2**20))
         line["roofline"] = {
             "bound": "hbm", "kernel": names[dom], "achieved": float(gbs[dom]), "peak": peak, "unit": "GB/s",
             "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": (TRAFFIC_BYTES_PER_TEMPLATE[dom] * float(batch_templates[dom])
@@ -315,6 +338,24 @@ def run_gpu(args):
                      "note": "whole step (both passes + epilogue) against the 16*p*N B/template two-pass model; "
                              "frac vs nominal 8 TB/s = %.3f" % (16.0 * w.p * w.n * value / world / 8e12)},
         }
+        if fused:
+            # the spill-free kernel moves (almost) no HBM bytes: it is bound by the FP32 pipes and shared memory
+            flops_unit = 5.0 * w.n * np.log2(w.n) * w.p            # p * 5 N log2 N per template-segment
+            apeak, asrc = alu_peak()
+            tfl = flops_unit * batch_templates[1] / (avg_ms[1] * 1e-3) / 1e12
+            hbm_model = line["roofline"]["path"]
+            hbm_model["note"] = ("for comparison only: what the two-pass model would have to move; the spill-free kernel "
+                                 "does not move these bytes (see traffic)")
+            line["roofline"] = {
+                "bound": "alu", "kernel": names[1], "achieved": float(tfl), "peak": apeak, "unit": "TFLOP/s",
+                "frac": float(tfl / apeak), "peak_source": asrc,
+                "traffic": (FUSED_TRAFFIC_BYTES_PER_TEMPLATE * float(batch_templates[1]) if args.workload == "headline" else None),
+                "flops_per_launch": float(flops_unit * batch_templates[1]), "avg_launch_ms": float(avg_ms[1]),
+                "kernels": {"wide_bands": {"avg_launch_ms": float(avg_ms[0]), "share_of_step": float(k_ms[0] / k_ms.sum())},
+                            "k_fused": {"avg_launch_ms": float(avg_ms[1]), "TFLOP/s": float(tfl), "frac": float(tfl / apeak),
+                                        "share_of_step": float(k_ms[1] / k_ms.sum())}},
+                "hbm_model_equivalent": hbm_model,
+            }
         if not args.no_cpu_baseline and world == 1:
             cores = min(host_cores(), 32)
             nt = cores * (2 if cores <= 16 else 1)
@@ -334,6 +375,8 @@ def run_gpu(args):
 # (profiles/r1_v13_final.md, 16 templates per launch): index 0 = k_pass1_narrow ((0.0070 + 2.0882) GB / 16),
 # 1 = k_pass2 ((2.1475 + 0.0036) GB / 16); scaled by the templates per launch of the run.
 TRAFFIC_BYTES_PER_TEMPLATE = {0: 2.0952e9 / 16, 1: 2.1511e9 / 16}
+# k_fused: 5.4 MB read + 0 written per 16-template launch (profiles/r1_v14_fused.md)
+FUSED_TRAFFIC_BYTES_PER_TEMPLATE = 5.42e6 / 16
 
 
 def main():
@@ -344,6 +387,8 @@ def main():
     ap.add_argument("--impl", default="gwmf", choices=["gwmf", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="headline", choices=sorted(WORKLOADS))
+    ap.add_argument("--path", default="auto", choices=["auto", "two_pass", "fused"],
+                    help="auto = the library's choice (spill-free for n <= 2^20); the others force a path (GWMF_FUSED)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

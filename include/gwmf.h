@@ -142,6 +142,12 @@ int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q);
  * interleaved complex fp32 (re, im), n = params.n; in != out.  async. */
 int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out);
 
+/* 1 if this context filters with the spill-free kernel (k_fused: narrow bands are formed from the correlated
+ * spectrum inside the row-transform kernel and never reach HBM), 0 if with the two-pass path (band intermediate
+ * written by pass 1, read by pass 2).  Chosen at gwmf_create: spill-free for n <= 2^20, two-pass above; the
+ * environment variable GWMF_FUSED=0/1 overrides.  Both paths compute the same quantities. */
+int gwmf_uses_fused(const gwmf_ctx* ctx);
+
 /* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
 int64_t gwmf_launch_count(const gwmf_ctx* ctx);
 

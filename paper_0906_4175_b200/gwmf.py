@@ -21,7 +21,7 @@ EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
     "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_series", "gwmf_correlate",
     "gwmf_fft_inverse",
-    "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
+    "gwmf_uses_fused", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
 
 
@@ -70,6 +70,7 @@ def load_library():
     L.gwmf_series.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.gwmf_correlate.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     L.gwmf_fft_inverse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.gwmf_uses_fused.argtypes = [C.c_void_p]
     L.gwmf_launch_count.argtypes = [C.c_void_p]
     L.gwmf_launch_count.restype = C.c_int64
     L.gwmf_destroy.argtypes = [C.c_void_p]
@@ -146,6 +147,10 @@ class Filter:
         return int(self._L.gwmf_launch_count(self._h))
 
     # ------------------------------------------------------------------ the four calls of the boundary
+    @property
+    def uses_fused(self) -> bool:
+        return bool(self._L.gwmf_uses_fused(self._h))
+
     def make_bank(self, masses):
         arr = (MassPair * len(masses))(*[MassPair(float(a), float(b)) for a, b in masses])
         self._check(self._L.gwmf_make_bank(self._h, arr, len(masses)))

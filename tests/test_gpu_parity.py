@@ -22,6 +22,22 @@ def gw():
     return gwmf
 
 
+@pytest.fixture(params=["auto", "two_pass", "fused"])
+def path(request):
+    """Forces the library's path for one test: auto = its own choice (spill-free kernel for 2^15 <= n <= 2^20,
+    two-pass otherwise); the environment variable is read by gwmf_create."""
+    old = os.environ.get("GWMF_FUSED")
+    if request.param == "auto":
+        os.environ.pop("GWMF_FUSED", None)
+    else:
+        os.environ["GWMF_FUSED"] = "1" if request.param == "fused" else "0"
+    yield request.param
+    if old is None:
+        os.environ.pop("GWMF_FUSED", None)
+    else:
+        os.environ["GWMF_FUSED"] = old
+
+
 def _run_gpu(gw, w, s, Sn, masses=None, batch=0, window=None, thresh=None, p=None):
     masses = w.masses if masses is None else masses
     f = gw.Filter(w.n, p or w.p, window or w.window, len(masses), rho_thresh=w.rho_thresh if thresh is None else thresh,
@@ -93,7 +109,7 @@ def test_correlate_alone(gw, log_n, masses):
 
 
 # ----------------------------------------------------------------------------- config 0, everything
-def test_config0_full(gw):
+def test_config0_full(gw, path):
     w = inputs.workload(0)
     s = inputs.segment(w)
     Sn = w.psd
@@ -129,7 +145,7 @@ def test_config0_noise_free_closed_forms(gw):
 # ----------------------------------------------------------------------------- ragged mid-size cases
 @pytest.mark.parametrize("log_n,p,window,batch", [(15, 5, 2048, 3), (16, 7, 8192, 2), (17, 16, 4096, 0),
                                                   (19, 3, 1 << 19, 5)])
-def test_midsize_full_series(gw, log_n, p, window, batch):
+def test_midsize_full_series(gw, path, log_n, p, window, batch):
     n = 1 << log_n
     masses = [(1.0, 1.0), (1.4, 1.4), (3.0, 1.2), (5.0, 5.0), (10.0, 1.4), (12.0, 9.0), (20.0, 14.0)]
     D = inputs.noise_spectrum(n, 40 + log_n)
@@ -169,7 +185,7 @@ def _sampled_config(gw, config, sample_ids, n_templates=None):
     return w, trig, compared
 
 
-def test_config1_all_templates(gw):
+def test_config1_all_templates(gw, path):
     w = inputs.workload(1)
     s = inputs.segment(w).astype(np.float32)
     Sn = w.psd
@@ -184,7 +200,20 @@ def test_config1_all_templates(gw):
         parity.assert_series(rho_g, chi_g, rho_o, chi_o, w.p, f"config 1 template {t}")
 
 
-def test_config2_headline_sampled(gw):
+@pytest.mark.parametrize("forced", ["0", "1"])
+def test_config2_headline_sampled(gw, forced):
+    old = os.environ.get("GWMF_FUSED")
+    os.environ["GWMF_FUSED"] = forced
+    try:
+        _config2_headline_sampled(gw)
+    finally:
+        if old is None:
+            os.environ.pop("GWMF_FUSED", None)
+        else:
+            os.environ["GWMF_FUSED"] = old
+
+
+def _config2_headline_sampled(gw):
     w0 = inputs.workload(2)
     inj = sorted({b for (b, *_rest) in w0.injections})[:6]
     ids = sorted(set(inj + [0, 31, 500, 1023]))
@@ -275,7 +304,7 @@ def test_config3_stream_segments_sampled(gw):
 
 
 # ----------------------------------------------------------------------------- edge cases and the boundary
-def test_p_extremes_and_covariance(gw):
+def test_p_extremes_and_covariance(gw, path):
     n = 1 << 15
     masses = [(2.0, 1.5), (9.0, 7.0)]
     s = inputs.time_series(inputs.noise_spectrum(n, 9) + inputs.injection_spectrum(n, 2.0, 1.5, 10.0, 777), n).astype(np.float32)
@@ -300,7 +329,7 @@ def test_p_extremes_and_covariance(gw):
     assert f2.sigma()[0] == pytest.approx(f1.sigma()[0] / math.sqrt(c), rel=1e-12)
 
 
-def test_empty_bands_and_few_bins(gw):
+def test_empty_bands_and_few_bins(gw, path):
     # a template that spans only a few dozen bins: with p = 32 most bands hold one bin and several are
     # empty (coinciding edges) -- their z_l must be exactly 0 in both pass-1 paths
     for log_n in (14, 15):           # n1 = 16: generic kernel only; n1 = 32: narrow kernel's empty-band path
@@ -322,7 +351,7 @@ def test_empty_bands_and_few_bins(gw):
         parity.assert_triggers(f.triggers(), out, 4.0, 2048, 32)
 
 
-def test_determinism_and_refilter(gw):
+def test_determinism_and_refilter(gw, path):
     w = inputs.workload(0)
     s = inputs.segment(w)
     f = _run_gpu(gw, w, s, w.psd)
@@ -336,7 +365,7 @@ def test_determinism_and_refilter(gw):
     assert f.triggers().tobytes() == a.tobytes()
 
 
-def test_batching_invariance(gw):
+def test_batching_invariance(gw, path):
     # the result must not depend on how the bank is cut into launches (double-buffered Q, side stream,
     # ragged last batch, partial filter calls)
     n = 1 << 17
