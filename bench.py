@@ -9,9 +9,10 @@ Contract (driver): `python bench.py --gpus N --steps K --warmup W [--impl refere
   value     = template-segments/s with segment, PSD and bank resident in HBM when the timed region starts.
   e2e       = the same through the C ABI with HOST buffers: every step uploads the segment and the PSD
               (gwmf_load_segment from pinned host memory), filters the bank and reads the triggers back.
-  roofline  = the dominant kernel's algorithmic HBM bytes / its device time (CUDA events recorded by the
-              library on its own stream around every launch, gwmf_filter_timed), against the measured
-              copy bandwidth in MEASURED_PEAKS.json.
+  roofline  = the dominant kernel's algorithmic work / its device time (CUDA events recorded by the library
+              on its own stream around every launch, gwmf_filter_timed): for the two-pass path HBM bytes against
+              the measured copy bandwidth in MEASURED_PEAKS.json; for the spill-free kernel (the library's
+              choice at this size: no band intermediate in HBM) flops against the FP32 ALU peak.
   cpu_baseline = the fp64 oracle as it stands, on the host cores, on a bounded sample of the workload.
   N > 1     : one process per GPU; every rank filters the whole bank against its own segment (seed +
               rank): independent units, no data-path collective, weak scaling.
@@ -375,8 +376,8 @@ def run_gpu(args):
 # (profiles/r1_v13_final.md, 16 templates per launch): index 0 = k_pass1_narrow ((0.0070 + 2.0882) GB / 16),
 # 1 = k_pass2 ((2.1475 + 0.0036) GB / 16); scaled by the templates per launch of the run.
 TRAFFIC_BYTES_PER_TEMPLATE = {0: 2.0952e9 / 16, 1: 2.1511e9 / 16}
-# k_fused: 5.4 MB read + 0 written per 16-template launch (profiles/r1_v14_fused.md)
-FUSED_TRAFFIC_BYTES_PER_TEMPLATE = 5.42e6 / 16
+# k_fused: 5.5-7.2 MB read + 0 written per 16-template launch (profiles/r1_v14_fused.md)
+FUSED_TRAFFIC_BYTES_PER_TEMPLATE = 6.35e6 / 16
 
 
 def main():

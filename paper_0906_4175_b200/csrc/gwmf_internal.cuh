@@ -58,7 +58,7 @@ struct Ctx {
   cudaEvent_t ev_fork, ev_join;
   int n_templates;
   bool have_bank, have_segment;
-  bool fused;                    // EXPERIMENTAL (env GWMF_FUSED=1): spill-free kernel instead of narrow pass 1 + pass 2
+  bool fused;                    // spill-free kernel (k_fused) instead of narrow pass 1 + pass 2 (n <= 2^20; GWMF_FUSED)
   int64_t launches;
   std::string cuda_err;
   TemplateMeta* h_meta;          // host staging of the bank (pinned)

@@ -223,12 +223,16 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// EXPERIMENTAL spill-free path: narrow bands never reach HBM.  A CTA owns 8 consecutive rows j1 of one
-// template (one per warp) and walks the p bands.  For a narrow band (<= 32 input rows) the row of Y is
-// formed directly from the correlated spectrum, Y_l[j1][k2] = e^{2 pi i j1 k2/n} sum_i Q[1024 k1_i + k2]
-// e^{2 pi i j1 k1_i/n1} (R complex MACs per sample with row-constant twiddles; the band's rows are staged in
-// shared memory once per CTA), then both 32-point stages of the row transform run in the warp.  Wide bands
-// come from the band buffer (generic pass-1 kernel + row stage) through a TMA load, as in k_pass2.
+// Spill-free path (the library's choice for n <= 2^20; gwmf_uses_fused): narrow bands never reach HBM.  A CTA
+// owns 8 consecutive rows j1 of one template (one per warp) and walks the p bands.  For a narrow band (<= 32
+// input rows) the row of Y is formed directly from the correlated spectrum,
+//     Y_l[j1][k2] = e^{2 pi i j1 k2/n} sum_i Q[1024 k1_i + k2] e^{2 pi i j1 k1_i/n1}
+// (R complex MACs per sample with row-constant twiddles).  The band's rows come from the band-separated copy
+// of the correlated spectrum (k_correlate_bands: rows of a band contiguous, bins outside the band zeroed) by
+// one TMA bulk copy per chunk of <= 8 rows, double-buffered in shared memory, issued one chunk ahead; one CTA
+// barrier per chunk hands the buffer over.  Both 32-point stages of the row transform then run in the warp
+// (transpose through its padded tile), followed by the accumulation and epilogue of k_pass2.  Wide bands come
+// from the band buffer (generic pass-1 kernel + row stage) through a TMA load, as in k_pass2.
 // ---------------------------------------------------------------------------------------------------
 struct FArgs {
   P2Args b;
