@@ -333,7 +333,8 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
       } else {
         const int R = s_meta[40 + l + 1] - s_meta[40 + l];
         if (R == 0) continue;                          // empty band: z_l = 0
-        const int row_lo = s_meta[l] >> kLogN2;
+        const int e_lo = s_meta[l], e_hi = s_meta[l + 1];
+        const int row_lo = e_lo >> kLogN2, row_hi = (e_hi - 1) >> kLogN2;
         float2 acc[32];
 #pragma unroll
         for (int m = 0; m < 32; ++m) acc[m] = make_float2(0.f, 0.f);
@@ -352,12 +353,22 @@ __global__ void __launch_bounds__(256, 1) k_fused(FArgs fa) {
           const float2* qbase = Qs + b * kFRows * 1024 + lane;
 #pragma unroll 1
           for (int i = 0; i < rc; ++i) {
-            const tw4 r = make_tw4(cmul(fa.tw_n1[(j1 * (row_lo + r0 + i)) & n1m], alpha));   // e^{2 pi i j1 (k1/n1 + lane/n)}
+            const int k1 = row_lo + r0 + i;
+            const tw4 r = make_tw4(cmul(fa.tw_n1[(j1 * k1) & n1m], alpha));   // e^{2 pi i j1 (k1/n1 + lane/n)}
             const float2* qs = qbase + i * 1024;
+            // the band's first and last row are only partly inside it: skip the blocks of 8 m (256 bins) that
+            // hold nothing but zeros (warp-uniform branches)
+            const int m_lo = (k1 == row_lo) ? ((e_lo & 1023) >> 5) : 0;
+            const int m_hi = (k1 == row_hi) ? (((e_hi - 1) & 1023) >> 5) + 1 : 32;
 #pragma unroll
-            for (int m = 0; m < 32; ++m) {
-              const float2 qv = qs[32 * m];
-              acc[m] = unpk(fma2(pk(-qv.y, qv.x), r.yy, fma2(pk(qv), r.xx, pk(acc[m]))));
+            for (int mb = 0; mb < 4; ++mb) {
+              if (8 * mb + 7 >= m_lo && 8 * mb < m_hi) {
+#pragma unroll
+                for (int m = 8 * mb; m < 8 * mb + 8; ++m) {
+                  const float2 qv = qs[32 * m];
+                  acc[m] = unpk(fma2(pk(-qv.y, qv.x), r.yy, fma2(pk(qv), r.xx, pk(acc[m]))));
+                }
+              }
             }
           }
         }
