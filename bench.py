@@ -34,7 +34,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_0906_4175_b200 import inputs  # noqa: E402
+import workloads as inputs  # noqa: E402
 
 METRIC = "template-segments/sec at N=2^20, p=16 (SNR+chi^2)"
 UNIT = "template-segments/s"

@@ -8,7 +8,7 @@ import pytest
 
 import oracle
 import parity
-from paper_0906_4175_b200 import inputs
+import workloads as inputs
 
 pytestmark = pytest.mark.gpu
 

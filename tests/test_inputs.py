@@ -4,7 +4,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_0906_4175_b200 import inputs
+import workloads as inputs
 
 
 def test_rng_is_a_pure_function_of_its_coordinates():

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_0906_4175_b200 import inputs
+import workloads as inputs
 
 
 def _rows(path):

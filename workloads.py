@@ -1,4 +1,5 @@
-"""Seeded synthetic workloads for the inspiral matched-filter hot path.
+"""Seeded synthetic workloads for the inspiral matched-filter hot path (test and bench inputs; not part of
+the shipped library package).
 
 This module is the ONLY code shared by the oracle tests and the CUDA tests/bench.
 It produces *inputs* (a strain segment s(t), a one-sided PSD array S_n(f_k), a list
