@@ -45,6 +45,20 @@ typedef enum {
   GWMF_E_WORKSPACE = -6       /* workspace smaller than gwmf_workspace_bytes()                      */
 } gwmf_status;
 
+/* Which kernels compute the p band transforms of step a3 (all three compute the same rho, chi^2 and events):
+ *   TWO_PASS   pass 1 writes every band's intermediate to HBM (p n complex per template), pass 2 reads it;
+ *   FUSED      spill-free: narrow bands are formed inside the row-transform kernel (n <= 2^20);
+ *   DECIMATED  narrow bands are transformed on a coarse grid of L >= 2 B points, their power spectra summed, and one
+ *              n-point transform returns sum_l |z_l|^2; only z, that sum and the wide bands keep n-point transforms
+ *              (n >= 2^15).  DESIGN.md section 5.
+ *   AUTO       the library's choice: DECIMATED for n >= 2^15, TWO_PASS below. */
+typedef enum {
+  GWMF_PATH_AUTO = 0,
+  GWMF_PATH_TWO_PASS = 1,
+  GWMF_PATH_FUSED = 2,
+  GWMF_PATH_DECIMATED = 3
+} gwmf_path;
+
 typedef struct gwmf_ctx gwmf_ctx;                      /* opaque */
 
 typedef struct { double m1, m2; } gwmf_mass_pair;      /* solar masses, > 0, any order */
@@ -67,6 +81,8 @@ typedef struct {
   int32_t batch;         /* templates filtered per kernel launch, 0 .. 64 (0 = library default: about
                             2 GiB of band intermediate); sizes the band-intermediate buffer,
                             batch * p * n * 8 bytes, and the correlated spectra, 2 * batch * n * 4 bytes */
+  int32_t path;          /* a gwmf_path; GWMF_PATH_AUTO (0) = the library's choice.  A path that does not support n
+                            (FUSED: 2^15 .. 2^20, DECIMATED: >= 2^15) is GWMF_E_ARG                               */
 } gwmf_params;
 
 /* Bytes of DEVICE memory the caller must provide to gwmf_create (0 if params are invalid). */
@@ -99,16 +115,21 @@ int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_t
 int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn);
 
 /* Matched-filter templates [first_template, first_template + n_templates) against the loaded segment
- * (the host may wait here for the segment preparation to finish: the call reads back which bands of which
- * templates need the wide-band kernels):
+ * (the FIRST call after a bank or PSD change waits on the host for the bank setup to finish: it reads back how
+ * many transforms each template needs; later calls do not wait):
  * p band inverse FFTs, rho and chi^2 at every sample (Eq. 3, 5) and the per-window
  * maxima above threshold.  Trigger slots of those templates are reset first.  async. */
 int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
 
-/* Measurement: the same work as gwmf_filter, with CUDA events recorded on the context's stream around
- * every launch of the two hot kernels.  host_ms[0] / host_ms[1] receive the summed device time (ms) of
- * the pass-1 (correlate + first FFT pass) and pass-2 (second FFT pass + rho/chi^2/trigger epilogue)
- * launches, host_launches[0..1] the number of launches of each.  syncs. */
+/* Measurement: the same work as gwmf_filter, with CUDA events recorded on the context's stream around the three
+ * stages of every batch.  host_ms: HOST array of 3 doubles, summed device time (ms) of
+ *   [0] the spectra of the decimated path (correlate, coarse-grid band powers, U+), serialised on the main stream
+ *       for this call (gwmf_filter runs them beside pass 1 on a side stream); 0 for the other paths, whose
+ *       correlate step is inside [1];
+ *   [1] pass 1: first FFT pass of every (effective) band -> band intermediate in HBM; for the spill-free path only
+ *       the wide bands' kernels;
+ *   [2] pass 2: last FFT stage + rho/chi^2/trigger epilogue (spill-free path: k_fused).
+ * host_launches: HOST array of 3 int32, batches timed in each stage.  syncs. */
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
                       int32_t* host_launches);
 
@@ -142,11 +163,11 @@ int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q);
  * interleaved complex fp32 (re, im), n = params.n; in != out.  async. */
 int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out);
 
-/* 1 if this context filters with the spill-free kernel (k_fused: narrow bands are formed from the correlated
- * spectrum inside the row-transform kernel and never reach HBM), 0 if with the two-pass path (band intermediate
- * written by pass 1, read by pass 2).  Chosen at gwmf_create: spill-free for n <= 2^20, two-pass above; the
- * environment variable GWMF_FUSED=0/1 overrides.  Both paths compute the same quantities. */
+/* 1 if this context filters with the spill-free kernel (gwmf_params::path = GWMF_PATH_FUSED), else 0. */
 int gwmf_uses_fused(const gwmf_ctx* ctx);
+
+/* The gwmf_path this context filters with (GWMF_PATH_AUTO resolved at gwmf_create); GWMF_E_ARG for a null ctx. */
+int gwmf_path_in_use(const gwmf_ctx* ctx);
 
 /* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
 int64_t gwmf_launch_count(const gwmf_ctx* ctx);

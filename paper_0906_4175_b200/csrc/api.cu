@@ -26,7 +26,16 @@ bool params_ok(const gwmf_params* p) {
   if (p->max_templates < 1) return false;
   if (p->batch < 0 || p->batch > kMaxBatch) return false;
   if (!(p->rho_thresh >= 0.0)) return false;
+  if (p->path < GWMF_PATH_AUTO || p->path > GWMF_PATH_DECIMATED) return false;
+  if (p->path == GWMF_PATH_FUSED && (p->n < (1 << 15) || p->n > (1 << 20))) return false;
+  if (p->path == GWMF_PATH_DECIMATED && p->n < (1 << 15)) return false;
   return true;
+}
+
+int resolve_path(const gwmf_params* p) {
+  // the decimated path needs n1 = n / 1024 >= 32; below that every band goes through the generic two-pass kernels
+  if (p->path != GWMF_PATH_AUTO) return p->path;
+  return p->n >= (1 << 15) ? GWMF_PATH_DECIMATED : GWMF_PATH_TWO_PASS;
 }
 
 int default_batch(const gwmf_params* p) {
@@ -70,8 +79,14 @@ Layout make_layout(const gwmf_params* p) {
   L.series_rho = take(n * sizeof(float));
   L.series_chi = take(n * sizeof(float));
   L.flags = take(256);
+  L.tw_l = take((size_t)kLMax * sizeof(float2));
+  L.eff = take((2 * T + 1) * sizeof(int32_t));
+  const int path = resolve_path(p);
   L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
-  L.qb = take(2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2));   // band-separated copy (k_fused)
+  L.qb = take(path == GWMF_PATH_FUSED ? 2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2) : 256);   // band-separated copy (k_fused)
+  // decimated path: per-band one-sided power spectra W_l and their sum U+, double-buffered across batches
+  L.wbuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * (size_t)p->p * kUCap * sizeof(float2) : 256);
+  L.ubuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * kUCap * sizeof(float2) : 256);
   size_t yb = (size_t)L.batch * (size_t)p->p * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;
@@ -90,6 +105,17 @@ int fail_cuda(Ctx* c, cudaError_t e) {
     cudaError_t e__ = (call);                          \
     if (e__ != cudaSuccess) return fail_cuda(c, e__);  \
   } while (0)
+
+// Every entry point runs on the context's device whatever device is current in the calling thread, and restores
+// the caller's device on return.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 // Host-side scalars of template I = (m1, m2) (phase of BASELINE.json:configs[0]):
 // phase coefficients in turns for u = f^(-1/3), and the first bin above the template.
@@ -157,16 +183,21 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->stream = (cudaStream_t)cuda_stream;
   c->n_templates = 0;
   c->have_bank = c->have_segment = false;
-  {
-    // path selection: the spill-free kernel wins while bands stay a few rows wide (n <= 2^20: measured +8..11 %
-    // at n = 2^18 and 2^20, -18 % at 2^22); GWMF_FUSED=0/1 forces the two-pass / the spill-free path
-    const char* f = getenv("GWMF_FUSED");
-    if (f && (f[0] == '0' || f[0] == '1')) c->fused = f[0] == '1';
-    else c->fused = params->n <= (1 << 20) && params->n >= (1 << 15);
-  }
+  c->path = resolve_path(params);
+  c->fused = c->path == GWMF_PATH_FUSED;
+  c->device = dev;
+  c->s_bins = (int)(params->n / 16 < kSBinsMax ? params->n / 16 : kSBinsMax);
+  c->t_max = 16;
   c->launches = 0;
   c->h_meta = nullptr;
   c->h_masks = nullptr;
+  c->h_eff = nullptr;
+  c->mirror_ready = false;
+  // > 48 KB of dynamic shared memory is an opt-in per function AND per device: do it for this context's device
+  if (configure_pass1(c->path) != cudaSuccess || configure_pass2() != cudaSuccess || configure_bandpower() != cudaSuccess) {
+    delete c;
+    return GWMF_E_CUDA;
+  }
   c->side = nullptr;
   c->ev_fork = c->ev_join = c->ev_masks = nullptr;
   {
@@ -176,11 +207,14 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_masks, cudaEventDisableTiming) != cudaSuccess ||
-        cudaMallocHost((void**)&c->h_masks, sizeof(uint32_t) * (size_t)params->max_templates) != cudaSuccess) {
+        cudaMallocHost((void**)&c->h_masks, sizeof(uint32_t) * (size_t)params->max_templates) != cudaSuccess ||
+        cudaMallocHost((void**)&c->h_eff, sizeof(int32_t) * (size_t)(2 * params->max_templates + 1)) != cudaSuccess) {
       if (c->side) cudaStreamDestroy(c->side);
       if (c->ev_fork) cudaEventDestroy(c->ev_fork);
       if (c->ev_join) cudaEventDestroy(c->ev_join);
       if (c->ev_masks) cudaEventDestroy(c->ev_masks);
+      if (c->h_masks) cudaFreeHost(c->h_masks);
+      if (c->h_eff) cudaFreeHost(c->h_eff);
       delete c;
       return GWMF_E_CUDA;
     }
@@ -203,12 +237,14 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
 void gwmf_destroy(gwmf_ctx* ctx) {
   if (!ctx) return;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   cudaStreamSynchronize(c->stream);
   if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
   if (c->ev_masks) cudaEventDestroy(c->ev_masks);
   if (c->h_masks) cudaFreeHost(c->h_masks);
+  if (c->h_eff) cudaFreeHost(c->h_eff);
   if (c->h_meta) cudaFreeHost(c->h_meta);
   delete c;
 }
@@ -216,6 +252,7 @@ void gwmf_destroy(gwmf_ctx* ctx) {
 int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_templates) {
   if (!ctx || !host_masses) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   if (n_templates < 1 || n_templates > c->prm.max_templates) return GWMF_E_ARG;
   CU(cudaStreamSynchronize(c->stream));            // h_meta may still be in flight from a previous call
   for (int t = 0; t < n_templates; ++t) {
@@ -234,6 +271,7 @@ int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_t
 int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn) {
   if (!ctx || !s || !Sn) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   CU(cudaMemcpyAsync(ws_ptr<float>(c, c->lay.s_in), s, sizeof(float) * (size_t)c->n, cudaMemcpyDefault, c->stream));
   CU(cudaMemcpyAsync(ws_ptr<double>(c, c->lay.sn), Sn, sizeof(double) * (size_t)(c->n / 2 + 1), cudaMemcpyDefault,
                      c->stream));
@@ -250,58 +288,132 @@ int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn) {
   return GWMF_OK;
 }
 
-int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates) {
-  if (!ctx) return GWMF_E_ARG;
-  Ctx* c = reinterpret_cast<Ctx*>(ctx);
-  if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
-  if (first_template < 0 || n_templates < 0 || first_template + n_templates > c->n_templates) return GWMF_E_ARG;
-  if (n_templates == 0) return GWMF_OK;
+// ---- host mirrors of the per-template masks / effective-band counts (written by the bank setup) ----
+// Waited for ONCE after every bank setup, not per call.
+static int ensure_mirror(Ctx* c) {
+  if (!c->mirror_ready) {
+    CU(cudaEventSynchronize(c->ev_masks));
+    c->mirror_ready = true;
+  }
+  return GWMF_OK;
+}
+
+// Q, W_l and U+ of a batch (decimated path), on stream st
+static cudaError_t launch_spectra(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+  cudaError_t e = launch_correlate(c, first, count, parity, st);
+  if (e == cudaSuccess) e = launch_bandpower(c, first, count, parity, st);
+  return e;
+}
+
+static bool any_generic(const Ctx* c, int first, int count) {
+  for (int t = first; t < first + count; ++t)
+    if (c->h_eff[c->n_templates + 1 + t]) return true;
+  return false;
+}
+
+// One batch of the decimated path.  Main stream: pass 1 of the effective bands, pass 2.  Side stream (high
+// priority, between a fork and a join): the generic kernel for the very wide bands of THIS batch, then the spectra
+// (correlate, band powers) of the NEXT batch into the other half of the double buffers.
+//   ev: optional 4 events (timed mode: everything serialised on the main stream) recorded before the spectra,
+//   before pass 1, before pass 2 and after pass 2.
+static cudaError_t decimated_batch(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool ready,
+                                   bool update_slots, float* series_rho, float* series_chi, cudaEvent_t* ev) {
+  cudaError_t e;
+  const bool gen = any_generic(c, first, count);
+  if (ev) {
+    if ((e = cudaEventRecord(ev[0], c->stream)) != cudaSuccess) return e;
+    if ((e = launch_spectra(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(ev[1], c->stream)) != cudaSuccess) return e;
+    if (gen && (e = launch_pass1_generic_eff(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+    if ((e = launch_pass1_eff(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(ev[2], c->stream)) != cudaSuccess) return e;
+    if ((e = launch_pass2_eff(c, first, count, update_slots, series_rho, series_chi)) != cudaSuccess) return e;
+    return cudaEventRecord(ev[3], c->stream);
+  }
+  if (!ready && (e = launch_spectra(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+  const bool side_work = gen || next_count > 0;
+  if (side_work) {
+    // fork: everything enqueued so far on the main stream (this batch's spectra, the previous batch's pass 2, which
+    // read the band buffer and the other half of the spectra buffers) precedes the side work
+    if ((e = cudaEventRecord(c->ev_fork, c->stream)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(c->side, c->ev_fork, 0)) != cudaSuccess) return e;
+    if (gen && (e = launch_pass1_generic_eff(c, first, count, parity, c->side)) != cudaSuccess) return e;
+    if (next_count > 0 && (e = launch_spectra(c, next_first, next_count, parity ^ 1, c->side)) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(c->ev_join, c->side)) != cudaSuccess) return e;
+  }
+  if ((e = launch_pass1_eff(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+  if (side_work && (e = cudaStreamWaitEvent(c->stream, c->ev_join, 0)) != cudaSuccess) return e;
+  return launch_pass2_eff(c, first, count, update_slots, series_rho, series_chi);
+}
+
+// All batches of [first_template, first_template + n_templates).  ev: 4 events per batch (timed mode) or nullptr.
+static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t* ev) {
+  int rc = ensure_mirror(c);
+  if (rc != GWMF_OK) return rc;
   CU(launch_reset_slots(c, first_template, n_templates));
-  int parity = 0;
-  for (int done = 0; done < n_templates; done += c->lay.batch, parity ^= 1) {
+  int parity = 0, b = 0;
+  for (int done = 0; done < n_templates; done += c->lay.batch, parity ^= 1, ++b) {
     const int cnt = n_templates - done < c->lay.batch ? n_templates - done : c->lay.batch;
     const int rest = n_templates - done - cnt;
     const int next = rest < c->lay.batch ? rest : c->lay.batch;
-    CU(launch_pass1_filter(c, first_template + done, cnt, first_template + done + cnt, next, parity, done > 0));
-    if (c->fused) CU(launch_fused_filter(c, first_template + done, cnt, parity, true, nullptr, nullptr));
-    else CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
+    const int f0 = first_template + done;
+    cudaEvent_t* evb = ev ? ev + 4 * b : nullptr;
+    if (c->path == GWMF_PATH_DECIMATED) {
+      CU(decimated_batch(c, f0, cnt, f0 + cnt, next, parity, done > 0, true, nullptr, nullptr, evb));
+      continue;
+    }
+    if (evb) CU(cudaEventRecord(evb[0], c->stream));
+    if (evb) CU(cudaEventRecord(evb[1], c->stream));
+    CU(launch_pass1_filter(c, f0, cnt, f0 + cnt, next, parity, done > 0));
+    if (evb) CU(cudaEventRecord(evb[2], c->stream));
+    if (c->fused) CU(launch_fused_filter(c, f0, cnt, parity, true, nullptr, nullptr));
+    else CU(launch_pass2_filter(c, f0, cnt, true, nullptr, nullptr));
+    if (evb) CU(cudaEventRecord(evb[3], c->stream));
   }
   return GWMF_OK;
+}
+
+static bool range_ok(const Ctx* c, int32_t first_template, int32_t n_templates) {
+  return first_template >= 0 && n_templates >= 0 && first_template <= c->n_templates &&
+         n_templates <= c->n_templates - first_template;          // no signed overflow for hostile arguments
+}
+
+int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates) {
+  if (!ctx) return GWMF_E_ARG;
+  Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
+  if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
+  if (!range_ok(c, first_template, n_templates)) return GWMF_E_ARG;
+  if (n_templates == 0) return GWMF_OK;
+  return run_batches(c, first_template, n_templates, nullptr);
 }
 
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
                       int32_t* host_launches) {
   if (!ctx || !host_ms || !host_launches) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
-  if (first_template < 0 || n_templates < 1 || first_template + n_templates > c->n_templates) return GWMF_E_ARG;
+  if (!range_ok(c, first_template, n_templates) || n_templates < 1) return GWMF_E_ARG;
   const int nb = (n_templates + c->lay.batch - 1) / c->lay.batch;
-  std::vector<cudaEvent_t> ev((size_t)nb * 3);
-  for (auto& e : ev) CU(cudaEventCreate(&e));
-  CU(launch_reset_slots(c, first_template, n_templates));
-  for (int b = 0; b < nb; ++b) {
-    int done = b * c->lay.batch;
-    int cnt = n_templates - done < c->lay.batch ? n_templates - done : c->lay.batch;
-    const int rest = n_templates - done - cnt;
-    const int next = rest < c->lay.batch ? rest : c->lay.batch;
-    CU(cudaEventRecord(ev[3 * b], c->stream));
-    CU(launch_pass1_filter(c, first_template + done, cnt, first_template + done + cnt, next, b & 1, b > 0));
-    CU(cudaEventRecord(ev[3 * b + 1], c->stream));
-    if (c->fused) CU(launch_fused_filter(c, first_template + done, cnt, b & 1, true, nullptr, nullptr));
-    else CU(launch_pass2_filter(c, first_template + done, cnt, true, nullptr, nullptr));
-    CU(cudaEventRecord(ev[3 * b + 2], c->stream));
-  }
+  struct Events {                                   // destroyed on every exit path
+    std::vector<cudaEvent_t> v;
+    ~Events() { for (cudaEvent_t e : v) if (e) cudaEventDestroy(e); }
+  } ev;
+  ev.v.assign((size_t)nb * 4, nullptr);
+  for (auto& e : ev.v) CU(cudaEventCreate(&e));
+  int rc = run_batches(c, first_template, n_templates, ev.v.data());
+  if (rc != GWMF_OK) return rc;
   CU(cudaStreamSynchronize(c->stream));
-  host_ms[0] = host_ms[1] = 0.0;
-  for (int b = 0; b < nb; ++b) {
-    float m1 = 0.f, m2 = 0.f;
-    CU(cudaEventElapsedTime(&m1, ev[3 * b], ev[3 * b + 1]));
-    CU(cudaEventElapsedTime(&m2, ev[3 * b + 1], ev[3 * b + 2]));
-    host_ms[0] += m1;
-    host_ms[1] += m2;
-  }
-  host_launches[0] = host_launches[1] = nb;
-  for (auto& e : ev) cudaEventDestroy(e);
+  host_ms[0] = host_ms[1] = host_ms[2] = 0.0;
+  for (int b = 0; b < nb; ++b)
+    for (int i = 0; i < 3; ++i) {
+      float m = 0.f;
+      CU(cudaEventElapsedTime(&m, ev.v[4 * b + i], ev.v[4 * b + i + 1]));
+      host_ms[i] += m;
+    }
+  host_launches[0] = c->path == GWMF_PATH_DECIMATED ? nb : 0;
+  host_launches[1] = host_launches[2] = nb;
   return GWMF_OK;
 }
 
@@ -316,6 +428,7 @@ static int check_flags(Ctx* c) {
 int gwmf_triggers(gwmf_ctx* ctx, gwmf_trigger* host_out, int64_t capacity, int64_t* n_out) {
   if (!ctx || !n_out || capacity < 0 || (capacity > 0 && !host_out)) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   *n_out = 0;
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
   // compaction first, then ONE synchronisation for the input-check flag and the event count
@@ -351,6 +464,7 @@ static int fetch_meta(Ctx* c, std::vector<TemplateMeta>& v) {
 int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma) {
   if (!ctx || !host_sigma) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   std::vector<TemplateMeta> v;
   int rc = fetch_meta(c, v);
   if (rc != GWMF_OK) return rc;
@@ -361,6 +475,7 @@ int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma) {
 int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges) {
   if (!ctx || !host_edges) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   std::vector<TemplateMeta> v;
   int rc = fetch_meta(c, v);
   if (rc != GWMF_OK) return rc;
@@ -373,15 +488,22 @@ int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges) {
 int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host_chisq) {
   if (!ctx) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
   if (template_id < 0 || template_id >= c->n_templates) return GWMF_E_ARG;
   int rc = check_flags(c);
   if (rc != GWMF_OK) return rc;
   float* d_rho = ws_ptr<float>(c, c->lay.series_rho);
   float* d_chi = ws_ptr<float>(c, c->lay.series_chi);
-  CU(launch_pass1_filter(c, template_id, 1, 0, 0, 0, false));
-  if (c->fused) CU(launch_fused_filter(c, template_id, 1, 0, false, d_rho, d_chi));
-  else CU(launch_pass2_filter(c, template_id, 1, false, d_rho, d_chi));
+  rc = ensure_mirror(c);
+  if (rc != GWMF_OK) return rc;
+  if (c->path == GWMF_PATH_DECIMATED) {
+    CU(decimated_batch(c, template_id, 1, 0, 0, 0, false, false, d_rho, d_chi, nullptr));
+  } else {
+    CU(launch_pass1_filter(c, template_id, 1, 0, 0, 0, false));
+    if (c->fused) CU(launch_fused_filter(c, template_id, 1, 0, false, d_rho, d_chi));
+    else CU(launch_pass2_filter(c, template_id, 1, false, d_rho, d_chi));
+  }
   if (host_rho)
     CU(cudaMemcpyAsync(host_rho, d_rho, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
   if (host_chisq)
@@ -393,6 +515,7 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
 int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q) {
   if (!ctx || !host_q) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
   if (template_id < 0 || template_id >= c->n_templates) return GWMF_E_ARG;
   int rc = check_flags(c);
@@ -409,6 +532,7 @@ int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q) {
 int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out) {
   if (!ctx || !d_in || !d_out || d_in == d_out) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
   // the band intermediate doubles as the pass-1 output of the dense transform
   CU(launch_fft_dense(c, reinterpret_cast<const float2*>(d_in), ws_ptr<float2>(c, c->lay.y),
                       reinterpret_cast<float2*>(d_out)));
@@ -416,6 +540,8 @@ int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out) {
 }
 
 int gwmf_uses_fused(const gwmf_ctx* ctx) { return ctx && reinterpret_cast<const Ctx*>(ctx)->fused ? 1 : 0; }
+
+int gwmf_path_in_use(const gwmf_ctx* ctx) { return ctx ? reinterpret_cast<const Ctx*>(ctx)->path : GWMF_E_ARG; }
 
 int64_t gwmf_launch_count(const gwmf_ctx* ctx) {
   return ctx ? reinterpret_cast<const Ctx*>(ctx)->launches : 0;

@@ -1,0 +1,166 @@
+// bandpower.cu -- decimated path, the chi^2 side of step a3/a4 for the narrow bands (class S: at most s_bins bins).
+//
+// Eq. 5 needs sum_l |z_l[j]|^2 at every sample j (identity P7: sum_l |z_l - z/p|^2 =
+// sum_l |z_l|^2 - |z|^2/p).  A band of B contiguous bins gives z_l[j] = e^{2 pi i j e_l/n} y_l[j] with y_l
+// band-limited to B bins, so u_l[j] = |z_l[j]|^2 = |y_l[j]|^2 is a REAL series whose spectrum lives on the bins
+// |m| < B:  u_l[j] = sum_{|m|<B} U_l[m] e^{2 pi i jm/n},  U_l[m] = sum_k Q[k+m] conj(Q[k]).  Sampling u_l on a
+// coarse grid of L >= 2B points (every (n/L)-th sample) therefore loses nothing:
+//     y_l[j'] = sum_{i<B} Q[e_l + i] e^{2 pi i j' i/L}            (L-point inverse transform of the band, in shared memory)
+//     w_l[j'] = |y_l[j']|^2 = u_l[j' n/L]
+//     U_l[m]  = (1/L) sum_{j'} w_l[j'] e^{-2 pi i j' m/L},  |m| < L/2   (L-point forward transform)
+// The spectra of all class-S bands of a template are added bin by bin in a fixed order,
+//     U+[m] = (m == 0 ? 1 : 2) sum_{l in S} U_l[m],  0 <= m < u_hi = max_l B_l,
+// and ONE n-point inverse transform of U+ (an "effective band" of the two-pass FFT, pass1.cu / pass2.cu) returns
+// sum_{l in S} |z_l[j]|^2 = Re IFFT_n(U+)[j] at every sample: exact trigonometric interpolation, no approximation.
+// The p n-point transforms of the paper's Fig. 3 become: one for z (the union of the S bands), one
+// for U+, one per wide (class D) band -- about 2.7 instead of 16 at the headline config -- plus 2 L-point
+// transforms per narrow band, L = 2^11 .. 2^14 (a few percent of one n-point transform each).
+//
+// The L-point transforms run in place in shared memory as radix 32 x 32 x (L/1024): decimation in frequency on the
+// way in (natural -> digit-reversed order), |.|^2 element-wise, decimation in time on the way out (digit-reversed ->
+// natural): no permutation pass.  The forward transform of the real w is conj(inverse transform).
+#include "fft_reg.cuh"
+#include "gwmf_internal.cuh"
+
+namespace gwmf {
+
+__device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }        // one float2 of padding per 16: the
+                                                                            // stride-1 groups of the last stage become conflict-free
+constexpr int kBpThreads = 512;
+constexpr size_t kBpSmem = (size_t)(kLMax + (kLMax >> 4)) * sizeof(float2);
+
+template <int LOG_L>
+__device__ __forceinline__ void bandpower_body(float2* __restrict__ sm, const float2* __restrict__ tw_l,
+                                               const float2* __restrict__ qband, int B, float2* __restrict__ wout) {
+  constexpr int L = 1 << LOG_L;
+  constexpr int R3 = L / 1024;                    // last radix: 2, 4, 8, 16
+  constexpr int S1 = L / 32;                      // stride of the first radix-32 stage
+  constexpr int TWS = kLMax / L;                  // tw_l[t * TWS] = e^{2 pi i t / L}
+  const int tid = threadIdx.x;
+
+  for (int i = tid; i < L; i += kBpThreads) sm[pad16(i)] = i < B ? qband[i] : make_float2(0.f, 0.f);
+  __syncthreads();
+  // ---- inverse transform, decimation in frequency: stage 1 (inputs i >= L/2 are zero since L >= 2B)
+  for (int o = tid; o < S1; o += kBpThreads) {
+    float2 x[32];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[brev<32>(q)] = sm[pad16(o + S1 * q)];
+    fft_dit<32, 16>(x);
+#pragma unroll
+    for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = cmul(x[k], tw_l[((o * k) & (L - 1)) * TWS]);
+  }
+  __syncthreads();
+  // ---- stage 2: inside each block k1 of S1 = 32 R3 points
+  for (int g = tid; g < S1; g += kBpThreads) {
+    const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
+    float2 x[32];
+#pragma unroll
+    for (int q = 0; q < 32; ++q) x[brev<32>(q)] = sm[pad16(base + R3 * q)];
+    fft_dit<32>(x);
+#pragma unroll
+    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = cmul(x[k], tw_l[((32 * o2 * k) & (L - 1)) * TWS]);
+  }
+  __syncthreads();
+  // ---- stage 3 (R3 points, stride 1), |y|^2, and the first stage of the way back (same groups, no twiddle)
+  for (int g = tid; g < 1024; g += kBpThreads) {
+    const int base = g * R3;
+    float2 x[R3];
+#pragma unroll
+    for (int q = 0; q < R3; ++q) x[brev<R3>(q)] = sm[pad16(base + q)];
+    fft_dit<R3>(x);
+    float2 w[R3];
+#pragma unroll
+    for (int q = 0; q < R3; ++q) w[brev<R3>(q)] = make_float2(fmaf(x[q].x, x[q].x, x[q].y * x[q].y), 0.f);
+    fft_dit<R3>(w);
+#pragma unroll
+    for (int k = 0; k < R3; ++k) sm[pad16(base + k)] = w[k];
+  }
+  __syncthreads();
+  // ---- decimation in time: twiddle first, then the radix-32 transform (transposes of stages 2 and 1)
+  for (int g = tid; g < S1; g += kBpThreads) {
+    const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
+    float2 x[32];
+#pragma unroll
+    for (int q = 0; q < 32; ++q) x[brev<32>(q)] = cmul(sm[pad16(base + R3 * q)], tw_l[((32 * o2 * q) & (L - 1)) * TWS]);
+    fft_dit<32>(x);
+#pragma unroll
+    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = x[k];
+  }
+  __syncthreads();
+  // last stage: only the outputs m = o + S1 k < B <= L/2 are wanted, i.e. k < 16; they leave straight to global memory
+  const float inv_l = 1.0f / (float)L;
+  for (int o = tid; o < S1; o += kBpThreads) {
+    float2 x[32];
+#pragma unroll
+    for (int q = 0; q < 32; ++q) x[brev<32>(q)] = cmul(sm[pad16(o + S1 * q)], tw_l[((o * q) & (L - 1)) * TWS]);
+    fft_dit<32>(x);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int m = o + S1 * k;
+      if (m < B) {
+        const float sc = m == 0 ? inv_l : 2.0f * inv_l;                  // one-sided: U+[m] = 2 U[m] for m > 0
+        wout[m] = make_float2(x[k].x * sc, -x[k].y * sc);               // conj: forward transform of a real series
+      }
+    }
+  }
+}
+
+// grid (p, templates of the batch): W[tb][l][m] = one-sided power spectrum of class-S band l, 0 <= m < B_l
+__global__ void __launch_bounds__(kBpThreads, 1) k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q,
+                                                             const float2* __restrict__ tw_l, float2* __restrict__ wbuf,
+                                                             int p, int half_n) {
+  extern __shared__ __align__(16) float2 sm_bp[];
+  const int l = blockIdx.x, tb = blockIdx.y;
+  const TemplateMeta* m = meta + tb;
+  if (!((m->s_mask >> l) & 1u)) return;
+  const int e_lo = m->edges[l], B = m->edges[l + 1] - e_lo;
+  const float2* qband = q + (size_t)tb * half_n + e_lo;
+  float2* wout = wbuf + ((size_t)tb * p + l) * kUCap;
+  int log_l = kLogLMin;
+  while ((1 << log_l) < 2 * B) ++log_l;
+  switch (log_l) {
+    case 11: bandpower_body<11>(sm_bp, tw_l, qband, B, wout); break;
+    case 12: bandpower_body<12>(sm_bp, tw_l, qband, B, wout); break;
+    case 13: bandpower_body<13>(sm_bp, tw_l, qband, B, wout); break;
+    default: bandpower_body<14>(sm_bp, tw_l, qband, B, wout); break;
+  }
+}
+
+// U+[tb][m] = sum over the class-S bands, ascending l (fixed order: bit-reproducible), 0 <= m < u_hi
+__global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wbuf,
+                                               float2* __restrict__ ubuf, int p) {
+  const int tb = blockIdx.y, m = blockIdx.x * 256 + threadIdx.x;
+  const TemplateMeta* mt = meta + tb;
+  if (m >= mt->u_hi) return;
+  float2 acc = make_float2(0.f, 0.f);
+  unsigned s = mt->s_mask;
+  while (s) {
+    const int l = __ffs(s) - 1;
+    s &= s - 1;
+    if (m < mt->edges[l + 1] - mt->edges[l]) {
+      const float2 v = wbuf[((size_t)tb * p + l) * kUCap + m];
+      acc.x += v.x;
+      acc.y += v.y;
+    }
+  }
+  ubuf[(size_t)tb * kUCap + m] = acc;
+}
+
+cudaError_t configure_bandpower() {
+  return cudaFuncSetAttribute(k_bandpower, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBpSmem);
+}
+
+cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+  const int p = c->prm.p;
+  const size_t half = (size_t)(c->n / 2);
+  const TemplateMeta* meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
+  const float2* q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half;
+  float2* wbuf = ws_ptr<float2>(c, c->lay.wbuf) + (size_t)parity * c->lay.batch * p * kUCap;
+  float2* ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
+  k_bandpower<<<dim3(p, count), kBpThreads, kBpSmem, st>>>(meta, q, ws_ptr<float2>(c, c->lay.tw_l), wbuf, p, (int)half);
+  k_uspec<<<dim3(c->s_bins / 256, count), 256, 0, st>>>(meta, wbuf, ubuf, p);
+  c->launches += 2;
+  return cudaGetLastError();
+}
+
+}  // namespace gwmf

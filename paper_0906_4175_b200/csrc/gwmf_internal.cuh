@@ -13,6 +13,12 @@ constexpr int kLogN2 = 10;
 constexpr int kMaxBands = 32;
 constexpr int kColsPerCta = 8;   // pass-1 column tile: 8 columns x 8 B = 64 B segments per output row
 constexpr int kP2Warps = 8;      // pass-2 rows (j1 values) per CTA, one warp each
+// Decimated path: a band of at most kSBinsMax bins is transformed on a coarse grid of L <= kLMax points (class S);
+// wider bands keep their own n-point transform (class D).  See bandpower.cu.
+constexpr int kSBinsMax = 8192;
+constexpr int kLMax = 16384;
+constexpr int kLogLMin = 11;     // smallest coarse grid (2048 points)
+constexpr int kUCap = kSBinsMax; // entries of the one-sided power spectrum U+ kept per template
 
 // Per-template record (device).  Phase in TURNS: psi(u) = (((c0 u^2 + c2) u + c3) u + c4) u - 1/8 with
 // u = f^(-1/3); this is Psi0/(2 pi) of the 2PN SPA phase (BASELINE.json:configs[0]).
@@ -24,7 +30,39 @@ struct TemplateMeta {
   int32_t edges[kMaxBands + 1];  // band l = bins [edges[l], edges[l+1])
   uint32_t wide_mask;            // bit l: band l goes through the generic pass-1 kernel (> 32 input rows)
   uint16_t row_off[kMaxBands + 2];  // band-separated spectrum Qb: rows of narrow band l start at row_off[l] (k_fused)
+  // ---- decimated path: the template's EFFECTIVE bands (n-point transforms that are really run) ----
+  //   if s_mask != 0:  e = 0: Z = the union of the class-S bands (one transform, gives their share of z)
+  //                    e = 1: U = one-sided spectrum of sum_{l in S} |z_l|^2 (real part of its transform)
+  //   then one per class-D band in ascending l (z_l itself: contributes to z and to sum |z_l|^2)
+  uint32_t s_mask;               // bit l: band l is class S (0 < bins <= s_bins)
+  uint32_t d_mask;               // bit l: band l is class D (bins > s_bins)
+  uint32_t gen_mask;             // bit e: effective band e goes through the generic pass-1 kernel (very many input rows)
+  int32_t eff_prefix;            // effective bands of all earlier templates of the bank
+  int32_t n_eff;                 // effective bands of this template
+  int32_t z_lo, z_hi;            // hull of the class-S bands, bins [z_lo, z_hi)
+  int32_t u_hi;                  // support of U+: bins [0, u_hi), u_hi = widest class-S band
 };
+
+// One effective band: which spectrum it reads (kind) and the bins [e_lo, e_hi) it owns.
+enum EffKind { kEffZ = 0, kEffU = 1, kEffD = 2 };
+struct EffBand { int kind, e_lo, e_hi, l; };
+#ifdef __CUDACC__
+__device__ __forceinline__ EffBand eff_band(const TemplateMeta* m, int e) {
+  EffBand b;
+  if (m->s_mask) {
+    if (e == 0) { b.kind = kEffZ; b.e_lo = m->z_lo; b.e_hi = m->z_hi; b.l = -1; return b; }
+    if (e == 1) { b.kind = kEffU; b.e_lo = 0; b.e_hi = m->u_hi; b.l = -1; return b; }
+    e -= 2;
+  }
+  unsigned d = m->d_mask;
+  for (int i = 0; i < e; ++i) d &= d - 1;
+  b.l = __ffs(d) - 1;
+  b.kind = kEffD;
+  b.e_lo = m->edges[b.l];
+  b.e_hi = m->edges[b.l + 1];
+  return b;
+}
+#endif
 
 // One (template, window) trigger slot, updated with a 128-bit compare-and-swap.
 //   key  = (bits(rho) << 32) | (0xFFFFFFFF - sample)   -> max key = max rho, lowest sample on ties
@@ -36,7 +74,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, qb, y, total;
+         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, total;
   size_t y_bytes;
   int batch;
 };
@@ -58,7 +96,13 @@ struct Ctx {
   cudaEvent_t ev_fork, ev_join;
   int n_templates;
   bool have_bank, have_segment;
-  bool fused;                    // spill-free kernel (k_fused) instead of narrow pass 1 + pass 2 (n <= 2^20; GWMF_FUSED)
+  int path;                      // GWMF_PATH_TWO_PASS / _FUSED / _DECIMATED (resolved from gwmf_params::path at create)
+  bool fused;                    // path == GWMF_PATH_FUSED
+  int device;                    // CUDA device the context lives on
+  int s_bins;                    // decimated path: class-S threshold in bins = min(kSBinsMax, n / 16)
+  int t_max;                     // decimated path: effective bands of more than 32 * t_max input rows use the generic kernel
+  int32_t* h_eff;                // host mirror (pinned): eff_prefix[0 .. n_templates], then one "has generic band" flag per template
+  bool mirror_ready;             // the host mirrors (h_masks, h_eff) have been waited for since the last bank setup
   int64_t launches;
   std::string cuda_err;
   TemplateMeta* h_meta;          // host staging of the bank (pinned)
@@ -86,6 +130,14 @@ inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, f
   if (e == cudaSuccess) e = launch_rowstage_dense(c, d_mid);
   return e != cudaSuccess ? e : launch_pass2_dense(c, d_mid, d_out);
 }
+// decimated path
+cudaError_t configure_pass1(int path);
+cudaError_t configure_pass2();
+cudaError_t configure_bandpower();
+cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st);      // W_l, then U+
+cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
+cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
+cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi);
 cudaError_t launch_reset_slots(Ctx* c, int first, int count);
 cudaError_t launch_compact(Ctx* c);
 

@@ -31,7 +31,31 @@ struct P1Args {
   int log_n;
   int n1;
   int batch;                  // templates in this launch
+  // decimated path (effective bands, gwmf_internal.cuh): y is indexed by slot = eff_prefix - slot_base + e
+  int eff;                    // 0: y is indexed by tb * p + l (two-pass / spill-free paths)
+  int slot_base;              // eff_prefix of the first template of the batch
+  const float2* ubuf;         // [batch][kUCap] one-sided power spectra U+ (bandpower.cu)
 };
+
+// The effective bands of a batch whose bit is set in TemplateMeta::gen_mask, as (tb << 6 | e), ascending, identical
+// in every CTA.  s_list: batch * kMaxBands ints, s_cnt: batch + 1 ints of shared memory.  Returns the list length.
+__device__ inline int build_gen_list(const TemplateMeta* meta, int batch, int* s_list, int* s_cnt) {
+  for (int t = threadIdx.x; t < batch; t += blockDim.x) s_cnt[t] = __popc(meta[t].gen_mask);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int run = 0;
+    for (int t = 0; t < batch; ++t) { const int v = s_cnt[t]; s_cnt[t] = run; run += v; }
+    s_cnt[batch] = run;
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < batch; t += blockDim.x) {
+    unsigned m = meta[t].gen_mask;
+    int o = s_cnt[t];
+    while (m) { const int e = __ffs(m) - 1; m &= m - 1; s_list[o++] = (t << 6) | e; }
+  }
+  __syncthreads();
+  return s_cnt[batch];
+}
 
 __device__ __forceinline__ float2 cis_frac(unsigned num, int log_n) {
   // e^{2 pi i num / 2^log_n}, num < 2^log_n <= 2^22: the argument 2 num / n is exact in fp32
@@ -57,7 +81,8 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 
   // work list: the wide bands of the batch (DENSE: the one dense transform); every CTA builds the same list
   int n_list = 1;
-  if constexpr (!DENSE) n_list = build_wide_list(a.meta, a.batch, a.p, s_list, s_cnt);
+  if constexpr (!DENSE)
+    n_list = a.eff ? build_gen_list(a.meta, a.batch, s_list, s_cnt) : build_wide_list(a.meta, a.batch, a.p, s_list, s_cnt);
 
   const int tid = threadIdx.x;
   const int x = tid >> 3, c = tid & 7;
@@ -68,13 +93,21 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 #pragma unroll 1
   for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
     const int tile = item % TILES, r = (item / TILES) % G;
-    const int band_index = DENSE ? 0 : s_list[item / (TILES * G)];      // tb * p + l
+    int band_index = DENSE ? 0 : s_list[item / (TILES * G)];      // tb * p + l (eff: tb << 6 | e, replaced by the slot)
     const int k2 = tile * C + c;
 
     int e_lo, e_hi, tb_q = 0;
     if constexpr (DENSE) {
       e_lo = 0;
       e_hi = 1 << a.log_n;
+    } else if (a.eff) {
+      const int tb = band_index >> 6, e = band_index & 63;
+      const TemplateMeta* m = a.meta + tb;
+      const EffBand eb = eff_band(m, e);                // only class-D bands are ever generic: src = Q, no holes
+      e_lo = eb.e_lo;
+      e_hi = eb.e_hi;
+      tb_q = tb;
+      band_index = m->eff_prefix - a.slot_base + e;
     } else {
       const int tb = band_index / a.p, l = band_index - tb * a.p;
       const TemplateMeta* m = a.meta + tb;
@@ -154,10 +187,19 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const float2* __restrict__ tw_p2,
                                                   const TemplateMeta* __restrict__ meta, int batch, int p, int log_n1,
-                                                  int n_bands_all, int use_mask) {
+                                                  int n_bands_all, int use_mask, int slot_base) {
+  // use_mask: 0 = every band, 1 = the wide bands (wide_mask), 2 = the generic effective bands (gen_mask, decimated path)
   __shared__ int s_list[kMaxBatch * kMaxBands];
   __shared__ int s_cnt[kMaxBatch + 1];
-  const int n_list = use_mask ? build_wide_list(meta, batch, p, s_list, s_cnt) : n_bands_all;
+  const int n_list = use_mask == 2 ? build_gen_list(meta, batch, s_list, s_cnt)
+                   : use_mask ? build_wide_list(meta, batch, p, s_list, s_cnt) : n_bands_all;
+  if (use_mask == 2) {                                   // (tb << 6 | e) -> slot
+    for (int i = threadIdx.x; i < n_list; i += blockDim.x) {
+      const int v = s_list[i];
+      s_list[i] = meta[v >> 6].eff_prefix - slot_base + (v & 63);
+    }
+    __syncthreads();
+  }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long total_rows = (long long)n_list << log_n1;
   for (long long row = (long long)blockIdx.x * 8 + warp; row < total_rows; row += (long long)gridDim.x * 8) {
@@ -312,32 +354,188 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Decimated path: first pass of the n-point transform of an EFFECTIVE band (gwmf_internal.cuh: Z = union of the
+// narrow bands read from Q, U = one-sided power spectrum read from ubuf, D = one wide band read from Q), any number
+// of input rows.  Same CTA shape and phases as k_pass1_narrow; what is new is the sum over the input rows that share
+// a residue b' = (k1 - row_lo) mod 32: with k1 = row_lo + b' + 32 t,
+//     sum_t X[k_t] e^{2 pi i ja k_t/n} = e^{2 pi i ja k_0/n} sum_t X[k_t] g^t,  g = e^{2 pi i ja 32 * 1024/n} = e^{2 pi i ja/NA},
+// evaluated by Horner's rule with the CTA-constant g: ceil(R/32) complex multiply-adds per (b', column), then the
+// same 32-point transform over b'.  Bands of at most 16 rows keep the pruned variants.  Bins of class-D bands that
+// lie inside the hull of Z ("holes": only with unusual spectra) are masked out.
+// ---------------------------------------------------------------------------------------------------
+struct EffSrc {
+  const float2* src;      // spectrum indexed by absolute bin k (Q of the template, or U+ of the template)
+  int e_lo, e_hi;
+  int n_holes;            // Z only
+  const int* holes;       // shared memory: [2h] = first bin of hole h, [2h+1] = one past its last bin
+};
+
+__device__ __forceinline__ bool eff_inside(const EffSrc& es, int k) {
+  if (k < es.e_lo || k >= es.e_hi) return false;
+  for (int h = 0; h < es.n_holes; ++h)
+    if (k >= es.holes[2 * h] && k < es.holes[2 * h + 1]) return false;
+  return true;
+}
+
+template <int RMAX>
+__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float2* __restrict__ T1,
+                                           float2* __restrict__ tile, float2 Aja, int R, int row_lo, int ja, int k2, int m,
+                                           int ci) {
+  float2 v[32];
+  const int n1m = a.n1 - 1;
+  if constexpr (RMAX < 32) {
+#pragma unroll
+    for (int i = 0; i < RMAX; ++i) {
+      float2 val = make_float2(0.f, 0.f);
+      const int k = ((row_lo + i) << kLogN2) + k2;
+      if (i < R && eff_inside(es, k)) {
+        const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], Aja);      // e^{2 pi i ja k/n}, k = 1024 k1 + k2
+        val = cmul(es.src[k], t);
+      }
+      v[brev<32>(i)] = val;
+    }
+  } else {
+    const int T = (R + 31) >> 5;
+    const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                        // e^{2 pi i ja/NA}
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = make_float2(0.f, 0.f);
+#pragma unroll 1
+    for (int t = T - 1; t >= 0; --t) {
+#pragma unroll
+      for (int i = 0; i < 32; ++i) {
+        const int k = ((row_lo + i + 32 * t) << kLogN2) + k2;
+        float2 val = make_float2(0.f, 0.f);
+        if (eff_inside(es, k)) val = es.src[k];
+        const float2 w = v[brev<32>(i)];
+        v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], Aja);        // e^{2 pi i ja k_0/n}, k_0 = 1024 (row_lo + i) + k2
+      v[brev<32>(i)] = cmul(v[brev<32>(i)], t);
+    }
+  }
+  fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
+  const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
+#pragma unroll
+  for (int jb = 0; jb < 32; jb += 2) {
+    const float4 w = t1[jb >> 1];
+    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], make_float2(w.x, w.y));
+    tile[(jb + 1) * kTileStride + m * 8 + ci] = cmul(v[jb + 1], make_float2(w.z, w.w));
+  }
+}
+
+__global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a) {
+  extern __shared__ __align__(128) float2 smem[];
+  float2* tile = smem;                          // [32][kStageStride] (phase 1 uses stride kTileStride)
+  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i jb m/1024}
+  __shared__ int s_holes[2 * kMaxBands];
+  __shared__ int s_nholes;
+
+  const int tid = threadIdx.x;
+  const int na = a.n1 >> 5;
+  const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
+  const int slot = blockIdx.y;
+  const unsigned nmask = (1u << a.log_n) - 1u;
+
+  // the template that owns this slot: the last tb with eff_prefix - slot_base <= slot
+  int lo = 0, hi = a.batch - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (a.meta[mid].eff_prefix - a.slot_base <= slot) lo = mid; else hi = mid - 1;
+  }
+  const int tb = lo;
+  const TemplateMeta* mt = a.meta + tb;
+  const int e = slot - (mt->eff_prefix - a.slot_base);
+  if ((mt->gen_mask >> e) & 1u) return;         // very many rows: k_pass1 (generic) + k_rowstage write this slot
+  const EffBand eb = eff_band(mt, e);
+
+  EffSrc es;
+  es.e_lo = eb.e_lo;
+  es.e_hi = eb.e_hi;
+  es.holes = s_holes;
+  es.src = eb.kind == kEffU ? a.ubuf + (size_t)tb * kUCap : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
+  if (tid == 0) {
+    int nh = 0;
+    if (eb.kind == kEffZ) {
+      unsigned d = mt->d_mask;
+      while (d) {
+        const int l = __ffs(d) - 1;
+        d &= d - 1;
+        if (mt->edges[l] >= eb.e_lo && mt->edges[l + 1] <= eb.e_hi) { s_holes[2 * nh] = mt->edges[l]; s_holes[2 * nh + 1] = mt->edges[l + 1]; ++nh; }
+      }
+    }
+    s_nholes = nh;
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) T1[(tid >> 5) * kT1Stride + 8 * i * kT1Stride + (tid & 31)] = __ldg(&a.tw_p2[tid + 256 * i]);
+  __syncthreads();
+  es.n_holes = s_nholes;
+
+  float2* out0 = a.y + ((size_t)slot * a.n1 + (size_t)ja) * kN2 + cg * 256;   // row jb adds jb * na * 1024
+  const size_t row_stride = (size_t)na * kN2;
+  const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
+  const int R = row_hi - row_lo + 1;
+  // ---- phase 1: thread (m, ci), column k2
+  {
+    const int ci = tid & 7, m = tid >> 3;
+    const int k2 = 32 * m + 8 * cg + ci;
+    const float2 Aja = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
+    if (R <= 4) eff_phase1<4>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
+    else if (R <= 8) eff_phase1<8>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
+    else if (R <= 16) eff_phase1<16>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
+    else eff_phase1<32>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
+  }
+  __syncthreads();
+  // ---- phase 2: thread (jb = lane, ci = warp)
+  {
+    const int jb = tid & 31, ci = tid >> 5;
+    const int c = 8 * cg + ci;
+    float sn, cs;
+    const unsigned num = ((unsigned)jb * (unsigned)(c + 1024 * (row_lo & 31))) & 32767u;
+    sincospif((float)num * (1.0f / 16384.0f), &sn, &cs);
+    const tw4 S = make_tw4(make_float2(cs, sn));
+    float2 x[32];
+#pragma unroll
+    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cmul_tw(tile[jb * kTileStride + m * 8 + ci], S);
+    fft_dit<32>(x);                                   // over m -> jm
+    __syncthreads();                                  // the tile has been read by everyone: reuse it as staging
+    float4* st = reinterpret_cast<float4*>(tile + jb * kStageStride + ci * 32);
+#pragma unroll
+    for (int jm = 0; jm < 32; jm += 2) st[jm >> 1] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic writes -> visible to the bulk copy engine
+  __syncthreads();
+  if (tid < 32) {
+    const unsigned src = (unsigned)__cvta_generic_to_shared(tile + tid * kStageStride);
+    float2* dst = out0 + (size_t)tid * row_stride;
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], 2048;" ::"l"(dst), "r"(src) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the copy's reads
+  }
+}
+
 constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 32 * kT1Stride) * sizeof(float2);
 
 static cudaError_t launch_narrow(Ctx* c, const P1Args& args, int batch) {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass1_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNarrowSmem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
   dim3 grid(4 * c->na, c->prm.p, batch);
   k_pass1_narrow<<<grid, 256, kNarrowSmem, c->stream>>>(args);
   c->launches++;
   return cudaGetLastError();
 }
 
-template <int NA, int NB, bool DENSE>
-static cudaError_t launch_p1(Ctx* c, const P1Args& args, cudaStream_t st) {
+template <int NA, int NB>
+constexpr size_t p1_smem() {
   constexpr int FR = NA >= 32 ? 32 : NA;
   constexpr int SROW = NB * kColsPerCta + kColsPerCta;
-  const size_t smem = (size_t)(FR * SROW + FR * kColsPerCta + NB * kColsPerCta) * sizeof(float2);
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass1<NA, NB, DENSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  return (size_t)(FR * SROW + FR * kColsPerCta + NB * kColsPerCta) * sizeof(float2);
+}
+
+template <int NA, int NB, bool DENSE>
+static cudaError_t launch_p1(Ctx* c, const P1Args& args, cudaStream_t st) {
+  const size_t smem = p1_smem<NA, NB>();
   // persistent over the work list; a CTA with nothing to do exits after building the (empty) list
   k_pass1<NA, NB, DENSE><<<2 * c->n_sms, 256, smem, st>>>(args);
   c->launches++;
@@ -362,9 +560,9 @@ static cudaError_t dispatch_p1(Ctx* c, const P1Args& args, cudaStream_t st) {
 }
 
 static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, int batch, int n_bands_all, int use_mask,
-                                   cudaStream_t st) {
+                                   cudaStream_t st, int slot_base = 0) {
   k_rowstage<<<4 * c->n_sms, 256, 0, st>>>(y, ws_ptr<float2>(c, c->lay.tw_p2), meta, batch, c->prm.p,
-                                                  c->log_n - kLogN2, n_bands_all, use_mask);
+                                                  c->log_n - kLogN2, n_bands_all, use_mask, slot_base);
   c->launches++;
   return cudaGetLastError();
 }
@@ -435,6 +633,9 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = count;
+  args.eff = 0;
+  args.slot_base = 0;
+  args.ubuf = nullptr;
   args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   args.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
   cudaError_t e;
@@ -449,9 +650,8 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   // read the band buffer) precedes the side work
   if ((e = cudaEventRecord(c->ev_fork, c->stream)) != cudaSuccess) return e;
   if ((e = cudaStreamWaitEvent(c->side, c->ev_fork, 0)) != cudaSuccess) return e;
-  // which kernels have anything to do: host mirror of the wide-band masks (written by k_bank_setup; the event
-  // has normally fired long before the first filter call)
-  if ((e = cudaEventSynchronize(c->ev_masks)) != cudaSuccess) return e;
+  // which kernels have anything to do: host mirror of the wide-band masks (written by k_bank_setup; the caller has
+  // waited for it once since the last bank setup, api.cu:ensure_mirror)
   const uint32_t full = c->prm.p >= 32 ? 0xFFFFFFFFu : ((1u << c->prm.p) - 1u);
   bool any_wide = false, any_narrow = false;
   for (int t = first; t < first + count; ++t) {
@@ -504,9 +704,76 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = 1;
+  args.eff = 0;
+  args.slot_base = 0;
+  args.ubuf = nullptr;
   return dispatch_p1<true>(c, args, c->stream);
 }
 
 cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid) { return launch_rowstage(c, d_mid, nullptr, 1, 1, 0, c->stream); }
+
+// ---- decimated path launchers ---------------------------------------------------------------------
+static void fill_eff_args(Ctx* c, P1Args& args, int first, int count, int parity) {
+  args.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
+  args.wq = ws_ptr<float2>(c, c->lay.wq);
+  args.u_tab = ws_ptr<double>(c, c->lay.u_tab);
+  args.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
+  args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
+  args.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
+  args.dense_in = nullptr;
+  args.y = ws_ptr<float2>(c, c->lay.y);
+  args.p = c->prm.p;
+  args.log_n = c->log_n;
+  args.n1 = c->n1;
+  args.batch = count;
+  args.eff = 1;
+  args.slot_base = c->h_eff[first];
+  args.ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
+}
+
+// first pass of every effective band of the batch (needs Q and U+ of the batch; host mirror h_eff valid)
+cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+  P1Args args;
+  fill_eff_args(c, args, first, count, parity);
+  const int n_slots = c->h_eff[first + count] - c->h_eff[first];
+  if (n_slots <= 0) return cudaSuccess;
+  k_pass1_eff<<<dim3(4 * c->na, n_slots), 256, kNarrowSmem, st>>>(args);
+  c->launches++;
+  return cudaGetLastError();
+}
+
+// the effective bands flagged in gen_mask: generic kernel (plain layout) + row stage, into their slots
+cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+  P1Args args;
+  fill_eff_args(c, args, first, count, parity);
+  cudaError_t e = dispatch_p1<false>(c, args, st);
+  if (e != cudaSuccess) return e;
+  return launch_rowstage(c, args.y, args.meta, count, 0, 2, st, args.slot_base);
+}
+
+template <int NA, int NB>
+static cudaError_t configure_p1_one() {
+  cudaError_t e = cudaFuncSetAttribute(k_pass1<NA, NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p1_smem<NA, NB>());
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_pass1<NA, NB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p1_smem<NA, NB>());
+  return e;
+}
+
+// Opt-in to > 48 KB of dynamic shared memory for every pass-1 kernel, on the CURRENT device (called by gwmf_create
+// for each context: the attribute is per device, not per process).
+cudaError_t configure_pass1(int /*path*/) {
+  cudaError_t e = cudaFuncSetAttribute(k_pass1_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNarrowSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass1_eff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNarrowSmem);
+  if (e == cudaSuccess) e = configure_p1_one<1, 16>();
+  if (e == cudaSuccess) e = configure_p1_one<1, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<2, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<4, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<8, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<16, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<32, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<64, 32>();
+  if (e == cudaSuccess) e = configure_p1_one<128, 32>();
+  return e;
+}
 
 }  // namespace gwmf

@@ -223,6 +223,136 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Decimated path: the same last stage and epilogue over a template's EFFECTIVE bands (gwmf_internal.cuh).  A row
+// (template, j1) owns n_eff 8 KB rows of the band buffer, at slots eff_prefix - slot_base + e:
+//     Z (e = 0): z  += x                      the narrow bands' share of z, one transform for all of them
+//     U (e = 1): q  += Re x                   sum over the narrow bands of |z_l|^2 (bandpower.cu)
+//     D (wide) : z  += x,  q += |x|^2         a wide band's own transform, as in k_pass2
+// then the same rho / chi^2 / trigger epilogue.  Warps are persistent and prefetch through the same ring of TMA
+// bulk copies, across band and row boundaries.
+// ---------------------------------------------------------------------------------------------------
+struct P2EArgs {
+  P2Args b;
+  int slot_base;              // eff_prefix of the first template of the batch
+  int batch;
+};
+
+template <bool SERIES>
+__global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
+  const P2Args& a = ea.b;
+  extern __shared__ __align__(128) float2 smem2[];
+  __shared__ int s_slot0[kMaxBatch];          // first slot of template tb (batch-relative)
+  __shared__ int s_neff[kMaxBatch];           // n_eff | has_s << 8
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float2* tw_s = smem2;                                               // [c][jm]
+  float2* bufs = smem2 + 1024 + warp * (kP2Ring * kN2);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * kP2Ring * kN2) + kP2Ring * warp;
+  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
+  for (int t = threadIdx.x; t < ea.batch; t += blockDim.x) {
+    s_slot0[t] = a.meta[t].eff_prefix - ea.slot_base;
+    s_neff[t] = a.meta[t].n_eff | (a.meta[t].s_mask ? 256 : 0);
+  }
+  __syncthreads();                                                    // the only CTA-wide barrier
+
+  const int total_warps = gridDim.x * kP2Warps;
+  const int first_row = blockIdx.x * kP2Warps + warp;
+  if (first_row >= a.n_rows) return;                                  // warps are independent: no CTA barrier below
+  const int n1_mask = a.n1 - 1;
+
+  unsigned long long policy;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+
+  // Rows are walked from the END of the band buffer: what pass 1 wrote last is still in L2.
+  const int last_row = a.n_rows - 1 - first_row;
+  int pf_item = 0, pf_e = 0, pf_row = last_row;                       // prefetch cursor (next item to request)
+  auto prefetch = [&]() {
+    // caller: lane 0 only, and only after every lane has consumed the buffer being refilled
+    const int tb = pf_row >> a.log_n1, j1 = pf_row & n1_mask;
+    const float2* src = a.y + ((size_t)(s_slot0[tb] + pf_e) * a.n1 + j1) * kN2;
+    const int b = pf_item % kP2Ring;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_expect_tx(&bars[b], kRowBytes);
+    bulk_load_row(bufs + b * kN2, src, kRowBytes, &bars[b], policy);
+  };
+  auto advance = [&]() {
+    ++pf_item;
+    if (++pf_e == (s_neff[pf_row >> a.log_n1] & 255)) { pf_e = 0; pf_row -= total_warps; }
+  };
+  if (lane == 0) {
+#pragma unroll
+    for (int b = 0; b < kP2Ring; ++b) mbar_init(&bars[b], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncwarp();
+#pragma unroll 1
+  for (int b = 0; b < kP2Ring && pf_row >= 0; ++b) {
+    if (lane == 0) prefetch();
+    advance();
+  }
+
+  float2 az[32];
+  float aq[32];
+#pragma unroll
+  for (int i = 0; i < 32; ++i) { az[i] = make_float2(0.f, 0.f); aq[i] = 0.f; }
+
+  int item = 0;
+#pragma unroll 1
+  for (int row = last_row; row >= 0; row -= total_warps) {
+    const int tb = row >> a.log_n1, j1 = row & n1_mask;
+    const int ne = s_neff[tb] & 255;
+    const bool has_s = (s_neff[tb] & 256) != 0;
+#pragma unroll 1
+    for (int e = 0; e < ne; ++e, ++item) {
+      const int b = item % kP2Ring;
+      const float2* cur = bufs + b * kN2;
+      mbar_wait(&bars[b], (item / kP2Ring) & 1);
+      float2 x[32];
+#pragma unroll
+      for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(cur[32 * c + lane], tw_s[32 * c + lane]);     // lane = jm
+      fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
+      __syncwarp();                                                         // every lane holds its 32 values
+      if (pf_row >= 0) {
+        if (lane == 0) prefetch();
+        advance();
+      }
+      if (has_s && e == 0) {                    // Z
+#pragma unroll
+        for (int jc = 0; jc < 32; ++jc) az[jc] = cadd(az[jc], x[jc]);
+      } else if (has_s && e == 1) {             // U
+#pragma unroll
+        for (int jc = 0; jc < 32; ++jc) aq[jc] += x[jc].x;
+      } else {                                  // D
+#pragma unroll
+        for (int jc = 0; jc < 32; ++jc) {
+          const float2 z = x[jc];
+          az[jc] = cadd(az[jc], z);
+          aq[jc] = fmaf(z.x, z.x, fmaf(z.y, z.y, aq[jc]));
+        }
+      }
+    }
+    // ---- epilogue of one row: rho, chi^2 and the trigger slots (steps a4, a5) ----
+    const float scale = __ldg(&a.meta[tb].scale_rho2);
+    const float fp_scale = (float)a.p * scale, inv_p = 1.0f / (float)a.p;
+    const float thr2 = a.thresh * a.thresh * 0.999f;
+    Slot* slots_t = a.slots ? a.slots + (size_t)tb * a.n_windows : nullptr;
+#pragma unroll
+    for (int jc = 0; jc < 32; ++jc) {
+      const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
+      const float rho2 = z2 * scale;                                        // Eq. 3 squared
+      const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * fp_scale;         // Eq. 5
+      const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
+      if constexpr (SERIES) {
+        if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
+        if (a.series_chi) a.series_chi[j] = chi;
+      }
+      if (rho2 > thr2 && slots_t) emit_candidate(slots_t, j, rho2, chi, a.thresh, a.log_w);
+      az[jc] = make_float2(0.f, 0.f);
+      aq[jc] = 0.f;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Spill-free path (the library's choice for n <= 2^20; gwmf_uses_fused): narrow bands never reach HBM.  A CTA
 // owns 8 consecutive rows j1 of one template (one per warp) and walks the p bands.  For a narrow band (<= 32
 // input rows) the row of Y is formed directly from the correlated spectrum,
@@ -417,13 +547,6 @@ constexpr size_t kFusedSmem = (size_t)(1024 + 2 * kFRows * 1024 + 8 * kFTile + 8
                               10 * sizeof(unsigned long long) + 80 * sizeof(int);
 
 cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool update_slots, float* series_rho, float* series_chi) {
-  static bool done = false;
-  if (!done) {
-    cudaError_t e = cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
-    if (e != cudaSuccess) return e;
-    done = true;
-  }
   FArgs fa;
   P2Args& a = fa.b;
   a.y = ws_ptr<float2>(c, c->lay.y);
@@ -456,13 +579,15 @@ cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool u
 
 constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
 
-static cudaError_t p2_configure() {
-  static bool done = false;
-  if (done) return cudaSuccess;
+// Opt-in to > 48 KB of dynamic shared memory on the CURRENT device (gwmf_create calls this for every context).
+cudaError_t configure_pass2() {
   cudaError_t e = cudaFuncSetAttribute(k_pass2<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  done = (e == cudaSuccess);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
   return e;
 }
 
@@ -489,8 +614,6 @@ cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots,
   a.n_windows = c->n_windows;
   a.n_rows = count * c->n1;
   a.thresh = (float)c->prm.rho_thresh;
-  cudaError_t e = p2_configure();
-  if (e != cudaSuccess) return e;
   if (series_rho || series_chi) k_pass2<false, true><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
   else k_pass2<false, false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
   c->launches++;
@@ -513,9 +636,34 @@ cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
   a.n_windows = 0;
   a.n_rows = c->n1;
   a.thresh = 0.f;
-  cudaError_t e = p2_configure();
-  if (e != cudaSuccess) return e;
   k_pass2<true, false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  c->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi) {
+  P2EArgs ea;
+  P2Args& a = ea.b;
+  a.y = ws_ptr<float2>(c, c->lay.y);
+  a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
+  a.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
+  a.slots = update_slots ? ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows : nullptr;
+  a.series_rho = series_rho;
+  a.series_chi = series_chi;
+  a.dense_out = nullptr;
+  a.p = c->prm.p;
+  a.n1 = c->n1;
+  a.log_n1 = c->log_n - kLogN2;
+  int lw = 0;
+  while ((1 << lw) < c->prm.window) ++lw;
+  a.log_w = lw;
+  a.n_windows = c->n_windows;
+  a.n_rows = count * c->n1;
+  a.thresh = (float)c->prm.rho_thresh;
+  ea.slot_base = c->h_eff[first];
+  ea.batch = count;
+  if (series_rho || series_chi) k_pass2_eff<true><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(ea);
+  else k_pass2_eff<false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(ea);
   c->launches++;
   return cudaGetLastError();
 }

@@ -9,10 +9,16 @@ namespace gwmf {
 //   u_tab[k]  = f_k^(-1/3) (fp64), k = 0 .. n/2-1 (u_tab[0] = 0)
 //   tw_n1[m]  = e^{2 pi i m / n1}, m = 0 .. n1-1        (pass-1 inter-stage twiddles)
 //   tw_p2[jm][c] = e^{2 pi i jm c / 1024}, 32 x 32      (pass-2 inter-stage twiddles)
+//   tw_l[t]   = e^{2 pi i t / 16384}                    (coarse-grid transforms of the decimated path)
 // ---------------------------------------------------------------------------------------------------
 __global__ void k_tables(double* __restrict__ u_tab, float2* __restrict__ tw_n1, float2* __restrict__ tw_p2,
-                         int half_n, int n1, double df) {
+                         float2* __restrict__ tw_l, int half_n, int n1, double df) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < kLMax) {                      // tw_l[t] = e^{2 pi i t / kLMax}: coarse-grid transforms of bandpower.cu
+    double s, c;
+    sincospi(2.0 * (double)i / (double)kLMax, &s, &c);
+    tw_l[i] = make_float2((float)c, (float)s);
+  }
   if (i < half_n) u_tab[i] = (i == 0) ? 0.0 : rcbrt((double)i * df);
   if (i < n1) {
     double s, c;
@@ -29,10 +35,11 @@ __global__ void k_tables(double* __restrict__ u_tab, float2* __restrict__ tw_n1,
 
 cudaError_t launch_tables(Ctx* c) {
   int half = (int)(c->n / 2);
-  int work = half > 1024 ? half : 1024;
+  int work = half > kLMax ? half : kLMax;
   k_tables<<<(work + 255) / 256, 256, 0, c->stream>>>(ws_ptr<double>(c, c->lay.u_tab),
                                                       ws_ptr<float2>(c, c->lay.tw_n1),
-                                                      ws_ptr<float2>(c, c->lay.tw_p2), half, c->n1, c->df);
+                                                      ws_ptr<float2>(c, c->lay.tw_p2), ws_ptr<float2>(c, c->lay.tw_l), half,
+                                                      c->n1, c->df);
   c->launches++;
   return cudaGetLastError();
 }
@@ -165,7 +172,7 @@ cudaError_t launch_segment_prepare(Ctx* c) {
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ meta, uint32_t* __restrict__ masks,
                                                     const double* __restrict__ c_tab, int n_templates, int p, int k_low,
-                                                    int half_n, double four_df, int all_wide) {
+                                                    int half_n, double four_df, int all_wide, int s_bins, int t_max) {
   // thread (l = threadIdx.x, template = 8 blockIdx.x + threadIdx.y): one band edge each, then the wide-band mask
   __shared__ int s_edges[8][kMaxBands + 1];
   const int l = threadIdx.x, ty = threadIdx.y;
@@ -212,6 +219,31 @@ __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ m
   meta[t].row_off[l + 1] = (uint16_t)incl;
   if (l == 0) { meta[t].row_off[0] = 0; meta[t].row_off[kMaxBands + 1] = 0; }
   meta[t].edges[l] = s_edges[ty][l];
+  // ---- decimated path: classes and effective bands (gwmf_internal.cuh).  s_bins == 0 switches it off.
+  {
+    int bins = 0, e_lo = 0, e_hi = 0;
+    if (l < p) { e_lo = s_edges[ty][l]; e_hi = s_edges[ty][l + 1]; bins = e_hi - e_lo; }
+    const bool is_s = s_bins > 0 && bins > 0 && bins <= s_bins;
+    const bool is_d = bins > 0 && !is_s;
+    const unsigned s_mask = __ballot_sync(0xFFFFFFFFu, is_s), d_mask = __ballot_sync(0xFFFFFFFFu, is_d);
+    const int z_lo = __reduce_min_sync(0xFFFFFFFFu, is_s ? e_lo : 0x7FFFFFFF);
+    const int z_hi = __reduce_max_sync(0xFFFFFFFFu, is_s ? e_hi : 0);
+    const int u_hi = __reduce_max_sync(0xFFFFFFFFu, is_s ? bins : 0);
+    const int base = s_mask ? 2 : 0;
+    // generic kernel for class-D bands of more than 32 t_max input rows (the Horner sum of k_pass1_eff would be long)
+    unsigned gen = 0u;
+    if (is_d && rows > 32 * t_max) gen = 1u << (base + __popc(d_mask & ((1u << l) - 1u)));
+    gen = __reduce_or_sync(0xFFFFFFFFu, gen);
+    if (l == 0) {
+      meta[t].s_mask = s_mask;
+      meta[t].d_mask = d_mask;
+      meta[t].gen_mask = gen;
+      meta[t].n_eff = base + __popc(d_mask);
+      meta[t].z_lo = s_mask ? z_lo : 0;
+      meta[t].z_hi = z_hi;
+      meta[t].u_hi = u_hi;
+    }
+  }
   if (l == 0) {
     meta[t].edges[kMaxBands] = k_high;
     meta[t].sigma = sqrt(four_df * total);
@@ -221,13 +253,49 @@ __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ m
   }
 }
 
+// eff_prefix[t] = sum_{t' < t} n_eff[t'] (exclusive), total in eff_out[n_templates]; eff_out[n_templates + 1 + t] = 1 if
+// template t has a generic effective band.  One block; sequential over chunks, fixed order.
+__global__ void __launch_bounds__(1024) k_eff_scan(TemplateMeta* __restrict__ meta, int32_t* __restrict__ eff_out, int n_templates) {
+  __shared__ int part[1024];
+  const int t = threadIdx.x;
+  const int L = (n_templates + 1023) / 1024;
+  const int lo = min(t * L, n_templates), hi = min(lo + L, n_templates);
+  int acc = 0;
+  for (int i = lo; i < hi; ++i) acc += meta[i].n_eff;
+  part[t] = acc;
+  __syncthreads();
+  if (t == 0) {
+    int run = 0;
+    for (int i = 0; i < 1024; ++i) { const int v = part[i]; part[i] = run; run += v; }
+    eff_out[n_templates] = run;
+  }
+  __syncthreads();
+  acc = part[t];
+  for (int i = lo; i < hi; ++i) {
+    meta[i].eff_prefix = acc;
+    eff_out[i] = acc;
+    eff_out[n_templates + 1 + i] = meta[i].gen_mask ? 1 : 0;
+    acc += meta[i].n_eff;
+  }
+}
+
 cudaError_t launch_bank_setup(Ctx* c) {
+  const bool decim = c->path == GWMF_PATH_DECIMATED;
   k_bank_setup<<<(c->n_templates + 7) / 8, dim3(32, 8), 0, c->stream>>>(
       ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<uint32_t>(c, c->lay.masks), ws_ptr<double>(c, c->lay.c_tab),
-      c->n_templates, c->prm.p, c->k_low, (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1);
+      c->n_templates, c->prm.p, c->k_low, (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1, decim ? c->s_bins : 0, c->t_max);
   c->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  c->mirror_ready = false;
+  if (decim) {
+    int32_t* d_eff = ws_ptr<int32_t>(c, c->lay.eff);
+    k_eff_scan<<<1, 1024, 0, c->stream>>>(ws_ptr<TemplateMeta>(c, c->lay.meta), d_eff, c->n_templates);
+    c->launches++;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    e = cudaMemcpyAsync(c->h_eff, d_eff, sizeof(int32_t) * (size_t)(2 * c->n_templates + 1), cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return e;
+  }
   // host mirror of the wide-band masks: lets gwmf_filter skip kernels that would find nothing to do
   e = cudaMemcpyAsync(c->h_masks, ws_ptr<uint32_t>(c, c->lay.masks), sizeof(uint32_t) * (size_t)c->n_templates,
                       cudaMemcpyDeviceToHost, c->stream);

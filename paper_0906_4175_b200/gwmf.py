@@ -16,19 +16,21 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgwmf.so")
 
 OK, E_ARG, E_EMPTY_TEMPLATE, E_STATE, E_CAPACITY, E_CUDA, E_WORKSPACE = 0, -1, -2, -3, -4, -5, -6
+PATHS = {"auto": 0, "two_pass": 1, "fused": 2, "decimated": 3}          # gwmf_path
+PATH_NAMES = {v: k for k, v in PATHS.items()}
 
 EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
     "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_series", "gwmf_correlate",
     "gwmf_fft_inverse",
-    "gwmf_uses_fused", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
+    "gwmf_uses_fused", "gwmf_path_in_use", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
 
 
 class Params(C.Structure):
     _fields_ = [("n", C.c_int64), ("fs", C.c_double), ("f_low", C.c_double), ("p", C.c_int32),
                 ("rho_thresh", C.c_double), ("window", C.c_int32), ("max_templates", C.c_int32),
-                ("batch", C.c_int32)]
+                ("batch", C.c_int32), ("path", C.c_int32)]
 
 
 class MassPair(C.Structure):
@@ -71,6 +73,7 @@ def load_library():
     L.gwmf_correlate.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     L.gwmf_fft_inverse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.gwmf_uses_fused.argtypes = [C.c_void_p]
+    L.gwmf_path_in_use.argtypes = [C.c_void_p]
     L.gwmf_launch_count.argtypes = [C.c_void_p]
     L.gwmf_launch_count.restype = C.c_int64
     L.gwmf_destroy.argtypes = [C.c_void_p]
@@ -83,8 +86,9 @@ def load_library():
     return L
 
 
-def workspace_bytes(n, p, window, max_templates, fs=4096.0, f_low=40.0, rho_thresh=6.0, batch=0) -> int:
-    prm = Params(int(n), float(fs), float(f_low), int(p), float(rho_thresh), int(window), int(max_templates), int(batch))
+def workspace_bytes(n, p, window, max_templates, fs=4096.0, f_low=40.0, rho_thresh=6.0, batch=0, path="auto") -> int:
+    prm = Params(int(n), float(fs), float(f_low), int(p), float(rho_thresh), int(window), int(max_templates), int(batch),
+                 PATHS[path])
     return int(load_library().gwmf_workspace_bytes(C.byref(prm)))
 
 
@@ -92,7 +96,7 @@ class Filter:
     """One gwmf context: a device workspace, a stream, a bank and the current segment."""
 
     def __init__(self, n, p, window, max_templates, rho_thresh=6.0, fs=4096.0, f_low=40.0, batch=0,
-                 device="cuda:0", stream=None):
+                 device="cuda:0", stream=None, path="auto"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("gwmf needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -101,7 +105,7 @@ class Filter:
         self.device = torch.device(device)
         self.n, self.p, self.window = int(n), int(p), int(window)
         self.params = Params(int(n), float(fs), float(f_low), int(p), float(rho_thresh), int(window),
-                             int(max_templates), int(batch))
+                             int(max_templates), int(batch), PATHS[path])
         nbytes = int(self._L.gwmf_workspace_bytes(C.byref(self.params)))
         if nbytes == 0:
             raise GwmfError(E_ARG, "invalid parameters")
@@ -151,6 +155,11 @@ class Filter:
     def uses_fused(self) -> bool:
         return bool(self._L.gwmf_uses_fused(self._h))
 
+    @property
+    def path(self) -> str:
+        """The path the library resolved at create: two_pass, fused or decimated."""
+        return PATH_NAMES[int(self._L.gwmf_path_in_use(self._h))]
+
     def make_bank(self, masses):
         arr = (MassPair * len(masses))(*[MassPair(float(a), float(b)) for a, b in masses])
         self._check(self._L.gwmf_make_bank(self._h, arr, len(masses)))
@@ -183,13 +192,13 @@ class Filter:
         self._check(self._L.gwmf_filter(self._h, int(first), int(count)))
 
     def filter_timed(self, first=0, count=None):
-        """As filter(), returning ((ms_pass1, ms_pass2), (launches_pass1, launches_pass2)); syncs."""
+        """As filter(), returning ((ms_spectra, ms_pass1, ms_pass2), (batches timed in each)); syncs."""
         if count is None:
             count = self.n_templates - first
-        ms = (C.c_double * 2)()
-        nl = (C.c_int32 * 2)()
+        ms = (C.c_double * 3)()
+        nl = (C.c_int32 * 3)()
         self._check(self._L.gwmf_filter_timed(self._h, int(first), int(count), ms, nl))
-        return (ms[0], ms[1]), (nl[0], nl[1])
+        return (ms[0], ms[1], ms[2]), (nl[0], nl[1], nl[2])
 
     def triggers(self, capacity=None) -> np.ndarray:
         if capacity is None:

@@ -22,26 +22,25 @@ def gw():
     return gwmf
 
 
-@pytest.fixture(params=["auto", "two_pass", "fused"])
+@pytest.fixture(params=["decimated", "two_pass", "fused"])
 def path(request):
-    """Forces the library's path for one test: auto = its own choice (spill-free kernel for 2^15 <= n <= 2^20,
-    two-pass otherwise); the environment variable is read by gwmf_create."""
-    old = os.environ.get("GWMF_FUSED")
-    if request.param == "auto":
-        os.environ.pop("GWMF_FUSED", None)
-    else:
-        os.environ["GWMF_FUSED"] = "1" if request.param == "fused" else "0"
-    yield request.param
-    if old is None:
-        os.environ.pop("GWMF_FUSED", None)
-    else:
-        os.environ["GWMF_FUSED"] = old
+    """The library's three paths (gwmf_params::path), each checked against the oracle."""
+    return request.param
 
 
-def _run_gpu(gw, w, s, Sn, masses=None, batch=0, window=None, thresh=None, p=None):
+def _path_for(path, n):
+    """A path the library supports at this n (fused: 2^15..2^20, decimated: >= 2^15), else auto."""
+    if path == "fused" and not (1 << 15) <= n <= (1 << 20):
+        return "auto"
+    if path == "decimated" and n < (1 << 15):
+        return "auto"
+    return path
+
+
+def _run_gpu(gw, w, s, Sn, masses=None, batch=0, window=None, thresh=None, p=None, path="auto"):
     masses = w.masses if masses is None else masses
     f = gw.Filter(w.n, p or w.p, window or w.window, len(masses), rho_thresh=w.rho_thresh if thresh is None else thresh,
-                  batch=batch)
+                  batch=batch, path=_path_for(path, w.n))
     f.make_bank(masses)
     f.load_segment(s.astype(np.float32), Sn)
     f.filter()
@@ -113,7 +112,7 @@ def test_config0_full(gw, path):
     w = inputs.workload(0)
     s = inputs.segment(w)
     Sn = w.psd
-    f = _run_gpu(gw, w, s, Sn)
+    f = _run_gpu(gw, w, s, Sn, path=path)
     out = oracle.filter_bank(s.astype(np.float32).astype(np.float64), Sn, w.masses, w.p, w.window, w.rho_thresh)
     parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
     s32 = s.astype(np.float32).astype(np.float64)
@@ -153,7 +152,7 @@ def test_midsize_full_series(gw, path, log_n, p, window, batch):
     s = inputs.time_series(D, n).astype(np.float32)
     Sn = inputs.psd_array(n)
     w = inputs.Workload(config=-1, n=n, p=p, rho_thresh=5.0, window=window, masses=masses, seed=0)
-    f = _run_gpu(gw, w, s, Sn, batch=batch)
+    f = _run_gpu(gw, w, s, Sn, batch=batch, path=path)
     out = oracle.filter_bank(s.astype(np.float64), Sn, masses, p, window, 5.0)
     parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
     for t, (m1, m2) in enumerate(masses):
@@ -165,11 +164,11 @@ def test_midsize_full_series(gw, path, log_n, p, window, batch):
 
 
 # ----------------------------------------------------------------------------- configs 1, 2, 4: sampled templates
-def _sampled_config(gw, config, sample_ids, n_templates=None):
+def _sampled_config(gw, config, sample_ids, n_templates=None, path="auto"):
     w = inputs.workload(config, n_templates)
     s = inputs.segment(w).astype(np.float32)
     Sn = w.psd
-    f = _run_gpu(gw, w, s, Sn)
+    f = _run_gpu(gw, w, s, Sn, path=path)
     trig = f.triggers()
     sub = [w.masses[i] for i in sample_ids]
     s64 = s.astype(np.float64)
@@ -189,7 +188,7 @@ def test_config1_all_templates(gw, path):
     w = inputs.workload(1)
     s = inputs.segment(w).astype(np.float32)
     Sn = w.psd
-    f = _run_gpu(gw, w, s, Sn)
+    f = _run_gpu(gw, w, s, Sn, path=path)
     out = oracle.filter_bank(s.astype(np.float64), Sn, w.masses, w.p, w.window, w.rho_thresh)
     parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
     compared, exempt = parity.assert_triggers(f.triggers(), out, w.rho_thresh, w.window, w.p)
@@ -200,34 +199,22 @@ def test_config1_all_templates(gw, path):
         parity.assert_series(rho_g, chi_g, rho_o, chi_o, w.p, f"config 1 template {t}")
 
 
-@pytest.mark.parametrize("forced", ["0", "1"])
-def test_config2_headline_sampled(gw, forced):
-    old = os.environ.get("GWMF_FUSED")
-    os.environ["GWMF_FUSED"] = forced
-    try:
-        _config2_headline_sampled(gw)
-    finally:
-        if old is None:
-            os.environ.pop("GWMF_FUSED", None)
-        else:
-            os.environ["GWMF_FUSED"] = old
-
-
-def _config2_headline_sampled(gw):
+def test_config2_headline_sampled(gw, path):
     w0 = inputs.workload(2)
     inj = sorted({b for (b, *_rest) in w0.injections})[:6]
     ids = sorted(set(inj + [0, 31, 500, 1023]))
-    w, trig, compared = _sampled_config(gw, 2, ids)
+    w, trig, compared = _sampled_config(gw, 2, ids, path=path)
     assert compared >= len(inj)
     # order-of-magnitude check on noise exceedances: exp(-18) * N * T ~ 16 samples
     assert len(trig) < 2000
 
 
-def test_config4_long_segment_sampled(gw):
+@pytest.mark.parametrize("path4", ["decimated", "two_pass"])
+def test_config4_long_segment_sampled(gw, path4):
     w0 = inputs.workload(4)
     inj = sorted({b for (b, *_rest) in w0.injections})[:2]
     ids = sorted(set(inj + [0, 511]))
-    _sampled_config(gw, 4, ids)
+    _sampled_config(gw, 4, ids, path=path4)
 
 
 def test_noise_statistics_at_full_size(gw):
@@ -311,7 +298,7 @@ def test_p_extremes_and_covariance(gw, path):
     Sn = inputs.psd_array(n)
     for p in (1, 2, 32):
         w = inputs.Workload(config=-1, n=n, p=p, rho_thresh=5.5, window=n, masses=masses, seed=0)
-        f = _run_gpu(gw, w, s, Sn)
+        f = _run_gpu(gw, w, s, Sn, path=path)
         for t, (m1, m2) in enumerate(masses):
             rho_o, chi_o, _, _ = oracle.filter_template(s.astype(np.float64), Sn, m1, m2, p)
             rho_g, chi_g = f.series(t)
@@ -320,10 +307,10 @@ def test_p_extremes_and_covariance(gw, path):
                 assert np.all(chi_g == 0.0)
     # (S_n, s) -> (c S_n, sqrt(c) s) leaves rho and chi^2 unchanged (P8), also at physical scales
     w = inputs.Workload(config=-1, n=n, p=8, rho_thresh=5.5, window=4096, masses=masses, seed=0)
-    f1 = _run_gpu(gw, w, s, Sn)
+    f1 = _run_gpu(gw, w, s, Sn, path=path)
     r1, c1 = f1.series(0)
     c = 9e-46
-    f2 = _run_gpu(gw, w, (s.astype(np.float64) * math.sqrt(c)), Sn * c)
+    f2 = _run_gpu(gw, w, (s.astype(np.float64) * math.sqrt(c)), Sn * c, path=path)
     r2, c2 = f2.series(0)
     assert np.max(np.abs(r1 - r2)) < 2e-4 and np.max(np.abs(c1 - c2) / np.maximum(c1, 1)) < 1e-3
     assert f2.sigma()[0] == pytest.approx(f1.sigma()[0] / math.sqrt(c), rel=1e-12)
@@ -339,7 +326,7 @@ def test_empty_bands_and_few_bins(gw, path):
         s = s.astype(np.float32)
         Sn = inputs.psd_array(n)
         w = inputs.Workload(config=-1, n=n, p=32, rho_thresh=4.0, window=2048, masses=masses, seed=0)
-        f = _run_gpu(gw, w, s, Sn)
+        f = _run_gpu(gw, w, s, Sn, path=path)
         out = oracle.filter_bank(s.astype(np.float64), Sn, masses, 32, 2048, 4.0)
         parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
         e = np.asarray(out["edges"])
@@ -354,7 +341,7 @@ def test_empty_bands_and_few_bins(gw, path):
 def test_determinism_and_refilter(gw, path):
     w = inputs.workload(0)
     s = inputs.segment(w)
-    f = _run_gpu(gw, w, s, w.psd)
+    f = _run_gpu(gw, w, s, w.psd, path=path)
     a = f.triggers().copy()
     r1, c1 = f.series(4)
     f.filter()                      # slots are reset, not accumulated
@@ -374,9 +361,9 @@ def test_batching_invariance(gw, path):
     s = inputs.time_series(inputs.noise_spectrum(n, 5) + inputs.injection_spectrum(n, *masses[11], 10.0, 4242), n).astype(np.float32)
     Sn = inputs.psd_array(n)
     w = inputs.Workload(config=-1, n=n, p=16, rho_thresh=5.0, window=4096, masses=masses, seed=0)
-    ref = _run_gpu(gw, w, s, Sn, batch=37).triggers().tobytes()
+    ref = _run_gpu(gw, w, s, Sn, batch=37, path=path).triggers().tobytes()
     for batch in (1, 5, 8, 36):
-        f = _run_gpu(gw, w, s, Sn, batch=batch)
+        f = _run_gpu(gw, w, s, Sn, batch=batch, path=path)
         assert f.triggers().tobytes() == ref, f"batch {batch}"
     f.filter(3, 20)                 # partial re-filter in ragged batches keeps the other templates' events
     f.filter(30, 7)
