@@ -39,13 +39,20 @@ import workloads as inputs  # noqa: E402
 METRIC = "template-segments/sec at N=2^20, p=16 (SNR+chi^2)"
 UNIT = "template-segments/s"
 
-# --workload: the default is the headline config; the others are the "next" rows of SURVEY.md 8(f), measured
-# with the same protocol (their lines are context, not the contract's metric).
+# --workload: the default is the headline config (BASELINE.json:configs[2], the one `metric` is quoted on); the
+# others are the remaining configs and the "next" rows of SURVEY.md 8(f), measured with the same protocol (their
+# lines are records for DESIGN.md, not the contract's metric).
 WORKLOADS = {
     "headline": dict(config=2, p=None, templates=None, metric=METRIC,
                      text="BASELINE.json:configs[2]: N=2^20 (256 s at 4096 Hz), 1024 templates (total mass 2-34 Msun, "
                           "grid uniform in eta and chirp mass), p=16, threshold 6, window 4096; Eq. 2 coloured Gaussian "
                           "noise + 10 injections, seed 2 (+rank)"),
+    "config1": dict(config=1, p=None, templates=None, metric="template-segments/sec at N=2^18, p=16 (SNR+chi^2)",
+                    text="BASELINE.json:configs[1]: N=2^18 (64 s), 256 templates on a grid of m1,m2 in [1,3] Msun, p=16, "
+                         "threshold 6, window 4096, 3 injections, seed 1"),
+    "config4": dict(config=4, p=None, templates=None, metric="template-segments/sec at N=2^22, p=32 (SNR+chi^2)",
+                    text="BASELINE.json:configs[4]: N=2^22 (1024 s), 512 templates with m1,m2 in [1,2] Msun, p=32, "
+                         "threshold 5.5, window 4096, 4 injections, seed 4"),
     "snr_only": dict(config=2, p=1, templates=None, metric="template-segments/sec at N=2^20, p=1 (SNR only, PAPER.md:164)",
                      text="SURVEY.md 8(f)-2: configs[2]'s segment and bank with p=1 (one inverse FFT per template, no chi^2)"),
     "long16": dict(config=4, p=16, templates=None, metric="template-segments/sec at N=2^22, p=16 (SNR+chi^2)",
@@ -60,6 +67,8 @@ def load_workload(name):
     if spec["p"] is not None:
         w.p = spec["p"]
     return w, spec
+
+
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback, only if MEASURED_PEAKS.json is absent
 
 
@@ -207,6 +216,51 @@ def run_reference(args):
     return 0
 
 
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start N ranks (one per GPU) with torchrun and relay rank 0's line."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+STAGES = ("spectra", "pass1", "pass2")
+STAGE_TEXT = {
+    "decimated": {
+        "spectra": "k_correlate + k_bandpower + k_uspec (template phasors x data, coarse-grid band powers, U+); timed "
+                   "serialised, run beside pass 1 on a side stream in gwmf_filter",
+        "pass1": "k_pass1_eff (first FFT pass of every effective band: writes n complex fp32 per n-point transform) "
+                 "[+ generic kernel + row stage for bands of > 512 input rows]",
+        "pass2": "k_pass2_eff (last FFT stage + rho/chi^2/trigger epilogue: reads n complex fp32 per n-point transform)"},
+    "two_pass": {
+        "spectra": "-",
+        "pass1": "k_pass1_narrow (pruned column FFT + first row stage, writes p*N*8 B/template) with the low-volume kernels "
+                 "(k_correlate, k_pass1 generic, k_rowstage) beside it on the side stream; timed fork to join",
+        "pass2": "k_pass2 (last FFT stage + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"},
+    "fused": {
+        "spectra": "-",
+        "pass1": "wide bands only: k_pass1 generic + k_rowstage (side stream; the next batch's correlates run beside k_fused)",
+        "pass2": "k_fused (spill-free: narrow bands formed from the correlated spectrum, both row-transform stages, "
+                 "rho/chi^2/trigger epilogue; no band intermediate in HBM)"},
+}
+
+
+def traffic_record(path, workload, stage):
+    """ncu's dram__bytes_read.sum + dram__bytes_write.sum per template for a stage's kernel, from the committed
+    capture summary profiles/traffic.json (written from the `ncu --set full` reports named inside it)."""
+    fn = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(fn) as fh:
+            rec = json.load(fh)
+        ent = rec["entries"]["%s/%s/%s" % (workload, path, stage)]
+        return float(ent["dram_bytes_per_template"]), "profiles/traffic.json: " + ent["source"]
+    except Exception:
+        return None, None
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -215,6 +269,7 @@ def run_gpu(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node {args.gpus}"
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -234,10 +289,8 @@ def run_gpu(args):
     Sn = w.psd
     T = len(w.masses)
 
-    if args.path != "auto":
-        os.environ["GWMF_FUSED"] = "1" if args.path == "fused" else "0"
-    f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}")
-    fused = f.uses_fused
+    f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}", path=args.path, batch=args.batch)
+    path = f.path
     f.make_bank(w.masses)
     s_dev = torch.from_numpy(s32).to(dev)
     sn_dev = torch.from_numpy(Sn).to(dev)
@@ -263,27 +316,19 @@ def run_gpu(args):
     ms = reduce_max_ms(e0.elapsed_time(e1), dist if world > 1 else None, dev)
     value = world * count * args.steps / (ms * 1e-3)
 
-    # per-kernel device times (events inside the library, on its stream)
+    # per-stage device times (events inside the library, on its stream, stages serialised)
     reps = 3
-    k_ms = np.zeros(2)
-    k_launch = np.zeros(2)
+    k_ms = np.zeros(3)
+    k_launch = np.zeros(3)
     for _ in range(reps):
-        (m1, m2), (n1_, n2_) = f.filter_timed(first, count)
-        k_ms += (m1, m2)
-        k_launch += (n1_, n2_)
-    batch_templates = count / (k_launch / reps)             # templates per launch
-    bytes_per_launch = batch_templates * w.p * w.n * 8.0    # pass 1 writes / pass 2 reads p*N complex fp32 per template
-    avg_ms = k_ms / k_launch
-    gbs = bytes_per_launch / (avg_ms * 1e-3) / 1e9
+        m3, n3 = f.filter_timed(first, count)
+        k_ms += m3
+        k_launch += n3
+    k_ms /= reps                                            # ms per step and stage
+    k_launch /= reps
+    transforms = f.transform_counts()[first:first + count]  # n-point transforms per template
+    bytes_step = float(transforms.sum()) * w.n * 8.0        # pass 1 writes / pass 2 reads n complex fp32 per transform
     peak, peak_src = measured_peak()
-    dom = int(np.argmax(k_ms))
-    names = ["pass 1: k_pass1_narrow (pruned column FFT + first row stage, writes p*N*8 B/template) with the "
-             "low-volume kernels (k_correlate, k_pass1 generic, k_rowstage) beside it on the side stream; timed fork to join",
-             "pass 2: k_pass2 (last FFT stage + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"]
-    if fused:
-        names = ["wide bands only: k_pass1 generic + k_rowstage (side stream; the next batch's correlates run beside k_fused)",
-                 "k_fused (spill-free: narrow bands formed from the correlated spectrum, both row-transform stages, "
-                 "rho/chi^2/trigger epilogue; no band intermediate in HBM)"]
 
     # end to end through the C ABI with host buffers
     s_pin = torch.from_numpy(s32).pin_memory()
@@ -311,52 +356,61 @@ def run_gpu(args):
 
     if rank == 0:
         line = base_line(args, w, value, ms / args.steps, "f32")
-        line["config"]["l2"] = ("no flush: every launch streams a band intermediate of batch*p*N*8 B = %.2f GiB, "
-                                "%.0fx the 126 MB L2, through pass 1 (write) and pass 2 (read)"
-                                % (bytes_per_launch[0] / 2**30, bytes_per_launch[0] / 126e6))
-        line["config"]["batch_templates_per_launch"] = float(batch_templates[0])
+        line["config"]["path"] = path
+        line["config"]["batch_templates_per_launch"] = float(count / max(k_launch[2], 1))
+        line["config"]["n_point_transforms_per_template"] = float(transforms.mean())
+        line["config"]["l2"] = ("no flush: every step streams the band intermediate (%.2f GB written by pass 1 and read by "
+                                "pass 2 per step, %.0fx the 126 MB L2); the correlated spectra (%.0f MiB per launch) are "
+                                "produced and consumed through L2 by design"
+                                % (bytes_step / 1e9, bytes_step / 126e6, count / max(k_launch[2], 1) * w.n * 4 / 2**20))
         line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(s32.nbytes + Sn.nbytes),
                        "d2h_bytes_per_step": int(12 + trig.nbytes), "ms_per_step": ms_e2e / args.steps}
         line["gpu_launches"] = int(launches)
         line["clocks"] = clocks
         line["triggers_per_step"] = int(len(trig))
-        line["config"]["path"] = "spill-free (k_fused)" if fused else "two-pass (k_pass1_narrow + k_pass2)"
-        if fused:
-            line["config"]["l2"] = ("no flush: no band intermediate; per launch the kernel reads the batch's correlated "
-                                    "spectra (%.0f MiB, produced by the previous launch's side stream) out of L2"
-                                    % (batch_templates[1] * w.n * 4 / 2**20))
-        line["roofline"] = {
-            "bound": "hbm", "kernel": names[dom], "achieved": float(gbs[dom]), "peak": peak, "unit": "GB/s",
-            "frac": float(gbs[dom] / peak), "peak_source": peak_src, "traffic": (TRAFFIC_BYTES_PER_TEMPLATE[dom] * float(batch_templates[dom])
-                                                                  if args.workload == "headline" else None),
-            "bytes_per_launch": float(bytes_per_launch[dom]), "avg_launch_ms": float(avg_ms[dom]),
-            "kernels": {"k_pass1": {"avg_launch_ms": float(avg_ms[0]), "GB/s": float(gbs[0]), "frac": float(gbs[0] / peak),
-                                    "share_of_step": float(k_ms[0] / k_ms.sum())},
-                        "k_pass2": {"avg_launch_ms": float(avg_ms[1]), "GB/s": float(gbs[1]), "frac": float(gbs[1] / peak),
-                                    "share_of_step": float(k_ms[1] / k_ms.sum())}},
-            "path": {"bytes_per_unit": 16.0 * w.p * w.n, "achieved": 16.0 * w.p * w.n * value / world / 1e9,
+        kernels = {}
+        for i, st in enumerate(STAGES):
+            if k_launch[i] == 0:
+                continue
+            ent = {"kernel": STAGE_TEXT[path][st], "ms_per_step": float(k_ms[i]), "avg_launch_ms": float(k_ms[i] / k_launch[i]),
+                   "share_of_step": float(k_ms[i] / k_ms.sum())}
+            if st != "spectra" and path != "fused":
+                ent["GB/s"] = bytes_step / (k_ms[i] * 1e-3) / 1e9
+                ent["frac"] = ent["GB/s"] / peak
+            kernels[st] = ent
+        hbm_model = {"bytes_per_unit": 16.0 * w.p * w.n, "achieved": 16.0 * w.p * w.n * value / world / 1e9,
                      "frac": 16.0 * w.p * w.n * value / world / 1e9 / peak,
-                     "note": "whole step (both passes + epilogue) against the 16*p*N B/template two-pass model; "
-                             "frac vs nominal 8 TB/s = %.3f" % (16.0 * w.p * w.n * value / world / 8e12)},
-        }
-        if fused:
+                     "note": "for comparison only: SURVEY.md 8(d3)'s two-pass model (16*p*N B per template-segment) at this "
+                             "throughput; frac vs nominal 8 TB/s = %.3f.  The path that ran does not move these bytes"
+                             % (16.0 * w.p * w.n * value / world / 8e12)}
+        if path == "fused":
             # the spill-free kernel moves (almost) no HBM bytes: it is bound by the FP32 pipes and shared memory
             flops_unit = 5.0 * w.n * np.log2(w.n) * w.p            # p * 5 N log2 N per template-segment
             apeak, asrc = alu_peak()
-            tfl = flops_unit * batch_templates[1] / (avg_ms[1] * 1e-3) / 1e12
-            hbm_model = line["roofline"]["path"]
-            hbm_model["note"] = ("for comparison only: what the two-pass model would have to move; the spill-free kernel "
-                                 "does not move these bytes (see traffic)")
+            tfl = flops_unit * count / (k_ms[2] * 1e-3) / 1e12
+            tr, tr_src = traffic_record(path, args.workload, "pass2")
             line["roofline"] = {
-                "bound": "alu", "kernel": names[1], "achieved": float(tfl), "peak": apeak, "unit": "TFLOP/s",
-                "frac": float(tfl / apeak), "peak_source": asrc,
-                "traffic": (FUSED_TRAFFIC_BYTES_PER_TEMPLATE * float(batch_templates[1]) if args.workload == "headline" else None),
-                "flops_per_launch": float(flops_unit * batch_templates[1]), "avg_launch_ms": float(avg_ms[1]),
-                "kernels": {"wide_bands": {"avg_launch_ms": float(avg_ms[0]), "share_of_step": float(k_ms[0] / k_ms.sum())},
-                            "k_fused": {"avg_launch_ms": float(avg_ms[1]), "TFLOP/s": float(tfl), "frac": float(tfl / apeak),
-                                        "share_of_step": float(k_ms[1] / k_ms.sum())}},
-                "hbm_model_equivalent": hbm_model,
-            }
+                "bound": "alu", "kernel": STAGE_TEXT[path]["pass2"], "achieved": float(tfl), "peak": apeak, "unit": "TFLOP/s",
+                "frac": float(tfl / apeak), "peak_source": asrc, "flops": "dense-FFT equivalent (p*5N*log2N per unit), not executed flops",
+                "traffic": tr * count / k_launch[2] if tr else None, "traffic_source": tr_src,
+                "avg_launch_ms": float(k_ms[2] / k_launch[2]), "kernels": kernels, "hbm_model_equivalent": hbm_model}
+        else:
+            dom = "pass1" if k_ms[1] > k_ms[2] else "pass2"
+            di = STAGES.index(dom)
+            tr, tr_src = traffic_record(path, args.workload, dom)
+            line["roofline"] = {
+                "bound": "hbm", "kernel": STAGE_TEXT[path][dom], "achieved": kernels[dom]["GB/s"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "peak_source": peak_src,
+                "bytes_per_launch": bytes_step / k_launch[di], "avg_launch_ms": float(k_ms[di] / k_launch[di]),
+                "traffic": tr * count / k_launch[di] if tr else None, "traffic_source": tr_src,
+                "kernels": kernels,
+                "path": {"bytes_per_unit": 16.0 * w.n * float(transforms.mean()),
+                         "achieved": 2 * bytes_step / ((k_ms[1] + k_ms[2]) * 1e-3) / 1e9,
+                         "frac": 2 * bytes_step / ((k_ms[1] + k_ms[2]) * 1e-3) / 1e9 / peak,
+                         "note": "both passes together: 16*N bytes per n-point transform that is run (%.2f per "
+                                 "template-segment) over the summed device time of pass 1 and pass 2"
+                                 % float(transforms.mean())},
+                "hbm_model_equivalent": hbm_model}
         if not args.no_cpu_baseline and world == 1:
             cores = min(host_cores(), 32)
             nt = cores * (2 if cores <= 16 else 1)
@@ -364,20 +418,14 @@ def run_gpu(args):
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{nt} of the {T} templates (evenly spread), full N={w.n} segment, "
                                               f"p={w.p}, {dt:.1f} s wall",
+                                    "note": "the oracle as it stands: unoptimised fp64, own radix-2 FFT, p full-size "
+                                            "transforms per template; a baseline, not a comparable CPU implementation",
                                     "context": "paper: 16x total speed-up, GeForce 8800 Ultra vs one 2.5 GHz Q9300 core "
                                                "(PAPER.md:5) -- other hardware, context only"}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
     return 0
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum PER TEMPLATE from the committed `ncu --set full` capture
-# (profiles/r1_v13_final.md, 16 templates per launch): index 0 = k_pass1_narrow ((0.0070 + 2.0882) GB / 16),
-# 1 = k_pass2 ((2.1475 + 0.0036) GB / 16); scaled by the templates per launch of the run.
-TRAFFIC_BYTES_PER_TEMPLATE = {0: 2.0952e9 / 16, 1: 2.1511e9 / 16}
-# k_fused: 5.5-7.2 MB read + 0 written per 16-template launch (profiles/r1_v14_fused.md)
-FUSED_TRAFFIC_BYTES_PER_TEMPLATE = 6.35e6 / 16
 
 
 def main():
@@ -388,11 +436,14 @@ def main():
     ap.add_argument("--impl", default="gwmf", choices=["gwmf", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="headline", choices=sorted(WORKLOADS))
-    ap.add_argument("--path", default="auto", choices=["auto", "two_pass", "fused"],
-                    help="auto = the library's choice (spill-free for n <= 2^20); the others force a path (GWMF_FUSED)")
+    ap.add_argument("--path", default="auto", choices=["auto", "two_pass", "fused", "decimated"],
+                    help="gwmf_params::path: auto = the library's choice (decimated for n >= 2^15)")
+    ap.add_argument("--batch", type=int, default=0, help="templates per launch (0 = library default)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
     return run_gpu(args)
 
 

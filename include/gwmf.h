@@ -146,6 +146,12 @@ int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma);
 /* Band edges e_0..e_p of every loaded template, HOST array of n_templates*(p+1) int32.  syncs. */
 int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges);
 
+/* Measurement: the number of n-point transforms the library runs for every loaded template with its path, HOST array
+ * of n_templates int32: the non-empty bands (two-pass and spill-free paths), or the effective bands of the
+ * decimated path (2 + the number of bands wider than min(8192, n/16) bins; just the wide bands if no band is
+ * narrow).  Each one is n complex fp32 written by pass 1 and read by pass 2: the byte model of bench.py.  syncs. */
+int gwmf_transform_counts(gwmf_ctx* ctx, int32_t* host_counts);
+
 /* Debug/parity: full rho(t) and chi^2(t) of one template, n floats each, HOST arrays (either may be
  * NULL).  Runs the same kernels as gwmf_filter on that template with series output enabled; does not
  * touch trigger slots.  syncs. */

@@ -95,15 +95,16 @@ Layout make_layout(const gwmf_params* p) {
   return L;
 }
 
-int fail_cuda(Ctx* c, cudaError_t e) {
+int fail_cuda(Ctx* c, cudaError_t e, int line = 0) {
   c->cuda_err = cudaGetErrorString(e);
+  if (line) c->cuda_err += " (api.cu:" + std::to_string(line) + ")";
   return GWMF_E_CUDA;
 }
 
-#define CU(call)                                       \
-  do {                                                 \
-    cudaError_t e__ = (call);                          \
-    if (e__ != cudaSuccess) return fail_cuda(c, e__);  \
+#define CU(call)                                                 \
+  do {                                                           \
+    cudaError_t e__ = (call);                                    \
+    if (e__ != cudaSuccess) return fail_cuda(c, e__, __LINE__);  \
   } while (0)
 
 // Every entry point runs on the context's device whatever device is current in the calling thread, and restores
@@ -469,6 +470,23 @@ int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma) {
   int rc = fetch_meta(c, v);
   if (rc != GWMF_OK) return rc;
   for (size_t t = 0; t < v.size(); ++t) host_sigma[t] = v[t].sigma;
+  return GWMF_OK;
+}
+
+int gwmf_transform_counts(gwmf_ctx* ctx, int32_t* host_counts) {
+  if (!ctx || !host_counts) return GWMF_E_ARG;
+  Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
+  std::vector<TemplateMeta> v;
+  int rc = fetch_meta(c, v);
+  if (rc != GWMF_OK) return rc;
+  const int p = c->prm.p;
+  for (size_t t = 0; t < v.size(); ++t) {
+    if (c->path == GWMF_PATH_DECIMATED) { host_counts[t] = v[t].n_eff; continue; }
+    int cnt = 0;
+    for (int l = 0; l < p; ++l) cnt += v[t].edges[l + 1] > v[t].edges[l] ? 1 : 0;
+    host_counts[t] = cnt;
+  }
   return GWMF_OK;
 }
 

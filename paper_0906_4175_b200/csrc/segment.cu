@@ -223,7 +223,10 @@ __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ m
   {
     int bins = 0, e_lo = 0, e_hi = 0;
     if (l < p) { e_lo = s_edges[ty][l]; e_hi = s_edges[ty][l + 1]; bins = e_hi - e_lo; }
-    const bool is_s = s_bins > 0 && bins > 0 && bins <= s_bins;
+    bool is_s = s_bins > 0 && bins > 0 && bins <= s_bins;
+    // Z and U cost two n-point transforms: decimate only if that is fewer than the narrow bands themselves (this
+    // also keeps n_eff <= p, the size the band buffer is carved for)
+    if (__popc(__ballot_sync(0xFFFFFFFFu, is_s)) <= 2) is_s = false;
     const bool is_d = bins > 0 && !is_s;
     const unsigned s_mask = __ballot_sync(0xFFFFFFFFu, is_s), d_mask = __ballot_sync(0xFFFFFFFFu, is_d);
     const int z_lo = __reduce_min_sync(0xFFFFFFFFu, is_s ? e_lo : 0x7FFFFFFF);

@@ -21,7 +21,7 @@ PATH_NAMES = {v: k for k, v in PATHS.items()}
 
 EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
-    "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_series", "gwmf_correlate",
+    "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_transform_counts", "gwmf_series", "gwmf_correlate",
     "gwmf_fft_inverse",
     "gwmf_uses_fused", "gwmf_path_in_use", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
@@ -69,6 +69,7 @@ def load_library():
     L.gwmf_triggers.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
     L.gwmf_sigma.argtypes = [C.c_void_p, C.c_void_p]
     L.gwmf_band_edges.argtypes = [C.c_void_p, C.c_void_p]
+    L.gwmf_transform_counts.argtypes = [C.c_void_p, C.c_void_p]
     L.gwmf_series.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.gwmf_correlate.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     L.gwmf_fft_inverse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -220,6 +221,12 @@ class Filter:
     def band_edges(self) -> np.ndarray:
         out = np.zeros((self.n_templates, self.p + 1), dtype=np.int32)
         self._check(self._L.gwmf_band_edges(self._h, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def transform_counts(self) -> np.ndarray:
+        """n-point transforms the library runs per template with its path (bench.py's byte model)."""
+        out = np.zeros(self.n_templates, dtype=np.int32)
+        self._check(self._L.gwmf_transform_counts(self._h, out.ctypes.data_as(C.c_void_p)))
         return out
 
     def series(self, template_id):
