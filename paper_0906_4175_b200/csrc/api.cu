@@ -82,6 +82,7 @@ Layout make_layout(const gwmf_params* p) {
   L.tw_l = take((size_t)kLMax * sizeof(float2));
   L.eff = take((2 * T + 1) * sizeof(int32_t));
   const int path = resolve_path(p);
+  L.slot_tab = take(path == GWMF_PATH_DECIMATED ? T * (size_t)p->p * sizeof(SlotDesc) : 256);
   L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
   L.qb = take(path == GWMF_PATH_FUSED ? 2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2) : 256);   // band-separated copy (k_fused)
   // decimated path: per-band one-sided power spectra W_l and their sum U+, double-buffered across batches

@@ -46,6 +46,16 @@ struct TemplateMeta {
 // One effective band: which spectrum it reads (kind) and the bins [e_lo, e_hi) it owns.
 enum EffKind { kEffZ = 0, kEffU = 1, kEffD = 2 };
 struct EffBand { int kind, e_lo, e_hi, l; };
+// The same, one record per slot of the whole bank (slot = eff_prefix[t] + e), written once per bank setup so that a
+// pass-1 CTA finds its work with ONE 32-byte load instead of a search through the template records.
+struct alignas(32) SlotDesc {
+  int32_t t;                     // template (index into the bank)
+  int32_t kind;                  // EffKind
+  int32_t e_lo, e_hi;            // bins
+  int32_t n_holes;               // Z only: class-D bands inside the hull (0 except for unusual spectra)
+  int32_t generic;               // 1: written by the generic kernel + row stage, not by k_pass1_eff
+  int32_t pad0, pad1;
+};
 #ifdef __CUDACC__
 __device__ __forceinline__ EffBand eff_band(const TemplateMeta* m, int e) {
   EffBand b;
@@ -74,7 +84,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, total;
+         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, total;
   size_t y_bytes;
   int batch;
 };

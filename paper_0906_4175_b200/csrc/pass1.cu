@@ -34,6 +34,7 @@ struct P1Args {
   // decimated path (effective bands, gwmf_internal.cuh): y is indexed by slot = eff_prefix - slot_base + e
   int eff;                    // 0: y is indexed by tb * p + l (two-pass / spill-free paths)
   int slot_base;              // eff_prefix of the first template of the batch
+  int first_template;         // bank index of the first template of the batch
   const float2* ubuf;         // [batch][kUCap] one-sided power spectra U+ (bandpower.cu)
 };
 
@@ -371,51 +372,47 @@ struct EffSrc {
   const int* holes;       // shared memory: [2h] = first bin of hole h, [2h+1] = one past its last bin
 };
 
-__device__ __forceinline__ bool eff_inside(const EffSrc& es, int k) {
-  if (k < es.e_lo || k >= es.e_hi) return false;
-  for (int h = 0; h < es.n_holes; ++h)
-    if (k >= es.holes[2 * h] && k < es.holes[2 * h + 1]) return false;
-  return true;
+// Input of thread (column k2) from row k1.  Rows strictly inside the band need no bin test: fr / lr are the first /
+// last row whose bin in THIS column belongs to the band (the band's first and last row are only partly inside).
+template <bool HOLES>
+__device__ __forceinline__ float2 eff_load(const EffSrc& es, int k1, int k2, int fr, int lr) {
+  const int k = (k1 << kLogN2) + k2;
+  bool ok = k1 >= fr && k1 <= lr;
+  if constexpr (HOLES) {
+    for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
+  }
+  float2 val = make_float2(0.f, 0.f);
+  if (ok) val = es.src[k];
+  return val;
 }
 
-template <int RMAX>
-__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float2* __restrict__ T1,
-                                           float2* __restrict__ tile, float2 Aja, int R, int row_lo, int ja, int k2, int m,
-                                           int ci) {
+// TW[i] = e^{2 pi i ja (row_lo + i)/n1} (shared, CTA constant).  The column part e^{2 pi i ja k2/n} of the twiddle is
+// split off: its m part rides on the T1 table (built per CTA), its c part on the per-thread twiddle of phase 2.
+template <int RMAX, bool HOLES>
+__device__ __forceinline__ void eff_phase1(const EffSrc& es, const float2* __restrict__ T1, const float2* __restrict__ TW,
+                                           float2* __restrict__ tile, tw4 g, int R, int row_lo, int k2, int m, int ci) {
   float2 v[32];
-  const int n1m = a.n1 - 1;
+  const int row_hi = (es.e_hi - 1) >> kLogN2;
+  const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);
+  const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
   if constexpr (RMAX < 32) {
 #pragma unroll
-    for (int i = 0; i < RMAX; ++i) {
-      float2 val = make_float2(0.f, 0.f);
-      const int k = ((row_lo + i) << kLogN2) + k2;
-      if (i < R && eff_inside(es, k)) {
-        const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], Aja);      // e^{2 pi i ja k/n}, k = 1024 k1 + k2
-        val = cmul(es.src[k], t);
-      }
-      v[brev<32>(i)] = val;
-    }
+    for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(eff_load<HOLES>(es, row_lo + i, k2, fr, lr), TW[i]);
   } else {
     const int T = (R + 31) >> 5;
-    const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                        // e^{2 pi i ja/NA}
 #pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = make_float2(0.f, 0.f);
+    for (int i = 0; i < 32; ++i) v[brev<32>(i)] = eff_load<HOLES>(es, row_lo + i + 32 * (T - 1), k2, fr, lr);
 #pragma unroll 1
-    for (int t = T - 1; t >= 0; --t) {
+    for (int t = T - 2; t >= 0; --t) {
 #pragma unroll
       for (int i = 0; i < 32; ++i) {
-        const int k = ((row_lo + i + 32 * t) << kLogN2) + k2;
-        float2 val = make_float2(0.f, 0.f);
-        if (eff_inside(es, k)) val = es.src[k];
+        const float2 val = eff_load<HOLES>(es, row_lo + i + 32 * t, k2, fr, lr);
         const float2 w = v[brev<32>(i)];
         v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
       }
     }
 #pragma unroll
-    for (int i = 0; i < 32; ++i) {
-      const float2 t = cmul(a.tw_n1[(ja * (row_lo + i)) & n1m], Aja);        // e^{2 pi i ja k_0/n}, k_0 = 1024 (row_lo + i) + k2
-      v[brev<32>(i)] = cmul(v[brev<32>(i)], t);
-    }
+    for (int i = 0; i < 32; ++i) v[brev<32>(i)] = cmul(v[brev<32>(i)], TW[i]);
   }
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
   const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
@@ -427,82 +424,91 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
   }
 }
 
-__global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a) {
+template <bool HOLES>
+__device__ __forceinline__ void eff_phase1_dispatch(const EffSrc& es, const float2* T1, const float2* TW, float2* tile, tw4 g,
+                                                    int R, int row_lo, int k2, int m, int ci) {
+  if (R <= 4) eff_phase1<4, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
+  else if (R <= 8) eff_phase1<8, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
+  else if (R <= 16) eff_phase1<16, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
+  else eff_phase1<32, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
+}
+
+__global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
   extern __shared__ __align__(128) float2 smem[];
   float2* tile = smem;                          // [32][kStageStride] (phase 1 uses stride kTileStride)
-  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i jb m/1024}
+  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i (jb/1024 + 32 ja/n) m}
+  __shared__ float2 TW[32];                     // e^{2 pi i ja (row_lo + i)/n1}
   __shared__ int s_holes[2 * kMaxBands];
-  __shared__ int s_nholes;
 
   const int tid = threadIdx.x;
   const int na = a.n1 >> 5;
   const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
-  const int slot = blockIdx.y;
+  const int slot = blockIdx.y;                  // batch-relative
   const unsigned nmask = (1u << a.log_n) - 1u;
+  const int n1m = a.n1 - 1;
 
-  // the template that owns this slot: the last tb with eff_prefix - slot_base <= slot
-  int lo = 0, hi = a.batch - 1;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (a.meta[mid].eff_prefix - a.slot_base <= slot) lo = mid; else hi = mid - 1;
-  }
-  const int tb = lo;
-  const TemplateMeta* mt = a.meta + tb;
-  const int e = slot - (mt->eff_prefix - a.slot_base);
-  if ((mt->gen_mask >> e) & 1u) return;         // very many rows: k_pass1 (generic) + k_rowstage write this slot
-  const EffBand eb = eff_band(mt, e);
+  const SlotDesc d = slot_tab[a.slot_base + slot];      // one 32-byte load, same address in every thread
+  if (d.generic) return;                        // very many rows: k_pass1 (generic) + k_rowstage write this slot
+  const int tb = d.t - a.first_template;
 
   EffSrc es;
-  es.e_lo = eb.e_lo;
-  es.e_hi = eb.e_hi;
+  es.e_lo = d.e_lo;
+  es.e_hi = d.e_hi;
   es.holes = s_holes;
-  es.src = eb.kind == kEffU ? a.ubuf + (size_t)tb * kUCap : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
-  if (tid == 0) {
-    int nh = 0;
-    if (eb.kind == kEffZ) {
-      unsigned d = mt->d_mask;
-      while (d) {
-        const int l = __ffs(d) - 1;
-        d &= d - 1;
-        if (mt->edges[l] >= eb.e_lo && mt->edges[l + 1] <= eb.e_hi) { s_holes[2 * nh] = mt->edges[l]; s_holes[2 * nh + 1] = mt->edges[l + 1]; ++nh; }
-      }
-    }
-    s_nholes = nh;
+  es.n_holes = d.n_holes;
+  es.src = d.kind == kEffU ? a.ubuf + (size_t)tb * kUCap : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
+  const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
+  const int R = row_hi - row_lo + 1;
+
+  const int ci = tid & 7, m = tid >> 3;
+  {
+    // T1 row m for jb = 4 ci .. 4 ci + 3, times this thread's m part of the column twiddle, e^{2 pi i ja 32 m/n}
+    const float2 Am = cis_frac(((unsigned)ja * 32u * (unsigned)m) & nmask, a.log_n);
+    const float4* src4 = reinterpret_cast<const float4*>(a.tw_p2 + m * 32 + 4 * ci);
+    const float4 w0 = __ldg(src4), w1 = __ldg(src4 + 1);
+    float4* dst = reinterpret_cast<float4*>(T1 + m * kT1Stride + 4 * ci);
+    const float2 p0 = cmul(make_float2(w0.x, w0.y), Am), p1 = cmul(make_float2(w0.z, w0.w), Am);
+    const float2 p2 = cmul(make_float2(w1.x, w1.y), Am), p3 = cmul(make_float2(w1.z, w1.w), Am);
+    dst[0] = make_float4(p0.x, p0.y, p1.x, p1.y);
+    dst[1] = make_float4(p2.x, p2.y, p3.x, p3.y);
   }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) T1[(tid >> 5) * kT1Stride + 8 * i * kT1Stride + (tid & 31)] = __ldg(&a.tw_p2[tid + 256 * i]);
+  if (tid < 32) TW[tid] = a.tw_n1[(ja * (row_lo + tid)) & n1m];
+  if (d.n_holes > 0 && tid == 0) {              // rare: class-D bands inside the hull of Z
+    const TemplateMeta* mt = a.meta + tb;
+    int nh = 0;
+    unsigned dm = mt->d_mask;
+    while (dm) {
+      const int l = __ffs(dm) - 1;
+      dm &= dm - 1;
+      if (mt->edges[l] >= es.e_lo && mt->edges[l + 1] <= es.e_hi) { s_holes[2 * nh] = mt->edges[l]; s_holes[2 * nh + 1] = mt->edges[l + 1]; ++nh; }
+    }
+  }
   __syncthreads();
-  es.n_holes = s_nholes;
 
   float2* out0 = a.y + ((size_t)slot * a.n1 + (size_t)ja) * kN2 + cg * 256;   // row jb adds jb * na * 1024
   const size_t row_stride = (size_t)na * kN2;
-  const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
-  const int R = row_hi - row_lo + 1;
   // ---- phase 1: thread (m, ci), column k2
   {
-    const int ci = tid & 7, m = tid >> 3;
     const int k2 = 32 * m + 8 * cg + ci;
-    const float2 Aja = cis_frac(((unsigned)ja * (unsigned)k2) & nmask, a.log_n);
-    if (R <= 4) eff_phase1<4>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
-    else if (R <= 8) eff_phase1<8>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
-    else if (R <= 16) eff_phase1<16>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
-    else eff_phase1<32>(a, es, T1, tile, Aja, R, row_lo, ja, k2, m, ci);
+    const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                         // e^{2 pi i ja/NA}
+    if (d.n_holes > 0) eff_phase1_dispatch<true>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
+    else eff_phase1_dispatch<false>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
   }
   __syncthreads();
   // ---- phase 2: thread (jb = lane, ci = warp)
   {
-    const int jb = tid & 31, ci = tid >> 5;
-    const int c = 8 * cg + ci;
-    float sn, cs;
-    const unsigned num = ((unsigned)jb * (unsigned)(c + 1024 * (row_lo & 31))) & 32767u;
-    sincospif((float)num * (1.0f / 16384.0f), &sn, &cs);
-    const tw4 S = make_tw4(make_float2(cs, sn));
+    const int jb = tid & 31, cw = tid >> 5;
+    const int c = 8 * cg + cw;
+    // e^{2 pi i jb (c + 1024 b0)/32768} (rest of the column twiddle e^{2 pi i NA jb k2/n} and the rotation w_32^{jb b0})
+    // times the c part of e^{2 pi i ja k2/n}: one angle, exact in integers mod n
+    const unsigned num = ((unsigned)jb * (unsigned)(c + 1024 * (row_lo & 31)) * (unsigned)na + (unsigned)ja * (unsigned)c) & nmask;
+    const tw4 S = make_tw4(cis_frac(num, a.log_n));
     float2 x[32];
 #pragma unroll
-    for (int m = 0; m < 32; ++m) x[brev<32>(m)] = cmul_tw(tile[jb * kTileStride + m * 8 + ci], S);
+    for (int mm = 0; mm < 32; ++mm) x[brev<32>(mm)] = cmul_tw(tile[jb * kTileStride + mm * 8 + cw], S);
     fft_dit<32>(x);                                   // over m -> jm
     __syncthreads();                                  // the tile has been read by everyone: reuse it as staging
-    float4* st = reinterpret_cast<float4*>(tile + jb * kStageStride + ci * 32);
+    float4* st = reinterpret_cast<float4*>(tile + jb * kStageStride + cw * 32);
 #pragma unroll
     for (int jm = 0; jm < 32; jm += 2) st[jm >> 1] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
   }
@@ -635,6 +641,7 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   args.batch = count;
   args.eff = 0;
   args.slot_base = 0;
+  args.first_template = 0;
   args.ubuf = nullptr;
   args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   args.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
@@ -706,6 +713,7 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.batch = 1;
   args.eff = 0;
   args.slot_base = 0;
+  args.first_template = 0;
   args.ubuf = nullptr;
   return dispatch_p1<true>(c, args, c->stream);
 }
@@ -728,6 +736,7 @@ static void fill_eff_args(Ctx* c, P1Args& args, int first, int count, int parity
   args.batch = count;
   args.eff = 1;
   args.slot_base = c->h_eff[first];
+  args.first_template = first;
   args.ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
 }
 
@@ -737,7 +746,7 @@ cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStrea
   fill_eff_args(c, args, first, count, parity);
   const int n_slots = c->h_eff[first + count] - c->h_eff[first];
   if (n_slots <= 0) return cudaSuccess;
-  k_pass1_eff<<<dim3(4 * c->na, n_slots), 256, kNarrowSmem, st>>>(args);
+  k_pass1_eff<<<dim3(4 * c->na, n_slots), 256, kNarrowSmem, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab));
   c->launches++;
   return cudaGetLastError();
 }

@@ -282,6 +282,33 @@ __global__ void __launch_bounds__(1024) k_eff_scan(TemplateMeta* __restrict__ me
   }
 }
 
+// slot table of the whole bank: one thread per (template, effective band)
+__global__ void __launch_bounds__(256) k_slot_table(const TemplateMeta* __restrict__ meta, SlotDesc* __restrict__ tab,
+                                                    int n_templates) {
+  const int t = blockIdx.x * 8 + (threadIdx.x >> 5), e = threadIdx.x & 31;
+  if (t >= n_templates) return;
+  const TemplateMeta* m = meta + t;
+  if (e >= m->n_eff) return;
+  const EffBand eb = eff_band(m, e);
+  SlotDesc d;
+  d.t = t;
+  d.kind = eb.kind;
+  d.e_lo = eb.e_lo;
+  d.e_hi = eb.e_hi;
+  d.n_holes = 0;
+  if (eb.kind == kEffZ) {
+    unsigned dm = m->d_mask;
+    while (dm) {
+      const int l = __ffs(dm) - 1;
+      dm &= dm - 1;
+      if (m->edges[l] >= eb.e_lo && m->edges[l + 1] <= eb.e_hi) ++d.n_holes;
+    }
+  }
+  d.generic = (m->gen_mask >> e) & 1u;
+  d.pad0 = d.pad1 = 0;
+  tab[m->eff_prefix + e] = d;
+}
+
 cudaError_t launch_bank_setup(Ctx* c) {
   const bool decim = c->path == GWMF_PATH_DECIMATED;
   k_bank_setup<<<(c->n_templates + 7) / 8, dim3(32, 8), 0, c->stream>>>(
@@ -294,7 +321,9 @@ cudaError_t launch_bank_setup(Ctx* c) {
   if (decim) {
     int32_t* d_eff = ws_ptr<int32_t>(c, c->lay.eff);
     k_eff_scan<<<1, 1024, 0, c->stream>>>(ws_ptr<TemplateMeta>(c, c->lay.meta), d_eff, c->n_templates);
-    c->launches++;
+    k_slot_table<<<(c->n_templates + 7) / 8, 256, 0, c->stream>>>(ws_ptr<TemplateMeta>(c, c->lay.meta),
+                                                                    ws_ptr<SlotDesc>(c, c->lay.slot_tab), c->n_templates);
+    c->launches += 2;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     e = cudaMemcpyAsync(c->h_eff, d_eff, sizeof(int32_t) * (size_t)(2 * c->n_templates + 1), cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) return e;
