@@ -372,41 +372,56 @@ struct EffSrc {
   const int* holes;       // shared memory: [2h] = first bin of hole h, [2h+1] = one past its last bin
 };
 
-// Input of thread (column k2) from row k1.  Rows strictly inside the band need no bin test: fr / lr are the first /
-// last row whose bin in THIS column belongs to the band (the band's first and last row are only partly inside).
+// Input of thread (column k2) from row k1, staged through shared memory by an 8-byte cp.async (LDGSTS): no
+// register is tied up while the load is in flight, so a whole round of 32 rows is requested at once.  Rows strictly
+// inside the band need no bin test: fr / lr are the first / last row whose bin in THIS column belongs to the band
+// (the band's first and last row are only partly inside); a masked element is zero-filled (src-size 0).
 template <bool HOLES>
-__device__ __forceinline__ float2 eff_load(const EffSrc& es, int k1, int k2, int fr, int lr) {
+__device__ __forceinline__ void eff_request(const EffSrc& es, float2* slot, int k1, int k2, int fr, int lr) {
   const int k = (k1 << kLogN2) + k2;
   bool ok = k1 >= fr && k1 <= lr;
   if constexpr (HOLES) {
     for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
   }
-  float2 val = make_float2(0.f, 0.f);
-  if (ok) val = es.src[k];
-  return val;
+  const float2* src = es.src + (ok ? k : es.e_lo);                 // always a valid address
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((unsigned)__cvta_generic_to_shared(slot)), "l"(src),
+               "r"(ok ? 8 : 0)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// First round of requests of a thread (rows row_lo + i + 32 (T-1), i < RMAX), issued BEFORE the CTA builds its
+// twiddle tables so that their latency overlaps that work.  stage: [32 rows][256 columns] aliasing the exchange tile;
+// a thread only ever touches its own column of it.
+template <int RMAX, bool HOLES>
+__device__ __forceinline__ void eff_request_round(const EffSrc& es, float2* stage_col, int row0, int k2, int fr, int lr) {
+#pragma unroll
+  for (int i = 0; i < RMAX; ++i) eff_request<HOLES>(es, stage_col + i * 256, row0 + i, k2, fr, lr);
+  cp_async_commit();
 }
 
 // TW[i] = e^{2 pi i ja (row_lo + i)/n1} (shared, CTA constant).  The column part e^{2 pi i ja k2/n} of the twiddle is
 // split off: its m part rides on the T1 table (built per CTA), its c part on the per-thread twiddle of phase 2.
 template <int RMAX, bool HOLES>
 __device__ __forceinline__ void eff_phase1(const EffSrc& es, const float2* __restrict__ T1, const float2* __restrict__ TW,
-                                           float2* __restrict__ tile, tw4 g, int R, int row_lo, int k2, int m, int ci) {
+                                           float2* __restrict__ tile, float2* stage_col, tw4 g, int T, int row_lo, int k2,
+                                           int fr, int lr, int m, int ci) {
   float2 v[32];
-  const int row_hi = (es.e_hi - 1) >> kLogN2;
-  const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);
-  const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
+  cp_async_wait_all();                                             // round T-1 has landed (own column only)
   if constexpr (RMAX < 32) {
 #pragma unroll
-    for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(eff_load<HOLES>(es, row_lo + i, k2, fr, lr), TW[i]);
+    for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(stage_col[i * 256], TW[i]);
   } else {
-    const int T = (R + 31) >> 5;
 #pragma unroll
-    for (int i = 0; i < 32; ++i) v[brev<32>(i)] = eff_load<HOLES>(es, row_lo + i + 32 * (T - 1), k2, fr, lr);
+    for (int i = 0; i < 32; ++i) v[brev<32>(i)] = stage_col[i * 256];
 #pragma unroll 1
     for (int t = T - 2; t >= 0; --t) {
+      eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * t, k2, fr, lr);
+      cp_async_wait_all();
 #pragma unroll
       for (int i = 0; i < 32; ++i) {
-        const float2 val = eff_load<HOLES>(es, row_lo + i + 32 * t, k2, fr, lr);
+        const float2 val = stage_col[i * 256];
         const float2 w = v[brev<32>(i)];
         v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
       }
@@ -415,6 +430,7 @@ __device__ __forceinline__ void eff_phase1(const EffSrc& es, const float2* __res
     for (int i = 0; i < 32; ++i) v[brev<32>(i)] = cmul(v[brev<32>(i)], TW[i]);
   }
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
+  __syncthreads();                          // every thread has consumed its staged inputs: the tile may be written
   const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
 #pragma unroll
   for (int jb = 0; jb < 32; jb += 2) {
@@ -425,42 +441,24 @@ __device__ __forceinline__ void eff_phase1(const EffSrc& es, const float2* __res
 }
 
 template <bool HOLES>
-__device__ __forceinline__ void eff_phase1_dispatch(const EffSrc& es, const float2* T1, const float2* TW, float2* tile, tw4 g,
-                                                    int R, int row_lo, int k2, int m, int ci) {
-  if (R <= 4) eff_phase1<4, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
-  else if (R <= 8) eff_phase1<8, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
-  else if (R <= 16) eff_phase1<16, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
-  else eff_phase1<32, HOLES>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
-}
-
-__global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
-  extern __shared__ __align__(128) float2 smem[];
-  float2* tile = smem;                          // [32][kStageStride] (phase 1 uses stride kTileStride)
-  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i (jb/1024 + 32 ja/n) m}
-  __shared__ float2 TW[32];                     // e^{2 pi i ja (row_lo + i)/n1}
-  __shared__ int s_holes[2 * kMaxBands];
-
+__device__ __forceinline__ void eff_cta(const P1Args& a, const EffSrc& es, float2* tile, float2* T1, float2* TW, int ja, int cg) {
   const int tid = threadIdx.x;
-  const int na = a.n1 >> 5;
-  const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
-  const int slot = blockIdx.y;                  // batch-relative
   const unsigned nmask = (1u << a.log_n) - 1u;
   const int n1m = a.n1 - 1;
-
-  const SlotDesc d = slot_tab[a.slot_base + slot];      // one 32-byte load, same address in every thread
-  if (d.generic) return;                        // very many rows: k_pass1 (generic) + k_rowstage write this slot
-  const int tb = d.t - a.first_template;
-
-  EffSrc es;
-  es.e_lo = d.e_lo;
-  es.e_hi = d.e_hi;
-  es.holes = s_holes;
-  es.n_holes = d.n_holes;
-  es.src = d.kind == kEffU ? a.ubuf + (size_t)tb * kUCap : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
   const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
-
+  const int T = (R + 31) >> 5;
   const int ci = tid & 7, m = tid >> 3;
+  const int k2 = 32 * m + 8 * cg + ci;
+  const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);
+  const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
+  float2* stage_col = tile + tid;               // [i][256]: column tid = m * 8 + ci of the staging area
+  const int rmax = R <= 4 ? 4 : R <= 8 ? 8 : R <= 16 ? 16 : 32;
+  // ---- request the first round of inputs, then build the tables while they are in flight
+  if (rmax == 4) eff_request_round<4, HOLES>(es, stage_col, row_lo, k2, fr, lr);
+  else if (rmax == 8) eff_request_round<8, HOLES>(es, stage_col, row_lo, k2, fr, lr);
+  else if (rmax == 16) eff_request_round<16, HOLES>(es, stage_col, row_lo, k2, fr, lr);
+  else eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * (T - 1), k2, fr, lr);
   {
     // T1 row m for jb = 4 ci .. 4 ci + 3, times this thread's m part of the column twiddle, e^{2 pi i ja 32 m/n}
     const float2 Am = cis_frac(((unsigned)ja * 32u * (unsigned)m) & nmask, a.log_n);
@@ -473,28 +471,60 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
     dst[1] = make_float4(p2.x, p2.y, p3.x, p3.y);
   }
   if (tid < 32) TW[tid] = a.tw_n1[(ja * (row_lo + tid)) & n1m];
-  if (d.n_holes > 0 && tid == 0) {              // rare: class-D bands inside the hull of Z
-    const TemplateMeta* mt = a.meta + tb;
-    int nh = 0;
-    unsigned dm = mt->d_mask;
-    while (dm) {
-      const int l = __ffs(dm) - 1;
-      dm &= dm - 1;
-      if (mt->edges[l] >= es.e_lo && mt->edges[l + 1] <= es.e_hi) { s_holes[2 * nh] = mt->edges[l]; s_holes[2 * nh + 1] = mt->edges[l + 1]; ++nh; }
+  const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                           // e^{2 pi i ja/NA}
+  __syncthreads();
+  // ---- phase 1: thread (m, ci), column k2
+  if (rmax == 4) eff_phase1<4, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
+  else if (rmax == 8) eff_phase1<8, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
+  else if (rmax == 16) eff_phase1<16, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
+  else eff_phase1<32, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
+}
+
+__global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
+  extern __shared__ __align__(128) float2 smem[];
+  float2* tile = smem;                          // [32][kStageStride] (phase 1: stride kTileStride; before that: input staging)
+  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i (jb/1024 + 32 ja/n) m}
+  __shared__ float2 TW[32];                     // e^{2 pi i ja (row_lo + i)/n1}
+  __shared__ int s_holes[2 * kMaxBands];
+
+  const int tid = threadIdx.x;
+  const int na = a.n1 >> 5;
+  const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
+  const int slot = blockIdx.y;                  // batch-relative
+  const unsigned nmask = (1u << a.log_n) - 1u;
+
+  const SlotDesc d = slot_tab[a.slot_base + slot];      // one 32-byte load, same address in every thread
+  if (d.generic) return;                        // very many rows: k_pass1 (generic) + k_rowstage write this slot
+  const int tb = d.t - a.first_template;
+
+  EffSrc es;
+  es.e_lo = d.e_lo;
+  es.e_hi = d.e_hi;
+  es.holes = s_holes;
+  es.n_holes = d.n_holes;
+  es.src = d.kind == kEffU ? a.ubuf + (size_t)tb * kUCap : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
+  const int row_lo = es.e_lo >> kLogN2;
+
+  if (d.n_holes > 0) {                          // rare: class-D bands inside the hull of Z
+    if (tid == 0) {
+      const TemplateMeta* mt = a.meta + tb;
+      int nh = 0;
+      unsigned dm = mt->d_mask;
+      while (dm) {
+        const int l = __ffs(dm) - 1;
+        dm &= dm - 1;
+        if (mt->edges[l] >= es.e_lo && mt->edges[l + 1] <= es.e_hi) { s_holes[2 * nh] = mt->edges[l]; s_holes[2 * nh + 1] = mt->edges[l + 1]; ++nh; }
+      }
     }
+    __syncthreads();
+    eff_cta<true>(a, es, tile, T1, TW, ja, cg);
+  } else {
+    eff_cta<false>(a, es, tile, T1, TW, ja, cg);
   }
   __syncthreads();
 
   float2* out0 = a.y + ((size_t)slot * a.n1 + (size_t)ja) * kN2 + cg * 256;   // row jb adds jb * na * 1024
   const size_t row_stride = (size_t)na * kN2;
-  // ---- phase 1: thread (m, ci), column k2
-  {
-    const int k2 = 32 * m + 8 * cg + ci;
-    const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                         // e^{2 pi i ja/NA}
-    if (d.n_holes > 0) eff_phase1_dispatch<true>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
-    else eff_phase1_dispatch<false>(es, T1, TW, tile, g, R, row_lo, k2, m, ci);
-  }
-  __syncthreads();
   // ---- phase 2: thread (jb = lane, ci = warp)
   {
     const int jb = tid & 31, cw = tid >> 5;
