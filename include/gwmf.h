@@ -78,9 +78,10 @@ typedef struct {
   double  rho_thresh;    /* SNR threshold, strict '>'                                             */
   int32_t window;        /* W: trigger window in samples, power of two, divides n                 */
   int32_t max_templates; /* capacity of the bank                                                  */
-  int32_t batch;         /* templates filtered per kernel launch, 0 .. 64 (0 = library default: about
-                            2 GiB of band intermediate); sizes the band-intermediate buffer,
-                            batch * p * n * 8 bytes, and the correlated spectra, 2 * batch * n * 4 bytes */
+  int32_t batch;         /* most templates filtered per kernel launch, 0 .. 64; sizes the band-intermediate
+                            buffer, batch * p * n * 8 bytes, and the correlated spectra, 2 * batch * n * 4 bytes.
+                            0 = library default: a band buffer of about 2 GiB; the decimated path then takes up
+                            to 64 templates per launch, as many as fit in it (it needs ~3, not p, transforms each) */
   int32_t path;          /* a gwmf_path; GWMF_PATH_AUTO (0) = the library's choice.  A path that does not support n
                             (FUSED: 2^15 .. 2^20, DECIMATED: >= 2^15) is GWMF_E_ARG                               */
 } gwmf_params;
@@ -100,18 +101,25 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
  * are (re)computed on the device by gwmf_load_segment / here if a segment is already loaded.  async. */
 int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_templates);
 
-/* Load one strain segment and its PSD (Eq. 1 inputs).
+/* Load one strain segment and, optionally, a new PSD (Eq. 1 inputs).
  *   s  : n fp32 samples of s(t), HOST or DEVICE pointer.
- *   Sn : n/2+1 fp64 samples of the one-sided PSD at f_k = k fs/n, HOST or DEVICE pointer.  Entries
- *        below f_low and the Nyquist entry are ignored (Eq. 2 diverges at f -> 0).  Entries inside
- *        [f_low, fs/2) must be finite and > 0 -- checked on the device; a violation is reported by
+ *   Sn : n/2+1 fp64 samples of the one-sided PSD at f_k = k fs/n, HOST or DEVICE pointer, or NULL = keep the PSD
+ *        (and with it sigma and the band edges of every template) of the previous call; the first call must give
+ *        one (else GWMF_E_STATE).  Entries below f_low and the Nyquist entry are ignored (Eq. 2 diverges at f -> 0).
+ *        Entries inside [f_low, fs/2) must be finite and > 0 -- checked on the device; a violation is reported by
  *        the next syncing call as GWMF_E_ARG.
- * Computes on the device: the data spectrum D[k] = sum_j s[j] e^{-2 pi i jk/n} with the library's own
- * FFT, the weighted spectrum w[k] = (4/n) D[k] f_k^(-7/6) / S_n[k], the fp64 power table
- * C[k] = sum_{k'<=k} f^(-7/3)/S_n (Eq. 4) and, if a bank is loaded, sigma and band edges of every
- * template.  The arrays may be freed after the call returns (host sources are staged synchronously
- * with respect to the host; device sources are read on the stream before the call returns control
- * to later work on that stream).  async for device sources. */
+ * Computes on the device: the data spectrum D[k] = sum_j s[j] e^{-2 pi i jk/n} with the library's own FFT, the
+ * weighted spectrum w[k] = (4/n) D[k] f_k^(-7/6) / S_n[k] and, with a new PSD, the fp64 power table
+ * C[k] = sum_{k'<=k} f^(-7/3)/S_n (Eq. 4) and sigma and band edges of every loaded template.
+ * Ownership: both arrays may be freed as soon as the call returns (host sources are staged before it returns;
+ * device sources are read on the context's stream, ordered like any other work the caller puts on that stream).
+ * Overlap (the bank sweep of BASELINE.json:configs[3]): the segment buffers are double-buffered.
+ * With a HOST segment and Sn == NULL the upload and the transform run on the library's own upload stream, beside
+ * filters of the previous segment that are still running; gwmf_filter calls issued AFTER this call use the new
+ * segment (they wait for it on the device, not on the host).  The events of the previous segment stay readable by
+ * gwmf_triggers until the next gwmf_filter call, so the steady state of a sweep is
+ *     gwmf_filter(q);  gwmf_load_segment(q + 1, NULL);  gwmf_triggers(q).
+ * With a device segment or a new PSD the work is ordered on the context's stream (no overlap).  async. */
 int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn);
 
 /* Matched-filter templates [first_template, first_template + n_templates) against the loaded segment
@@ -133,7 +141,8 @@ int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
                       int32_t* host_launches);
 
-/* Collect the events of all templates filtered since the last gwmf_load_segment, sorted by
+/* Collect the events of all templates filtered on the segment the last gwmf_filter call used (a gwmf_load_segment
+ * issued after that call does not disturb them; the first gwmf_filter on the new segment clears them), sorted by
  * (template_id, window).  host_out: HOST array of `capacity` triggers (may be NULL if capacity = 0).
  * *n_out receives the number of events found; GWMF_E_CAPACITY if it exceeds capacity (nothing is
  * written beyond capacity).  syncs. */

@@ -57,7 +57,16 @@ Layout make_layout(const gwmf_params* p) {
   const size_t n1 = n / kN2;
   const size_t nw = n / (size_t)p->window;
   const size_t T = (size_t)p->max_templates;
+  const int path = resolve_path(p);
   L.batch = p->batch > 0 ? p->batch : default_batch(p);
+  L.y_slots = L.batch * p->p;
+  if (path == GWMF_PATH_DECIMATED && p->batch == 0) {
+    // this path needs far fewer than p transforms per template (2 + the wide bands): keep the ~2 GiB band buffer but
+    // let a launch take as many templates as fit in it, up to kMaxBatch (launch gaps and kernel tails amortise:
+    // measured 60.6 k -> 65.6 k template-segments/s from 16 to 64 templates per launch at n = 2^20)
+    L.batch = kMaxBatch;
+    if (L.y_slots < p->p) L.y_slots = p->p;
+  }
   if (L.batch > p->max_templates) L.batch = p->max_templates;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
@@ -65,8 +74,9 @@ Layout make_layout(const gwmf_params* p) {
   L.c_tab = take(half * sizeof(double));
   L.g_tab = take(half * sizeof(double));
   L.sn = take((half + 1) * sizeof(double));
-  L.wq = take(half * sizeof(float2));
-  L.s_in = take(n * sizeof(float));
+  L.wq = take(2 * half * sizeof(float2));                      // double-buffered across segments
+  L.s_in = take(2 * n * sizeof(float));
+  L.prep = take(3 * n * sizeof(float2));                       // segment preparation scratch: input, intermediate, transform
   L.tw_n1 = take(n1 * sizeof(float2));
   L.tw_p2 = take(1024 * sizeof(float2));
   L.meta = take(T * sizeof(TemplateMeta));
@@ -81,19 +91,41 @@ Layout make_layout(const gwmf_params* p) {
   L.flags = take(256);
   L.tw_l = take((size_t)kLMax * sizeof(float2));
   L.eff = take((2 * T + 1) * sizeof(int32_t));
-  const int path = resolve_path(p);
   L.slot_tab = take(path == GWMF_PATH_DECIMATED ? T * (size_t)p->p * sizeof(SlotDesc) : 256);
   L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
   L.qb = take(path == GWMF_PATH_FUSED ? 2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2) : 256);   // band-separated copy (k_fused)
   // decimated path: per-band one-sided power spectra W_l and their sum U+, double-buffered across batches
   L.wbuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * (size_t)p->p * kUCap * sizeof(float2) : 256);
   L.ubuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * kUCap * sizeof(float2) : 256);
-  size_t yb = (size_t)L.batch * (size_t)p->p * n * sizeof(float2);
+  size_t yb = (size_t)L.y_slots * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;
   L.y = take(yb);
   L.total = off;
   return L;
+}
+
+bool create_upload_side(Ctx* c) {
+  if (cudaStreamCreateWithFlags(&c->upload, cudaStreamNonBlocking) != cudaSuccess) return false;
+  if (cudaEventCreateWithFlags(&c->ev_last_load, cudaEventDisableTiming) != cudaSuccess) return false;
+  for (int b = 0; b < 2; ++b) {
+    if (cudaMallocHost((void**)&c->h_stage[b], sizeof(float) * (size_t)c->n) != cudaSuccess) return false;
+    if (cudaEventCreateWithFlags(&c->ev_seg_ready[b], cudaEventDisableTiming) != cudaSuccess) return false;
+    if (cudaEventCreateWithFlags(&c->ev_seg_free[b], cudaEventDisableTiming) != cudaSuccess) return false;
+    if (cudaEventCreateWithFlags(&c->ev_stage_free[b], cudaEventDisableTiming) != cudaSuccess) return false;
+  }
+  return true;
+}
+
+void destroy_upload_side(Ctx* c) {
+  if (c->upload) { cudaStreamSynchronize(c->upload); cudaStreamDestroy(c->upload); c->upload = nullptr; }
+  if (c->ev_last_load) cudaEventDestroy(c->ev_last_load);
+  for (int b = 0; b < 2; ++b) {
+    if (c->h_stage[b]) cudaFreeHost(c->h_stage[b]);
+    if (c->ev_seg_ready[b]) cudaEventDestroy(c->ev_seg_ready[b]);
+    if (c->ev_seg_free[b]) cudaEventDestroy(c->ev_seg_free[b]);
+    if (c->ev_stage_free[b]) cudaEventDestroy(c->ev_stage_free[b]);
+  }
 }
 
 int fail_cuda(Ctx* c, cudaError_t e, int line = 0) {
@@ -195,6 +227,12 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->h_masks = nullptr;
   c->h_eff = nullptr;
   c->mirror_ready = false;
+  c->front = 0;
+  c->have_psd = false;
+  c->pending_reset = false;
+  c->upload = nullptr;
+  c->ev_last_load = nullptr;
+  for (int b = 0; b < 2; ++b) { c->h_stage[b] = nullptr; c->ev_seg_ready[b] = c->ev_seg_free[b] = c->ev_stage_free[b] = nullptr; }
   // > 48 KB of dynamic shared memory is an opt-in per function AND per device: do it for this context's device
   if (configure_pass1(c->path) != cudaSuccess || configure_pass2() != cudaSuccess || configure_bandpower() != cudaSuccess) {
     delete c;
@@ -210,7 +248,9 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_masks, cudaEventDisableTiming) != cudaSuccess ||
         cudaMallocHost((void**)&c->h_masks, sizeof(uint32_t) * (size_t)params->max_templates) != cudaSuccess ||
-        cudaMallocHost((void**)&c->h_eff, sizeof(int32_t) * (size_t)(2 * params->max_templates + 1)) != cudaSuccess) {
+        cudaMallocHost((void**)&c->h_eff, sizeof(int32_t) * (size_t)(2 * params->max_templates + 1)) != cudaSuccess ||
+        !create_upload_side(c)) {
+      destroy_upload_side(c);
       if (c->side) cudaStreamDestroy(c->side);
       if (c->ev_fork) cudaEventDestroy(c->ev_fork);
       if (c->ev_join) cudaEventDestroy(c->ev_join);
@@ -241,6 +281,7 @@ void gwmf_destroy(gwmf_ctx* ctx) {
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
   DeviceGuard guard(c->device);
   cudaStreamSynchronize(c->stream);
+  destroy_upload_side(c);
   if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
@@ -266,27 +307,67 @@ int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_t
   c->n_templates = n_templates;
   c->have_bank = true;
   CU(launch_reset_slots(c, 0, c->prm.max_templates));
-  if (c->have_segment) CU(launch_bank_setup(c));
+  if (c->have_segment) {
+    CU(cudaStreamWaitEvent(c->stream, c->ev_last_load, 0));   // the PSD tables of a load that ran on the upload stream
+    CU(launch_bank_setup(c));
+  }
   return GWMF_OK;
 }
 
 int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn) {
-  if (!ctx || !s || !Sn) return GWMF_E_ARG;
+  if (!ctx || !s) return GWMF_E_ARG;
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
   DeviceGuard guard(c->device);
-  CU(cudaMemcpyAsync(ws_ptr<float>(c, c->lay.s_in), s, sizeof(float) * (size_t)c->n, cudaMemcpyDefault, c->stream));
-  CU(cudaMemcpyAsync(ws_ptr<double>(c, c->lay.sn), Sn, sizeof(double) * (size_t)(c->n / 2 + 1), cudaMemcpyDefault,
-                     c->stream));
-  // pinned host sources are copied truly asynchronously: wait so that the caller may free them
-  cudaPointerAttributes at_s, at_p;
-  bool dev_s = cudaPointerGetAttributes(&at_s, s) == cudaSuccess && at_s.type == cudaMemoryTypeDevice;
-  bool dev_p = cudaPointerGetAttributes(&at_p, Sn) == cudaSuccess && at_p.type == cudaMemoryTypeDevice;
+  if (!Sn && !c->have_psd) return GWMF_E_STATE;               // "same PSD" needs an earlier call that gave one
+  cudaPointerAttributes at;
+  const bool dev_s = cudaPointerGetAttributes(&at, s) == cudaSuccess && at.type == cudaMemoryTypeDevice;
   cudaGetLastError();
-  if (!dev_s || !dev_p) CU(cudaStreamSynchronize(c->stream));
-  CU(launch_segment_prepare(c));
+  const int back = c->have_segment ? c->front ^ 1 : 0;
+  const size_t s_bytes = sizeof(float) * (size_t)c->n;
+  // A host segment with an unchanged PSD is uploaded and transformed on the upload stream, beside the filters of the
+  // previous segment.  Everything else (device sources; a new PSD, which rewrites tables the filters read) is simply
+  // ordered on the main stream.
+  const bool overlapped = !dev_s && !Sn;
+  cudaStream_t st = overlapped ? c->upload : c->stream;
+  if (overlapped) {
+    CU(cudaEventSynchronize(c->ev_stage_free[back]));           // the staging buffer's previous upload (long done)
+    memcpy(c->h_stage[back], s, s_bytes);                       // the caller's array is free again on return
+    CU(cudaStreamWaitEvent(st, c->ev_seg_free[back], 0));       // filters that still read s_in / wq[back]
+    CU(cudaStreamWaitEvent(st, c->ev_last_load, 0));            // the preparation scratch
+    CU(cudaMemcpyAsync(s_buf(c, back), c->h_stage[back], s_bytes, cudaMemcpyHostToDevice, st));
+    CU(cudaEventRecord(c->ev_stage_free[back], st));
+  } else {
+    CU(cudaStreamWaitEvent(st, c->ev_last_load, 0));
+    CU(cudaMemcpyAsync(s_buf(c, back), s, s_bytes, cudaMemcpyDefault, st));
+    if (Sn)
+      CU(cudaMemcpyAsync(ws_ptr<double>(c, c->lay.sn), Sn, sizeof(double) * (size_t)(c->n / 2 + 1), cudaMemcpyDefault, st));
+    // pinned host sources are copied truly asynchronously: wait so that the caller may free them on return
+    bool dev_p = true;
+    if (Sn) { dev_p = cudaPointerGetAttributes(&at, Sn) == cudaSuccess && at.type == cudaMemoryTypeDevice; cudaGetLastError(); }
+    if (!dev_s || !dev_p) CU(cudaStreamSynchronize(st));
+  }
+  CU(launch_segment_fft(c, back, st));
+  if (Sn) CU(launch_psd_tables(c, st));
+  CU(launch_weighted_spectrum(c, back, st));
+  CU(cudaEventRecord(c->ev_seg_ready[back], st));
+  CU(cudaEventRecord(c->ev_last_load, st));
+  c->front = back;
   c->have_segment = true;
-  CU(launch_reset_slots(c, 0, c->prm.max_templates));
-  if (c->have_bank) CU(launch_bank_setup(c));
+  c->pending_reset = true;                                     // events of the previous segment stay readable until the next filter
+  if (Sn) {
+    c->have_psd = true;
+    if (c->have_bank) CU(launch_bank_setup(c));
+  }
+  return GWMF_OK;
+}
+
+// Before any work that reads the current segment's weighted spectrum on the main stream.
+static int begin_segment_use(Ctx* c) {
+  CU(cudaStreamWaitEvent(c->stream, c->ev_seg_ready[c->front], 0));
+  return GWMF_OK;
+}
+static int end_segment_use(Ctx* c) {
+  CU(cudaEventRecord(c->ev_seg_free[c->front], c->stream));
   return GWMF_OK;
 }
 
@@ -348,31 +429,53 @@ static cudaError_t decimated_batch(Ctx* c, int first, int count, int next_first,
   return launch_pass2_eff(c, first, count, update_slots, series_rho, series_chi);
 }
 
+// Cut [first, first + n) into launches: at most lay.batch templates each and, on the decimated path, at most
+// lay.y_slots n-point transforms (the band buffer's capacity); needs the host mirror.
+static void partition(const Ctx* c, int first, int n, std::vector<int>& counts) {
+  counts.clear();
+  int t = first;
+  const int end = first + n;
+  while (t < end) {
+    int cnt = 0;
+    if (c->path == GWMF_PATH_DECIMATED) {
+      while (t + cnt < end && cnt < c->lay.batch && c->h_eff[t + cnt + 1] - c->h_eff[t] <= c->lay.y_slots) ++cnt;
+      if (cnt == 0) cnt = 1;                      // cannot happen: n_eff <= p <= y_slots
+    } else {
+      cnt = end - t < c->lay.batch ? end - t : c->lay.batch;
+    }
+    counts.push_back(cnt);
+    t += cnt;
+  }
+}
+
 // All batches of [first_template, first_template + n_templates).  ev: 4 events per batch (timed mode) or nullptr.
-static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t* ev) {
-  int rc = ensure_mirror(c);
+static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t* ev, const std::vector<int>& counts) {
+  int rc = begin_segment_use(c);
   if (rc != GWMF_OK) return rc;
+  if (c->pending_reset) {                       // first filter call on a new segment: forget the previous segment's events
+    CU(launch_reset_slots(c, 0, c->prm.max_templates));
+    c->pending_reset = false;
+  }
   CU(launch_reset_slots(c, first_template, n_templates));
-  int parity = 0, b = 0;
-  for (int done = 0; done < n_templates; done += c->lay.batch, parity ^= 1, ++b) {
-    const int cnt = n_templates - done < c->lay.batch ? n_templates - done : c->lay.batch;
-    const int rest = n_templates - done - cnt;
-    const int next = rest < c->lay.batch ? rest : c->lay.batch;
-    const int f0 = first_template + done;
+  int parity = 0, f0 = first_template;
+  for (size_t b = 0; b < counts.size(); ++b, parity ^= 1) {
+    const int cnt = counts[b];
+    const int next = b + 1 < counts.size() ? counts[b + 1] : 0;
     cudaEvent_t* evb = ev ? ev + 4 * b : nullptr;
     if (c->path == GWMF_PATH_DECIMATED) {
-      CU(decimated_batch(c, f0, cnt, f0 + cnt, next, parity, done > 0, true, nullptr, nullptr, evb));
-      continue;
+      CU(decimated_batch(c, f0, cnt, f0 + cnt, next, parity, b > 0, true, nullptr, nullptr, evb));
+    } else {
+      if (evb) CU(cudaEventRecord(evb[0], c->stream));
+      if (evb) CU(cudaEventRecord(evb[1], c->stream));
+      CU(launch_pass1_filter(c, f0, cnt, f0 + cnt, next, parity, b > 0));
+      if (evb) CU(cudaEventRecord(evb[2], c->stream));
+      if (c->fused) CU(launch_fused_filter(c, f0, cnt, parity, true, nullptr, nullptr));
+      else CU(launch_pass2_filter(c, f0, cnt, true, nullptr, nullptr));
+      if (evb) CU(cudaEventRecord(evb[3], c->stream));
     }
-    if (evb) CU(cudaEventRecord(evb[0], c->stream));
-    if (evb) CU(cudaEventRecord(evb[1], c->stream));
-    CU(launch_pass1_filter(c, f0, cnt, f0 + cnt, next, parity, done > 0));
-    if (evb) CU(cudaEventRecord(evb[2], c->stream));
-    if (c->fused) CU(launch_fused_filter(c, f0, cnt, parity, true, nullptr, nullptr));
-    else CU(launch_pass2_filter(c, f0, cnt, true, nullptr, nullptr));
-    if (evb) CU(cudaEventRecord(evb[3], c->stream));
+    f0 += cnt;
   }
-  return GWMF_OK;
+  return end_segment_use(c);
 }
 
 static bool range_ok(const Ctx* c, int32_t first_template, int32_t n_templates) {
@@ -387,7 +490,11 @@ int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates) {
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
   if (!range_ok(c, first_template, n_templates)) return GWMF_E_ARG;
   if (n_templates == 0) return GWMF_OK;
-  return run_batches(c, first_template, n_templates, nullptr);
+  int rc = ensure_mirror(c);
+  if (rc != GWMF_OK) return rc;
+  std::vector<int> counts;
+  partition(c, first_template, n_templates, counts);
+  return run_batches(c, first_template, n_templates, nullptr, counts);
 }
 
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
@@ -397,14 +504,18 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
   DeviceGuard guard(c->device);
   if (!c->have_bank || !c->have_segment) return GWMF_E_STATE;
   if (!range_ok(c, first_template, n_templates) || n_templates < 1) return GWMF_E_ARG;
-  const int nb = (n_templates + c->lay.batch - 1) / c->lay.batch;
+  int rc = ensure_mirror(c);
+  if (rc != GWMF_OK) return rc;
+  std::vector<int> counts;
+  partition(c, first_template, n_templates, counts);
+  const int nb = (int)counts.size();
   struct Events {                                   // destroyed on every exit path
     std::vector<cudaEvent_t> v;
     ~Events() { for (cudaEvent_t e : v) if (e) cudaEventDestroy(e); }
   } ev;
   ev.v.assign((size_t)nb * 4, nullptr);
   for (auto& e : ev.v) CU(cudaEventCreate(&e));
-  int rc = run_batches(c, first_template, n_templates, ev.v.data());
+  rc = run_batches(c, first_template, n_templates, ev.v.data(), counts);
   if (rc != GWMF_OK) return rc;
   CU(cudaStreamSynchronize(c->stream));
   host_ms[0] = host_ms[1] = host_ms[2] = 0.0;
@@ -516,6 +627,7 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
   float* d_chi = ws_ptr<float>(c, c->lay.series_chi);
   rc = ensure_mirror(c);
   if (rc != GWMF_OK) return rc;
+  if ((rc = begin_segment_use(c)) != GWMF_OK) return rc;
   if (c->path == GWMF_PATH_DECIMATED) {
     CU(decimated_batch(c, template_id, 1, 0, 0, 0, false, false, d_rho, d_chi, nullptr));
   } else {
@@ -541,6 +653,7 @@ int gwmf_correlate(gwmf_ctx* ctx, int32_t template_id, float* host_q) {
   if (rc != GWMF_OK) return rc;
   const size_t half = (size_t)(c->n / 2);
   float2* d_q = ws_ptr<float2>(c, c->lay.q);
+  if ((rc = begin_segment_use(c)) != GWMF_OK) return rc;
   CU(cudaMemsetAsync(d_q, 0, half * sizeof(float2), c->stream));      // bins outside [k_low, k_high) are not written
   CU(launch_correlate(c, template_id, 1, 0, c->stream));
   CU(cudaMemcpyAsync(host_q, d_q, half * sizeof(float2), cudaMemcpyDeviceToHost, c->stream));
@@ -554,7 +667,7 @@ int gwmf_fft_inverse(gwmf_ctx* ctx, const float* d_in, float* d_out) {
   DeviceGuard guard(c->device);
   // the band intermediate doubles as the pass-1 output of the dense transform
   CU(launch_fft_dense(c, reinterpret_cast<const float2*>(d_in), ws_ptr<float2>(c, c->lay.y),
-                      reinterpret_cast<float2*>(d_out)));
+                      reinterpret_cast<float2*>(d_out), c->stream));
   return GWMF_OK;
 }
 

@@ -84,9 +84,10 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, total;
+         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, total;
   size_t y_bytes;
-  int batch;
+  int batch;                     // most templates per launch
+  int y_slots;                   // n-point transforms (n complex fp32 each) the band buffer holds
 };
 
 struct Ctx {
@@ -118,27 +119,42 @@ struct Ctx {
   TemplateMeta* h_meta;          // host staging of the bank (pinned)
   uint32_t* h_masks;             // host mirror of TemplateMeta::wide_mask (pinned), valid once ev_masks has fired
   cudaEvent_t ev_masks;
+  // ---- double-buffered segment (s_in, wq): a segment can be uploaded and prepared on the upload stream while the
+  // filters of the previous one still run on the main stream (gwmf_load_segment with Sn == NULL)
+  int front;                     // buffer the filters read
+  bool have_psd;
+  bool pending_reset;            // a segment was loaded since the last filter call: the next one clears every slot first
+  cudaStream_t upload;
+  float* h_stage[2];             // pinned staging of host segments (n floats each)
+  cudaEvent_t ev_seg_ready[2];   // wq[b] is complete (recorded on the stream that prepared it)
+  cudaEvent_t ev_seg_free[2];    // the last filter launch that reads wq[b] (recorded on the main stream)
+  cudaEvent_t ev_stage_free[2];  // the H2D copy out of h_stage[b] is done
+  cudaEvent_t ev_last_load;      // end of the latest load (orders the shared preparation scratch between streams)
 };
+inline float2* wq_buf(Ctx* c, int b) { return reinterpret_cast<float2*>(c->ws + c->lay.wq) + (size_t)b * (size_t)(c->n / 2); }
+inline float* s_buf(Ctx* c, int b) { return reinterpret_cast<float*>(c->ws + c->lay.s_in) + (size_t)b * (size_t)c->n; }
 
 // ---- launchers (defined in the .cu files) --------------------------------------------------------
 cudaError_t launch_tables(Ctx* c);
-cudaError_t launch_segment_prepare(Ctx* c);                       // after s/Sn are on the device
+cudaError_t launch_segment_fft(Ctx* c, int buf, cudaStream_t st);      // s_in[buf] -> data spectrum in the preparation scratch
+cudaError_t launch_psd_tables(Ctx* c, cudaStream_t st);                // sn -> g_tab, c_tab, flags
+cudaError_t launch_weighted_spectrum(Ctx* c, int buf, cudaStream_t st); // scratch spectrum, sn, c_tab -> wq[buf]
 cudaError_t launch_bank_setup(Ctx* c);
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready);
 cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st);
 cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cudaStream_t st);
 inline int qb_rows_cap(const Ctx* c) { return c->n1 / 2 + kMaxBands + 2; }   // rows of Qb per template
-cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid);
-cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid);
+cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid, cudaStream_t st);
+cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid, cudaStream_t st);
 cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots, float* series_rho,
                                 float* series_chi);
 cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool update_slots, float* series_rho,
                                 float* series_chi);
-cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out);
-inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, float2* d_out) {
-  cudaError_t e = launch_pass1_dense(c, d_in, d_mid);
-  if (e == cudaSuccess) e = launch_rowstage_dense(c, d_mid);
-  return e != cudaSuccess ? e : launch_pass2_dense(c, d_mid, d_out);
+cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out, cudaStream_t st);
+inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, float2* d_out, cudaStream_t st) {
+  cudaError_t e = launch_pass1_dense(c, d_in, d_mid, st);
+  if (e == cudaSuccess) e = launch_rowstage_dense(c, d_mid, st);
+  return e != cudaSuccess ? e : launch_pass2_dense(c, d_mid, d_out, st);
 }
 // decimated path
 cudaError_t configure_pass1(int path);

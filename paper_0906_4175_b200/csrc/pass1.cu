@@ -637,7 +637,7 @@ __global__ void __launch_bounds__(256) k_correlate_bands(const TemplateMeta* __r
 cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   const int cap = qb_rows_cap(c);
   k_correlate_bands<<<dim3(c->n1 / 2 + c->prm.p + 1, count), 256, 0, st>>>(
-      ws_ptr<TemplateMeta>(c, c->lay.meta) + first, ws_ptr<float2>(c, c->lay.wq), ws_ptr<double>(c, c->lay.u_tab),
+      ws_ptr<TemplateMeta>(c, c->lay.meta) + first, wq_buf(c, c->front), ws_ptr<double>(c, c->lay.u_tab),
       ws_ptr<float2>(c, c->lay.qb) + (size_t)parity * c->lay.batch * cap * kN2, c->prm.p, cap);
   c->launches++;
   return cudaGetLastError();
@@ -645,7 +645,7 @@ cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cud
 
 cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   const int half = (int)(c->n / 2);
-  k_correlate<<<dim3(half / 256, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, ws_ptr<float2>(c, c->lay.wq),
+  k_correlate<<<dim3(half / 256, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, wq_buf(c, c->front),
                                                       ws_ptr<double>(c, c->lay.u_tab),
                                                       ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half, half);
   c->launches++;
@@ -660,7 +660,7 @@ cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStrea
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready) {
   P1Args args;
   args.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
-  args.wq = ws_ptr<float2>(c, c->lay.wq);
+  args.wq = wq_buf(c, c->front);
   args.u_tab = ws_ptr<double>(c, c->lay.u_tab);
   args.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
   args.dense_in = nullptr;
@@ -727,7 +727,7 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   return cudaStreamWaitEvent(c->stream, c->ev_join, 0);
 }
 
-cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
+cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid, cudaStream_t st) {
   P1Args args;
   args.meta = nullptr;
   args.wq = nullptr;
@@ -745,15 +745,15 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid) {
   args.slot_base = 0;
   args.first_template = 0;
   args.ubuf = nullptr;
-  return dispatch_p1<true>(c, args, c->stream);
+  return dispatch_p1<true>(c, args, st);
 }
 
-cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid) { return launch_rowstage(c, d_mid, nullptr, 1, 1, 0, c->stream); }
+cudaError_t launch_rowstage_dense(Ctx* c, float2* d_mid, cudaStream_t st) { return launch_rowstage(c, d_mid, nullptr, 1, 1, 0, st); }
 
 // ---- decimated path launchers ---------------------------------------------------------------------
 static void fill_eff_args(Ctx* c, P1Args& args, int first, int count, int parity) {
   args.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
-  args.wq = ws_ptr<float2>(c, c->lay.wq);
+  args.wq = wq_buf(c, c->front);
   args.u_tab = ws_ptr<double>(c, c->lay.u_tab);
   args.tw_n1 = ws_ptr<float2>(c, c->lay.tw_n1);
   args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);

@@ -620,7 +620,7 @@ cudaError_t launch_pass2_filter(Ctx* c, int first, int count, bool update_slots,
   return cudaGetLastError();
 }
 
-cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
+cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out, cudaStream_t st) {
   P2Args a;
   a.y = d_mid;
   a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
@@ -636,7 +636,7 @@ cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out) {
   a.n_windows = 0;
   a.n_rows = c->n1;
   a.thresh = 0.f;
-  k_pass2<true, false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(a);
+  k_pass2<true, false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, st>>>(a);
   c->launches++;
   return cudaGetLastError();
 }

@@ -134,34 +134,44 @@ __global__ void k_weighted_spectrum(const float2* __restrict__ Z, const double* 
   wq[k] = out;
 }
 
-cudaError_t launch_segment_prepare(Ctx* c) {
-  const int half = (int)(c->n / 2);
-  float2* y = ws_ptr<float2>(c, c->lay.y);
-  float2* X = y;                       // n complex: the segment as complex input
-  float2* mid = y + c->n;              // n complex: pass-1 output
-  float2* Z = y + 2 * c->n;            // n complex: transform
-  k_real_to_complex<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(ws_ptr<float>(c, c->lay.s_in), X, c->n);
+// The preparation is cut in three so that the part that depends only on the samples (the transform) can run on the
+// upload stream while filters of the previous segment still use the PSD tables and the other wq buffer.
+// Scratch (own region of the workspace, 3 n complex): X = the segment as complex input, mid, Z = its transform.
+cudaError_t launch_segment_fft(Ctx* c, int buf, cudaStream_t st) {
+  float2* X = ws_ptr<float2>(c, c->lay.prep);
+  float2* mid = X + c->n;
+  float2* Z = X + 2 * c->n;
+  k_real_to_complex<<<(unsigned)((c->n + 255) / 256), 256, 0, st>>>(s_buf(c, buf), X, c->n);
   c->launches++;
-  cudaError_t e = launch_fft_dense(c, X, mid, Z);
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  return launch_fft_dense(c, X, mid, Z, st);
+}
+
+cudaError_t launch_psd_tables(Ctx* c, cudaStream_t st) {
+  const int half = (int)(c->n / 2);
   int* flags = ws_ptr<int>(c, c->lay.flags);
-  cudaMemsetAsync(flags, 0, sizeof(int), c->stream);
-  k_power_terms<<<(half + 255) / 256, 256, 0, c->stream>>>(ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab),
-                                                           ws_ptr<double>(c, c->lay.g_tab), flags, c->k_low, half);
-  {
-    const int L = (half + kPrefixChunks - 1) / kPrefixChunks;
-    const size_t sm = (size_t)L * sizeof(double);
-    double* totals = ws_ptr<double>(c, c->lay.prefix_totals);
-    k_prefix_totals<<<kPrefixChunks, 32, sm, c->stream>>>(ws_ptr<double>(c, c->lay.g_tab), totals, half, L);
-    k_prefix_scan<<<1, 1, 0, c->stream>>>(totals);
-    k_prefix_write<<<kPrefixChunks, 32, sm, c->stream>>>(ws_ptr<double>(c, c->lay.g_tab), totals,
-                                                         ws_ptr<double>(c, c->lay.c_tab), half, L);
-    c->launches += 2;
-  }
-  k_weighted_spectrum<<<(half + 255) / 256, 256, 0, c->stream>>>(
-      Z, ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab), ws_ptr<double>(c, c->lay.c_tab),
-      ws_ptr<float2>(c, c->lay.wq), c->k_low, half, 4.0 / (double)c->n, 4.0 * c->df);
-  c->launches += 3;
+  cudaError_t e = cudaMemsetAsync(flags, 0, sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  k_power_terms<<<(half + 255) / 256, 256, 0, st>>>(ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab),
+                                                    ws_ptr<double>(c, c->lay.g_tab), flags, c->k_low, half);
+  const int L = (half + kPrefixChunks - 1) / kPrefixChunks;
+  const size_t sm = (size_t)L * sizeof(double);
+  double* totals = ws_ptr<double>(c, c->lay.prefix_totals);
+  k_prefix_totals<<<kPrefixChunks, 32, sm, st>>>(ws_ptr<double>(c, c->lay.g_tab), totals, half, L);
+  k_prefix_scan<<<1, 1, 0, st>>>(totals);
+  k_prefix_write<<<kPrefixChunks, 32, sm, st>>>(ws_ptr<double>(c, c->lay.g_tab), totals, ws_ptr<double>(c, c->lay.c_tab), half, L);
+  c->launches += 4;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_weighted_spectrum(Ctx* c, int buf, cudaStream_t st) {
+  const int half = (int)(c->n / 2);
+  const float2* Z = ws_ptr<float2>(c, c->lay.prep) + 2 * c->n;
+  k_weighted_spectrum<<<(half + 255) / 256, 256, 0, st>>>(Z, ws_ptr<double>(c, c->lay.sn), ws_ptr<double>(c, c->lay.u_tab),
+                                                          ws_ptr<double>(c, c->lay.c_tab), wq_buf(c, buf), c->k_low, half,
+                                                          4.0 / (double)c->n, 4.0 * c->df);
+  c->launches++;
   return cudaGetLastError();
 }
 

@@ -166,8 +166,9 @@ class Filter:
         self._check(self._L.gwmf_make_bank(self._h, arr, len(masses)))
         self.n_templates = len(masses)
 
-    def load_segment(self, s, Sn):
-        """s: n samples (numpy or torch, host or device; cast to fp32); Sn: n/2+1 PSD samples (fp64)."""
+    def load_segment(self, s, Sn=None):
+        """s: n samples (numpy or torch, host or device; cast to fp32); Sn: n/2+1 PSD samples (fp64), or None to keep
+        the PSD of the previous call (then a host segment is uploaded and prepared beside the running filters)."""
         torch = self.torch
         keep = []
 
@@ -181,7 +182,7 @@ class Filter:
             return a.ctypes.data
 
         ps = as_ptr(s, torch.float32)
-        pn = as_ptr(Sn, torch.float64)
+        pn = as_ptr(Sn, torch.float64) if Sn is not None else None
         self._check(self._L.gwmf_load_segment(self._h, C.c_void_p(ps), C.c_void_p(pn)))
         # device sources are read asynchronously on the stream: keep them alive until it drains
         if any(isinstance(k, torch.Tensor) and k.is_cuda for k in keep):

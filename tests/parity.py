@@ -15,6 +15,7 @@ RHO_ABS, RHO_REL = 1e-3, 1e-4
 CHI_REL, CHI_ABS = 1e-3, 1e-3
 SIGMA_REL = 1e-5
 MARGIN = 1e-3
+NEIGHBOUR_MARGIN = 2e-5
 
 
 def assert_series(rho_gpu, chi_gpu, rho_orc, chi_orc, p, what=""):
@@ -35,9 +36,10 @@ def assert_sigma_edges(sig_gpu, edges_gpu, sig_orc, edges_orc):
     assert np.array_equal(np.asarray(edges_gpu, dtype=np.int64), np.asarray(edges_orc, dtype=np.int64))
 
 
-def assert_triggers(trig_gpu, bank_out, thresh, W, p, template_ids=None):
+def assert_triggers(trig_gpu, bank_out, thresh, W, p, template_ids=None, series_of=None):
     """trig_gpu: structured array from Filter.triggers(); bank_out: oracle.filter_bank(...) dict whose row
-    i describes template template_ids[i] (default: identity).  Returns (#compared, #exempt)."""
+    i describes template template_ids[i] (default: identity).  series_of(tid) -> (rho, chisq) fp64 oracle series of
+    a template, only called to settle a trigger that is one sample off.  Returns (#compared, #exempt)."""
     T, nw = bank_out["best_rho"].shape
     ids = list(range(T)) if template_ids is None else list(template_ids)
     got = {(int(t["template_id"]), int(t["sample"]) // W): t for t in trig_gpu if int(t["template_id"]) in set(ids)}
@@ -58,9 +60,16 @@ def assert_triggers(trig_gpu, bank_out, thresh, W, p, template_ids=None):
                 continue
             if rho > thresh:
                 assert g is not None, f"missing trigger: template {tid} window {w} oracle rho {rho}"
-                assert int(g["sample"]) == int(bank_out["best_j"][i, w]), (tid, w, g, bank_out["best_j"][i, w])
-                assert abs(float(g["rho"]) - rho) <= RHO_ABS + RHO_REL * rho
                 chi = bank_out["best_chisq"][i, w]
+                jg, jo = int(g["sample"]), int(bank_out["best_j"][i, w])
+                if jg != jo and abs(jg - jo) == 1 and series_of is not None:
+                    rho_s, chi_s = series_of(tid)         # near-tie with the sample next to the maximum?
+                    assert rho_s[jo] - rho_s[jg] <= NEIGHBOUR_MARGIN, (tid, w, g, jo, rho_s[jo], rho_s[jg])
+                    rho, chi = float(rho_s[jg]), float(chi_s[jg])
+                    exempt += 1
+                else:
+                    assert jg == jo, (tid, w, g, jo)
+                assert abs(float(g["rho"]) - rho) <= RHO_ABS + RHO_REL * rho
                 assert abs(float(g["chisq"]) - chi) <= CHI_REL * chi + CHI_ABS
                 compared += 1
             else:

@@ -48,8 +48,8 @@ def test_workspace_bytes_host_only(lib):
     b = gwmf.workspace_bytes(1 << 20, 16, 4096, 1024)
     # band intermediate: batch(16) * p * n * 8 B = 2 GiB, plus the double-buffered correlated spectra
     # (2 * batch * 4 MiB), tables / slots / staging
-    assert (2 << 30) + (128 << 20) < b < (2 << 30) + (384 << 20)
-    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (340 << 20)
+    assert (2 << 30) + (128 << 20) < b < (2 << 30) + (1024 << 20)
+    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (360 << 20)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
 
@@ -62,7 +62,7 @@ def test_null_arguments_are_rejected_without_a_gpu(lib):
     assert lib.gwmf_triggers(None, None, 0, ctypes.byref(n)) == -1
     h = ctypes.c_void_p()
     from paper_0906_4175_b200 import gwmf
-    prm = gwmf.Params(1 << 14, 4096.0, 40.0, 4, 6.0, 4096, 8, 0)
+    prm = gwmf.Params(1 << 14, 4096.0, 40.0, 4, 6.0, 4096, 8, 0, 0)
     assert lib.gwmf_create(ctypes.byref(prm), None, 0, None, ctypes.byref(h)) == -1     # no workspace
 
 
