@@ -410,13 +410,13 @@ def test_load_segment_semantics(gw):
 def test_wide_band_inside_narrow_ones(gw, path):
     # a PSD with a strong line: the band that has to cross it becomes wide while its neighbours stay narrow, so the
     # decimated path's union of narrow bands has a hole (a class-D band inside the hull of Z) -- DESIGN.md section 5
-    n = 1 << 18
+    n = 1 << 20                                 # 70 Hz = 17920 bins > 8192: the crossing band is class D
     Sn = inputs.psd_array(n)
     df = inputs.FS / n
     lo, hi = int(95.0 / df), int(165.0 / df)
     Sn = Sn.copy()
     Sn[lo:hi] *= 1e4                            # 95-165 Hz carries almost no weight
-    masses = [(1.4, 1.4), (5.0, 4.0), (2.0, 1.0)]
+    masses = [(1.4, 1.4), (5.0, 4.0), (12.0, 9.0)]
     D = inputs.noise_spectrum(n, 71)
     D[lo:hi] *= 100.0                           # noise consistent with the PSD
     D = D + inputs.injection_spectrum(n, 5.0, 4.0, 30.0, n // 5)
