@@ -55,6 +55,12 @@ WORKLOADS = {
                          "threshold 5.5, window 4096, 4 injections, seed 4"),
     "snr_only": dict(config=2, p=1, templates=None, metric="template-segments/sec at N=2^20, p=1 (SNR only, PAPER.md:164)",
                      text="SURVEY.md 8(f)-2: configs[2]'s segment and bank with p=1 (one inverse FFT per template, no chi^2)"),
+    "sweep": dict(config=3, p=None, templates=None,
+                  metric="sustained template-segments/sec over the 15-segment x 4096-template bank sweep at N=2^20, p=16 "
+                         "(SNR+chi^2), segment uploads included and overlapped",
+                  text="BASELINE.json:configs[3]: 15 half-overlapping segments of N=2^20 from one seeded 2^23-sample stream "
+                       "(Eq. 2 noise + 16 injections, seed 3), each against a 4096-template bank (total mass 2-34 Msun), "
+                       "p=16, threshold 6, window 4096"),
     "long16": dict(config=4, p=16, templates=None, metric="template-segments/sec at N=2^22, p=16 (SNR+chi^2)",
                    text="SURVEY.md 8(f)-3: configs[4]'s segment (N=2^22, 1024 s) and bank (512 templates, m1,m2 in [1,2] "
                         "Msun) with the headline p=16, threshold 5.5"),
@@ -92,11 +98,40 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def shard_plan(world_size: int, rank: int, n_templates: int):
-    """Weak scaling: every rank owns `n_templates` template-segments (the whole bank against its own
-    segment, seed offset = rank).  Returns (segment_seed_offset, first_template, count)."""
+def shard_plan(world_size: int, rank: int, n_templates: int, shard: str = "segments"):
+    """Returns (segment_seed_offset, first_template, count).
+    shard = "segments" (weak scaling, the default): every rank owns the whole bank against its OWN segment (seed offset =
+    rank): n_templates template-segments per rank, no data-path communication.
+    shard = "templates" (strong scaling, SURVEY.md 8(e) / PAPER.md:196): ONE segment, the bank split into contiguous
+    ranges of template ids; the segment is broadcast once, the per-rank event lists are gathered in template order."""
     assert 0 <= rank < world_size
-    return rank, 0, n_templates
+    if shard == "segments":
+        return rank, 0, n_templates
+    base, rem = divmod(n_templates, world_size)
+    first = rank * base + min(rank, rem)
+    return 0, first, base + (1 if rank < rem else 0)
+
+
+def gather_triggers(trig, dist=None, device=None):
+    """Template-sharded mode: concatenate the ranks' event lists (each already sorted by (template, window), ranges of
+    template ids ascending with the rank) into the bank's list on every rank: an all_gather of fixed-capacity
+    buffers, the capacity being the largest per-rank count."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return trig
+    import torch
+    world = dist.get_world_size()
+    dev = device if device is not None else "cpu"
+    cnt = torch.tensor([len(trig)], dtype=torch.int64, device=dev)
+    counts = [torch.zeros_like(cnt) for _ in range(world)]
+    dist.all_gather(counts, cnt)
+    cap = max(int(c.item()) for c in counts)
+    buf = torch.zeros(max(cap, 1) * 16, dtype=torch.uint8, device=dev)
+    raw = torch.from_numpy(np.frombuffer(trig.tobytes(), dtype=np.uint8).copy())
+    buf[: raw.numel()] = raw.to(dev)
+    bufs = [torch.zeros_like(buf) for _ in range(world)]
+    dist.all_gather(bufs, buf)
+    parts = [np.frombuffer(b.cpu().numpy().tobytes()[: int(c.item()) * 16], dtype=trig.dtype) for b, c in zip(bufs, counts)]
+    return np.concatenate(parts) if parts else trig
 
 
 def reduce_max_ms(ms: float, dist=None, device=None) -> float:
@@ -283,25 +318,39 @@ def run_gpu(args):
         torch.cuda.synchronize(dev)
 
     w, _ = load_workload(args.workload)
-    seed_off, first, count = shard_plan(world, rank, len(w.masses))
+    seed_off, first, count = shard_plan(world, rank, len(w.masses), args.shard)
     w.seed += seed_off
-    s32 = inputs.segment(w).astype(np.float32)
+    if w.config == 3:
+        x = inputs.stream(w).astype(np.float32)
+        segs = [np.ascontiguousarray(inputs.stream_segment(x, q, w.n)) for q in range(w.n_segments)]
+    else:
+        segs = [inputs.segment(w).astype(np.float32)]
+    nseg = len(segs)
+    s32 = segs[0]
     Sn = w.psd
     T = len(w.masses)
 
     f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}", path=args.path, batch=args.batch)
     path = f.path
     f.make_bank(w.masses)
-    s_dev = torch.from_numpy(s32).to(dev)
+    segs_dev = [torch.from_numpy(sg).to(dev) for sg in segs]
     sn_dev = torch.from_numpy(Sn).to(dev)
-    f.load_segment(s_dev, sn_dev)
+    if world > 1 and args.shard == "templates":
+        for sd in segs_dev:                                  # one segment for everybody: rank 0's copy over NVLink
+            dist.broadcast(sd, src=0)
+    f.load_segment(segs_dev[0], sn_dev)
 
     def step_resident():
-        f.filter(first, count)
-        return f.triggers()
+        out = None
+        for q in range(nseg):
+            if nseg > 1:
+                f.load_segment(segs_dev[q])                  # device-resident segment, same PSD
+            f.filter(first, count)
+            out = f.triggers()
+        return out
 
     sampler = ClockSampler(local)
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(args.warmup, 3) if nseg == 1 else max(min(args.warmup, 3), 1)):
         trig = step_resident()
     barrier()
     sampler.start()
@@ -314,7 +363,10 @@ def run_gpu(args):
     barrier()
     launches = f.launch_count - l0
     ms = reduce_max_ms(e0.elapsed_time(e1), dist if world > 1 else None, dev)
-    value = world * count * args.steps / (ms * 1e-3)
+    value = world * count * nseg * args.steps / (ms * 1e-3) if args.shard == "segments" else T * nseg * args.steps / (ms * 1e-3)
+    if world > 1 and args.shard == "templates":
+        trig = gather_triggers(trig, dist, dev)              # the bank's event list of the last segment, on every rank
+    f.load_segment(segs_dev[0])
 
     # per-stage device times (events inside the library, on its stream, stages serialised)
     reps = 3
@@ -330,41 +382,60 @@ def run_gpu(args):
     bytes_step = float(transforms.sum()) * w.n * 8.0        # pass 1 writes / pass 2 reads n complex fp32 per transform
     peak, peak_src = measured_peak()
 
-    # end to end through the C ABI with host buffers
-    s_pin = torch.from_numpy(s32).pin_memory()
-    sn_pin = torch.from_numpy(Sn).pin_memory()
+    # end to end through the C ABI with HOST buffers: every segment is uploaded from pinned host memory inside the timed
+    # region, overlapped with the filters of the segment before it (gwmf_load_segment with the PSD kept), and every
+    # segment's events are read back:   filter(q); load(q + 1); triggers(q)
+    segs_pin = [torch.from_numpy(sg).pin_memory() for sg in segs]
+    f.load_segment(segs_pin[0], Sn)
 
     def step_e2e():
-        f.load_segment(s_pin, sn_pin)
-        f.filter(first, count)
-        return f.triggers()
+        out = None
+        for q in range(nseg):
+            f.filter(first, count)
+            f.load_segment(segs_pin[(q + 1) % nseg])        # the next segment (of this or of the next step)
+            out = f.triggers()
+        return out
 
-    for _ in range(3):
-        trig = step_e2e()
+    for _ in range(3 if nseg == 1 else 1):
+        trig_e = step_e2e()
     barrier()
     t0 = time.perf_counter()
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     g0.record(f.stream)
+    d2h = 0
     for _ in range(args.steps):
-        trig = step_e2e()
+        trig_e = step_e2e()
     g1.record(f.stream)
     barrier()
     wall_ms = (time.perf_counter() - t0) * 1e3
     ms_e2e = reduce_max_ms(max(g0.elapsed_time(g1), wall_ms), dist if world > 1 else None, dev)
     clocks = sampler.stop()
-    e2e_value = world * count * args.steps / (ms_e2e * 1e-3)
+    units = world * count if args.shard == "segments" else T
+    e2e_value = units * nseg * args.steps / (ms_e2e * 1e-3)
+    f.load_segment(segs_dev[0])
+    f.filter(first, count)
+    f.synchronize()
 
     if rank == 0:
         line = base_line(args, w, value, ms / args.steps, "f32")
         line["config"]["path"] = path
+        if nseg > 1:
+            line["roofline_note"] = "per-stage times and bytes below are those of ONE segment (gwmf_filter_timed)"
         line["config"]["batch_templates_per_launch"] = float(count / max(k_launch[2], 1))
         line["config"]["n_point_transforms_per_template"] = float(transforms.mean())
         line["config"]["l2"] = ("no flush: every step streams the band intermediate (%.2f GB written by pass 1 and read by "
                                 "pass 2 per step, %.0fx the 126 MB L2); the correlated spectra (%.0f MiB per launch) are "
                                 "produced and consumed through L2 by design"
                                 % (bytes_step / 1e9, bytes_step / 126e6, count / max(k_launch[2], 1) * w.n * 4 / 2**20))
-        line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(s32.nbytes + Sn.nbytes),
-                       "d2h_bytes_per_step": int(12 + trig.nbytes), "ms_per_step": ms_e2e / args.steps}
+        line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(nseg * s32.nbytes),
+                       "d2h_bytes_per_step": int(nseg * 12 + nseg * trig_e.nbytes), "ms_per_step": ms_e2e / args.steps,
+                       "note": "per step: %d segment upload(s) from pinned host memory (the PSD is loaded once, before the timed "
+                               "region, and kept), %d filter call(s), %d event read-back(s); uploads overlap the previous "
+                               "segment's filters on the library's upload stream" % (nseg, nseg, nseg)}
+        line["config"]["segments_per_step"] = nseg
+        line["config"]["units_per_step"] = int(units * nseg)
+        line["scaling"] = "weak" if args.shard == "segments" else "strong"
+        line["config"]["shard"] = args.shard
         line["gpu_launches"] = int(launches)
         line["clocks"] = clocks
         line["triggers_per_step"] = int(len(trig))
@@ -439,6 +510,9 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "two_pass", "fused", "decimated"],
                     help="gwmf_params::path: auto = the library's choice (decimated for n >= 2^15)")
     ap.add_argument("--batch", type=int, default=0, help="templates per launch (0 = library default)")
+    ap.add_argument("--shard", default="segments", choices=["segments", "templates"],
+                    help="N > 1: segments = every rank filters the whole bank against its own segment (weak scaling); "
+                         "templates = one segment, the bank split by template id, events gathered (strong scaling)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
