@@ -26,8 +26,9 @@ namespace gwmf {
 
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }        // one float2 of padding per 16: the
                                                                             // stride-1 groups of the last stage become conflict-free
-constexpr int kBpThreads = 512;
-constexpr size_t kBpSmem = (size_t)(kLMax + (kLMax >> 4)) * sizeof(float2);
+constexpr int kBpThreads = 256;
+constexpr size_t bp_smem(int log_l) { return (size_t)((1 << log_l) + ((1 << log_l) >> 4)) * sizeof(float2); }
+constexpr int kBpSmallLogL = 13;      // size classes: L <= 8192 (69.6 KB of shared memory: two CTAs per SM) and L = 16384
 
 template <int LOG_L>
 __device__ __forceinline__ void bandpower_body(float2* __restrict__ sm, const float2* __restrict__ tw_l,
@@ -105,8 +106,11 @@ __device__ __forceinline__ void bandpower_body(float2* __restrict__ sm, const fl
   }
 }
 
-// grid (p, templates of the batch): W[tb][l][m] = one-sided power spectrum of class-S band l, 0 <= m < B_l
-__global__ void __launch_bounds__(kBpThreads, 1) k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q,
+// grid (p, templates of the batch): W[tb][l][m] = one-sided power spectrum of class-S band l, 0 <= m < B_l.
+// Two launches per batch, one per size class (LARGE = the 16384-point grid): a CTA whose band belongs to the other
+// class exits at once, so that the small class is not held to one CTA per SM by the large one's shared memory.
+template <bool LARGE>
+__global__ void __launch_bounds__(kBpThreads, 2) k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q,
                                                              const float2* __restrict__ tw_l, float2* __restrict__ wbuf,
                                                              int p, int half_n) {
   extern __shared__ __align__(16) float2 sm_bp[];
@@ -114,15 +118,19 @@ __global__ void __launch_bounds__(kBpThreads, 1) k_bandpower(const TemplateMeta*
   const TemplateMeta* m = meta + tb;
   if (!((m->s_mask >> l) & 1u)) return;
   const int e_lo = m->edges[l], B = m->edges[l + 1] - e_lo;
-  const float2* qband = q + (size_t)tb * half_n + e_lo;
-  float2* wout = wbuf + ((size_t)tb * p + l) * kUCap;
   int log_l = kLogLMin;
   while ((1 << log_l) < 2 * B) ++log_l;
-  switch (log_l) {
-    case 11: bandpower_body<11>(sm_bp, tw_l, qband, B, wout); break;
-    case 12: bandpower_body<12>(sm_bp, tw_l, qband, B, wout); break;
-    case 13: bandpower_body<13>(sm_bp, tw_l, qband, B, wout); break;
-    default: bandpower_body<14>(sm_bp, tw_l, qband, B, wout); break;
+  if ((log_l > kBpSmallLogL) != LARGE) return;
+  const float2* qband = q + (size_t)tb * half_n + e_lo;
+  float2* wout = wbuf + ((size_t)tb * p + l) * kUCap;
+  if constexpr (LARGE) {
+    bandpower_body<14>(sm_bp, tw_l, qband, B, wout);
+  } else {
+    switch (log_l) {
+      case 11: bandpower_body<11>(sm_bp, tw_l, qband, B, wout); break;
+      case 12: bandpower_body<12>(sm_bp, tw_l, qband, B, wout); break;
+      default: bandpower_body<13>(sm_bp, tw_l, qband, B, wout); break;
+    }
   }
 }
 
@@ -147,7 +155,9 @@ __global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ 
 }
 
 cudaError_t configure_bandpower() {
-  return cudaFuncSetAttribute(k_bandpower, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBpSmem);
+  cudaError_t e = cudaFuncSetAttribute(k_bandpower<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(kBpSmallLogL));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(14));
+  return e;
 }
 
 cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st) {
@@ -157,7 +167,12 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
   const float2* q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half;
   float2* wbuf = ws_ptr<float2>(c, c->lay.wbuf) + (size_t)parity * c->lay.batch * p * kUCap;
   float2* ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
-  k_bandpower<<<dim3(p, count), kBpThreads, kBpSmem, st>>>(meta, q, ws_ptr<float2>(c, c->lay.tw_l), wbuf, p, (int)half);
+  const float2* tw_l = ws_ptr<float2>(c, c->lay.tw_l);
+  k_bandpower<false><<<dim3(p, count), kBpThreads, bp_smem(kBpSmallLogL), st>>>(meta, q, tw_l, wbuf, p, (int)half);
+  if (c->s_bins > (1 << (kBpSmallLogL - 1))) {      // bands of more than 4096 bins exist only if the class allows them
+    k_bandpower<true><<<dim3(p, count), kBpThreads, bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half);
+    c->launches++;
+  }
   k_uspec<<<dim3(c->s_bins / 256, count), 256, 0, st>>>(meta, wbuf, ubuf, p);
   c->launches += 2;
   return cudaGetLastError();

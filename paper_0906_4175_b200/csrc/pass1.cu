@@ -226,9 +226,10 @@ __global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const 
 // read by every ja-slice of pass 1 out of L2.
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_correlate(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wq,
-                                                   const double* __restrict__ u_tab, float2* __restrict__ q, int half_n) {
+                                                   const double* __restrict__ u_tab, float2* __restrict__ q, int half_n,
+                                                   int k_first) {
   const TemplateMeta* m = meta + blockIdx.y;
-  const int k = blockIdx.x * 256 + threadIdx.x;
+  const int k = k_first + blockIdx.x * 256 + threadIdx.x;
   if (k < m->edges[0] || k >= m->k_high) return;
   // correlate: template phasor times weighted data bin (Eq. 1 integrand)
   const double u = u_tab[k];
@@ -645,9 +646,16 @@ cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cud
 
 cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   const int half = (int)(c->n / 2);
-  k_correlate<<<dim3(half / 256, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, wq_buf(c, c->front),
-                                                      ws_ptr<double>(c, c->lay.u_tab),
-                                                      ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half, half);
+  // only the bins some template of the batch owns: k_low .. the batch's largest k_high (host-side bank scalars)
+  int kh = 0;
+  for (int t = first; t < first + count; ++t) kh = c->h_meta[t].k_high > kh ? c->h_meta[t].k_high : kh;
+  const int k_first = c->k_low & ~255;
+  const int blocks = (kh - k_first + 255) / 256;
+  if (blocks <= 0) return cudaSuccess;
+  k_correlate<<<dim3(blocks, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, wq_buf(c, c->front),
+                                                  ws_ptr<double>(c, c->lay.u_tab),
+                                                  ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half, half,
+                                                  k_first);
   c->launches++;
   return cudaGetLastError();
 }
