@@ -27,62 +27,101 @@ namespace gwmf {
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }        // one float2 of padding per 16: the
                                                                             // stride-1 groups of the last stage become conflict-free
 constexpr int kBpThreads = 256;
-constexpr size_t bp_smem(int log_l) { return (size_t)((1 << log_l) + ((1 << log_l) >> 4)) * sizeof(float2); }
-constexpr int kBpSmallLogL = 13;      // size classes: L <= 8192 (69.6 KB of shared memory: two CTAs per SM) and L = 16384
+constexpr int kTwLo = 128;            // e^{2 pi i t/L} = TWH[t >> 7] * TWL[t & 127]: two small shared tables instead of one
+                                      // scattered 8-byte global load per twiddle (every lane in its own sector)
+constexpr size_t bp_smem(int log_l) {
+  return (size_t)((1 << log_l) + ((1 << log_l) >> 4) + kTwLo + ((1 << log_l) / kTwLo)) * sizeof(float2);
+}
 
 template <int LOG_L>
-__device__ __forceinline__ void bandpower_body(float2* __restrict__ sm, const float2* __restrict__ tw_l,
-                                               const float2* __restrict__ qband, int B, float2* __restrict__ wout) {
+struct BpTw {
+  const float2* hi;                   // [L / 128]  e^{2 pi i 128 t/L}
+  const float2* lo;                   // [128]      e^{2 pi i t/L}
+  __device__ __forceinline__ float2 operator()(int t) const {      // t already reduced mod L
+    return cmul(hi[t >> 7], lo[t & (kTwLo - 1)]);
+  }
+};
+
+// grid (p, templates of the batch), one kernel per coarse-grid size L = 2^LOG_L (a CTA whose band wants another size
+// exits at once): W[tb][l][m] = one-sided power spectrum of class-S band l, 0 <= m < B_l.
+template <int LOG_L>
+__global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
+    k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q, const float2* __restrict__ tw_l,
+                float2* __restrict__ wbuf, int p, int half_n) {
   constexpr int L = 1 << LOG_L;
   constexpr int R3 = L / 1024;                    // last radix: 2, 4, 8, 16
   constexpr int S1 = L / 32;                      // stride of the first radix-32 stage
   constexpr int TWS = kLMax / L;                  // tw_l[t * TWS] = e^{2 pi i t / L}
+  extern __shared__ __align__(16) float2 sm[];
+  const int l = blockIdx.x, tb = blockIdx.y;
+  const TemplateMeta* mt = meta + tb;
+  if (!((mt->s_mask >> l) & 1u)) return;
+  const int e_lo = mt->edges[l], B = mt->edges[l + 1] - e_lo;
+  int log_l = kLogLMin;
+  while ((1 << log_l) < 2 * B) ++log_l;
+  if (log_l != LOG_L) return;
+  const float2* __restrict__ qband = q + (size_t)tb * half_n + e_lo;
+  float2* __restrict__ wout = wbuf + ((size_t)tb * p + l) * kUCap;
   const int tid = threadIdx.x;
+  float2* twl = sm + L + (L >> 4);
+  float2* twh = twl + kTwLo;
+  for (int i = tid; i < kTwLo; i += kBpThreads) twl[i] = tw_l[i * TWS];
+  for (int i = tid; i < L / kTwLo; i += kBpThreads) twh[i] = tw_l[i * kTwLo * TWS];
+  BpTw<LOG_L> tw;
+  tw.hi = twh;
+  tw.lo = twl;
 
   for (int i = tid; i < L; i += kBpThreads) sm[pad16(i)] = i < B ? qband[i] : make_float2(0.f, 0.f);
   __syncthreads();
   // ---- inverse transform, decimation in frequency: stage 1 (inputs i >= L/2 are zero since L >= 2B)
+#pragma unroll 1
   for (int o = tid; o < S1; o += kBpThreads) {
     float2 x[32];
 #pragma unroll
-    for (int q = 0; q < 16; ++q) x[brev<32>(q)] = sm[pad16(o + S1 * q)];
+    for (int qq = 0; qq < 16; ++qq) x[brev<32>(qq)] = sm[pad16(o + S1 * qq)];
     fft_dit<32, 16>(x);
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = cmul(x[k], tw_l[((o * k) & (L - 1)) * TWS]);
+    for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = k == 0 ? x[0] : cmul(x[k], tw((o * k) & (L - 1)));
   }
   __syncthreads();
   // ---- stage 2: inside each block k1 of S1 = 32 R3 points
+#pragma unroll 1
   for (int g = tid; g < S1; g += kBpThreads) {
     const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
     float2 x[32];
 #pragma unroll
-    for (int q = 0; q < 32; ++q) x[brev<32>(q)] = sm[pad16(base + R3 * q)];
+    for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pad16(base + R3 * qq)];
     fft_dit<32>(x);
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = cmul(x[k], tw_l[((32 * o2 * k) & (L - 1)) * TWS]);
+    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = k == 0 ? x[0] : cmul(x[k], tw((32 * o2 * k) & (L - 1)));
   }
   __syncthreads();
   // ---- stage 3 (R3 points, stride 1), |y|^2, and the first stage of the way back (same groups, no twiddle)
+#pragma unroll 1
   for (int g = tid; g < 1024; g += kBpThreads) {
     const int base = g * R3;
     float2 x[R3];
 #pragma unroll
-    for (int q = 0; q < R3; ++q) x[brev<R3>(q)] = sm[pad16(base + q)];
+    for (int qq = 0; qq < R3; ++qq) x[brev<R3>(qq)] = sm[pad16(base + qq)];
     fft_dit<R3>(x);
     float2 w[R3];
 #pragma unroll
-    for (int q = 0; q < R3; ++q) w[brev<R3>(q)] = make_float2(fmaf(x[q].x, x[q].x, x[q].y * x[q].y), 0.f);
+    for (int qq = 0; qq < R3; ++qq) w[brev<R3>(qq)] = make_float2(fmaf(x[qq].x, x[qq].x, x[qq].y * x[qq].y), 0.f);
     fft_dit<R3>(w);
 #pragma unroll
     for (int k = 0; k < R3; ++k) sm[pad16(base + k)] = w[k];
   }
   __syncthreads();
   // ---- decimation in time: twiddle first, then the radix-32 transform (transposes of stages 2 and 1)
+#pragma unroll 1
   for (int g = tid; g < S1; g += kBpThreads) {
     const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
     float2 x[32];
 #pragma unroll
-    for (int q = 0; q < 32; ++q) x[brev<32>(q)] = cmul(sm[pad16(base + R3 * q)], tw_l[((32 * o2 * q) & (L - 1)) * TWS]);
+    for (int qq = 0; qq < 32; ++qq) {
+      const float2 v = sm[pad16(base + R3 * qq)];
+      x[brev<32>(qq)] = qq == 0 ? v : cmul(v, tw((32 * o2 * qq) & (L - 1)));
+    }
     fft_dit<32>(x);
 #pragma unroll
     for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = x[k];
@@ -90,10 +129,14 @@ __device__ __forceinline__ void bandpower_body(float2* __restrict__ sm, const fl
   __syncthreads();
   // last stage: only the outputs m = o + S1 k < B <= L/2 are wanted, i.e. k < 16; they leave straight to global memory
   const float inv_l = 1.0f / (float)L;
+#pragma unroll 1
   for (int o = tid; o < S1; o += kBpThreads) {
     float2 x[32];
 #pragma unroll
-    for (int q = 0; q < 32; ++q) x[brev<32>(q)] = cmul(sm[pad16(o + S1 * q)], tw_l[((o * q) & (L - 1)) * TWS]);
+    for (int qq = 0; qq < 32; ++qq) {
+      const float2 v = sm[pad16(o + S1 * qq)];
+      x[brev<32>(qq)] = qq == 0 ? v : cmul(v, tw((o * qq) & (L - 1)));
+    }
     fft_dit<32>(x);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
@@ -102,34 +145,6 @@ __device__ __forceinline__ void bandpower_body(float2* __restrict__ sm, const fl
         const float sc = m == 0 ? inv_l : 2.0f * inv_l;                  // one-sided: U+[m] = 2 U[m] for m > 0
         wout[m] = make_float2(x[k].x * sc, -x[k].y * sc);               // conj: forward transform of a real series
       }
-    }
-  }
-}
-
-// grid (p, templates of the batch): W[tb][l][m] = one-sided power spectrum of class-S band l, 0 <= m < B_l.
-// Two launches per batch, one per size class (LARGE = the 16384-point grid): a CTA whose band belongs to the other
-// class exits at once, so that the small class is not held to one CTA per SM by the large one's shared memory.
-template <bool LARGE>
-__global__ void __launch_bounds__(kBpThreads, 2) k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q,
-                                                             const float2* __restrict__ tw_l, float2* __restrict__ wbuf,
-                                                             int p, int half_n) {
-  extern __shared__ __align__(16) float2 sm_bp[];
-  const int l = blockIdx.x, tb = blockIdx.y;
-  const TemplateMeta* m = meta + tb;
-  if (!((m->s_mask >> l) & 1u)) return;
-  const int e_lo = m->edges[l], B = m->edges[l + 1] - e_lo;
-  int log_l = kLogLMin;
-  while ((1 << log_l) < 2 * B) ++log_l;
-  if ((log_l > kBpSmallLogL) != LARGE) return;
-  const float2* qband = q + (size_t)tb * half_n + e_lo;
-  float2* wout = wbuf + ((size_t)tb * p + l) * kUCap;
-  if constexpr (LARGE) {
-    bandpower_body<14>(sm_bp, tw_l, qband, B, wout);
-  } else {
-    switch (log_l) {
-      case 11: bandpower_body<11>(sm_bp, tw_l, qband, B, wout); break;
-      case 12: bandpower_body<12>(sm_bp, tw_l, qband, B, wout); break;
-      default: bandpower_body<13>(sm_bp, tw_l, qband, B, wout); break;
     }
   }
 }
@@ -155,8 +170,10 @@ __global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ 
 }
 
 cudaError_t configure_bandpower() {
-  cudaError_t e = cudaFuncSetAttribute(k_bandpower<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(kBpSmallLogL));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(14));
+  cudaError_t e = cudaFuncSetAttribute(k_bandpower<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(11));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(12));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(13));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<14>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(14));
   return e;
 }
 
@@ -168,13 +185,15 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
   float2* wbuf = ws_ptr<float2>(c, c->lay.wbuf) + (size_t)parity * c->lay.batch * p * kUCap;
   float2* ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
   const float2* tw_l = ws_ptr<float2>(c, c->lay.tw_l);
-  k_bandpower<false><<<dim3(p, count), kBpThreads, bp_smem(kBpSmallLogL), st>>>(meta, q, tw_l, wbuf, p, (int)half);
-  if (c->s_bins > (1 << (kBpSmallLogL - 1))) {      // bands of more than 4096 bins exist only if the class allows them
-    k_bandpower<true><<<dim3(p, count), kBpThreads, bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half);
-    c->launches++;
-  }
+  const dim3 grid(p, count);
+  // one launch per coarse-grid size that the class threshold allows (a band of B bins uses L = 2^ceil(log2 2B) >= 2048)
+  k_bandpower<11><<<grid, kBpThreads, bp_smem(11), st>>>(meta, q, tw_l, wbuf, p, (int)half);
+  c->launches++;
+  if (c->s_bins > 1024) { k_bandpower<12><<<grid, kBpThreads, bp_smem(12), st>>>(meta, q, tw_l, wbuf, p, (int)half); c->launches++; }
+  if (c->s_bins > 2048) { k_bandpower<13><<<grid, kBpThreads, bp_smem(13), st>>>(meta, q, tw_l, wbuf, p, (int)half); c->launches++; }
+  if (c->s_bins > 4096) { k_bandpower<14><<<grid, kBpThreads, bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half); c->launches++; }
   k_uspec<<<dim3(c->s_bins / 256, count), 256, 0, st>>>(meta, wbuf, ubuf, p);
-  c->launches += 2;
+  c->launches++;
   return cudaGetLastError();
 }
 

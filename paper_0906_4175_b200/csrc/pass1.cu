@@ -402,47 +402,31 @@ __device__ __forceinline__ void eff_request_round(const EffSrc& es, float2* stag
   cp_async_commit();
 }
 
-// TW[i] = e^{2 pi i ja (row_lo + i)/n1} (shared, CTA constant).  The column part e^{2 pi i ja k2/n} of the twiddle is
-// split off: its m part rides on the T1 table (built per CTA), its c part on the per-thread twiddle of phase 2.
-template <int RMAX, bool HOLES>
-__device__ __forceinline__ void eff_phase1(const EffSrc& es, const float2* __restrict__ T1, const float2* __restrict__ TW,
-                                           float2* __restrict__ tile, float2* stage_col, tw4 g, int T, int row_lo, int k2,
-                                           int fr, int lr, int m, int ci) {
-  float2 v[32];
-  cp_async_wait_all();                                             // round T-1 has landed (own column only)
-  if constexpr (RMAX < 32) {
-#pragma unroll
-    for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(stage_col[i * 256], TW[i]);
-  } else {
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[brev<32>(i)] = stage_col[i * 256];
-#pragma unroll 1
-    for (int t = T - 2; t >= 0; --t) {
-      eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * t, k2, fr, lr);
-      cp_async_wait_all();
-#pragma unroll
-      for (int i = 0; i < 32; ++i) {
-        const float2 val = stage_col[i * 256];
-        const float2 w = v[brev<32>(i)];
-        v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[brev<32>(i)] = cmul(v[brev<32>(i)], TW[i]);
+// Plain (register) load of the same element, for the round that is requested first of all, while the registers of
+// the transform are still free.
+template <bool HOLES>
+__device__ __forceinline__ float2 eff_load(const EffSrc& es, int k1, int k2, int fr, int lr) {
+  const int k = (k1 << kLogN2) + k2;
+  bool ok = k1 >= fr && k1 <= lr;
+  if constexpr (HOLES) {
+    for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
   }
-  fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
-  __syncthreads();                          // every thread has consumed its staged inputs: the tile may be written
-  const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
-#pragma unroll
-  for (int jb = 0; jb < 32; jb += 2) {
-    const float4 w = t1[jb >> 1];
-    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], make_float2(w.x, w.y));
-    tile[(jb + 1) * kTileStride + m * 8 + ci] = cmul(v[jb + 1], make_float2(w.z, w.w));
-  }
+  float2 val = make_float2(0.f, 0.f);
+  if (ok) val = __ldg(es.src + k);
+  return val;
 }
 
-template <bool HOLES>
-__device__ __forceinline__ void eff_cta(const P1Args& a, const EffSrc& es, float2* tile, float2* T1, float2* TW, int ja, int cg) {
+// Phase 1 of a CTA: thread (m, ci) owns column k2 and forms, for every residue b' = (k1 - row_lo) mod 32,
+//     v[b'] = TW[b'] sum_t X[row_lo + b' + 32 t][k2] g^t        (Horner, g = e^{2 pi i ja/NA})
+// then the 32-point transform over b', the T1 twiddle, and writes its column of the exchange tile.
+// TW[i] = e^{2 pi i ja (row_lo + i)/n1} (shared, CTA constant).  The column part e^{2 pi i ja k2/n} of the twiddle is
+// split off: its m part rides on the T1 table (built per CTA), its c part on the per-thread twiddle of phase 2.
+// Latency: round t = 0 is loaded straight into the registers v[] at the very top (they are free until the transform),
+// the last round t = T-1 (if T > 1) goes through cp.async into the staging area at the same time; both are in flight
+// while the CTA builds its tables.  Only bands of more than 64 rows have further rounds, requested one after the other.
+template <int RMAX, bool HOLES>
+__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, float2* __restrict__ T1, float2* __restrict__ TW,
+                                           float2* __restrict__ tile, int ja, int cg) {
   const int tid = threadIdx.x;
   const unsigned nmask = (1u << a.log_n) - 1u;
   const int n1m = a.n1 - 1;
@@ -454,31 +438,65 @@ __device__ __forceinline__ void eff_cta(const P1Args& a, const EffSrc& es, float
   const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);
   const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
   float2* stage_col = tile + tid;               // [i][256]: column tid = m * 8 + ci of the staging area
-  const int rmax = R <= 4 ? 4 : R <= 8 ? 8 : R <= 16 ? 16 : 32;
-  // ---- request the first round of inputs, then build the tables while they are in flight
-  if (rmax == 4) eff_request_round<4, HOLES>(es, stage_col, row_lo, k2, fr, lr);
-  else if (rmax == 8) eff_request_round<8, HOLES>(es, stage_col, row_lo, k2, fr, lr);
-  else if (rmax == 16) eff_request_round<16, HOLES>(es, stage_col, row_lo, k2, fr, lr);
-  else eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * (T - 1), k2, fr, lr);
-  {
-    // T1 row m for jb = 4 ci .. 4 ci + 3, times this thread's m part of the column twiddle, e^{2 pi i ja 32 m/n}
-    const float2 Am = cis_frac(((unsigned)ja * 32u * (unsigned)m) & nmask, a.log_n);
-    const float4* src4 = reinterpret_cast<const float4*>(a.tw_p2 + m * 32 + 4 * ci);
-    const float4 w0 = __ldg(src4), w1 = __ldg(src4 + 1);
-    float4* dst = reinterpret_cast<float4*>(T1 + m * kT1Stride + 4 * ci);
-    const float2 p0 = cmul(make_float2(w0.x, w0.y), Am), p1 = cmul(make_float2(w0.z, w0.w), Am);
-    const float2 p2 = cmul(make_float2(w1.x, w1.y), Am), p3 = cmul(make_float2(w1.z, w1.w), Am);
-    dst[0] = make_float4(p0.x, p0.y, p1.x, p1.y);
-    dst[1] = make_float4(p2.x, p2.y, p3.x, p3.y);
+
+  float2 v[32];
+  const bool preload = RMAX < 32 || T <= 2;     // CTA-uniform
+  if (preload) {
+#pragma unroll
+    for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = eff_load<HOLES>(es, row_lo + i, k2, fr, lr);        // round 0
+  }
+  if constexpr (RMAX == 32) {
+    if (T > 1) eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * (T - 1), k2, fr, lr);          // round T-1
   }
   if (tid < 32) TW[tid] = a.tw_n1[(ja * (row_lo + tid)) & n1m];
-  const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                           // e^{2 pi i ja/NA}
-  __syncthreads();
-  // ---- phase 1: thread (m, ci), column k2
-  if (rmax == 4) eff_phase1<4, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
-  else if (rmax == 8) eff_phase1<8, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
-  else if (rmax == 16) eff_phase1<16, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
-  else eff_phase1<32, HOLES>(es, T1, TW, tile, stage_col, g, T, row_lo, k2, fr, lr, m, ci);
+  __syncthreads();                              // T1 (built by the caller before the slot was known) and TW are ready
+
+  if constexpr (RMAX == 32) {
+    if (T > 1) {
+      const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                          // e^{2 pi i ja/NA}
+      cp_async_wait_all();                                                       // round T-1 has landed (own column only)
+      if (preload) {                                                             // T == 2: v = stage g + v
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          const float2 hi = stage_col[i * 256], val = v[brev<32>(i)];
+          v[brev<32>(i)] = unpk(fma2(pk(-hi.y, hi.x), g.yy, fma2(pk(hi), g.xx, pk(val))));
+        }
+      } else {                                                                   // more than 64 rows: round after round
+#pragma unroll
+        for (int i = 0; i < 32; ++i) v[brev<32>(i)] = stage_col[i * 256];
+#pragma unroll 1
+        for (int t = T - 2; t >= 0; --t) {
+          eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * t, k2, fr, lr);
+          cp_async_wait_all();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float2 val = stage_col[i * 256], w = v[brev<32>(i)];
+            v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
+          }
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(v[brev<32>(i)], TW[i]);
+  fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
+  if constexpr (RMAX == 32) __syncthreads();   // every thread has consumed its staged inputs: the tile may be written
+  const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
+#pragma unroll
+  for (int jb = 0; jb < 32; jb += 2) {
+    const float4 w = t1[jb >> 1];
+    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], make_float2(w.x, w.y));
+    tile[(jb + 1) * kTileStride + m * 8 + ci] = cmul(v[jb + 1], make_float2(w.z, w.w));
+  }
+}
+
+template <bool HOLES>
+__device__ __forceinline__ void eff_cta(const P1Args& a, const EffSrc& es, float2* tile, float2* T1, float2* TW, int ja, int cg) {
+  const int R = ((es.e_hi - 1) >> kLogN2) - (es.e_lo >> kLogN2) + 1;
+  if (R <= 4) eff_phase1<4, HOLES>(a, es, T1, TW, tile, ja, cg);
+  else if (R <= 8) eff_phase1<8, HOLES>(a, es, T1, TW, tile, ja, cg);
+  else if (R <= 16) eff_phase1<16, HOLES>(a, es, T1, TW, tile, ja, cg);
+  else eff_phase1<32, HOLES>(a, es, T1, TW, tile, ja, cg);
 }
 
 __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
@@ -495,6 +513,19 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
   const unsigned nmask = (1u << a.log_n) - 1u;
 
   const SlotDesc d = slot_tab[a.slot_base + slot];      // one 32-byte load, same address in every thread
+  {
+    // While the descriptor is on its way: T1 row m for jb = 4 ci .. 4 ci + 3 times this thread's m part of the column
+    // twiddle, e^{2 pi i ja 32 m/n} (depends on ja only)
+    const int ci = tid & 7, m = tid >> 3;
+    const float2 Am = cis_frac(((unsigned)ja * 32u * (unsigned)m) & nmask, a.log_n);
+    const float4* src4 = reinterpret_cast<const float4*>(a.tw_p2 + m * 32 + 4 * ci);
+    const float4 w0 = __ldg(src4), w1 = __ldg(src4 + 1);
+    float4* dst = reinterpret_cast<float4*>(T1 + m * kT1Stride + 4 * ci);
+    const float2 p0 = cmul(make_float2(w0.x, w0.y), Am), p1 = cmul(make_float2(w0.z, w0.w), Am);
+    const float2 p2 = cmul(make_float2(w1.x, w1.y), Am), p3 = cmul(make_float2(w1.z, w1.w), Am);
+    dst[0] = make_float4(p0.x, p0.y, p1.x, p1.y);
+    dst[1] = make_float4(p2.x, p2.y, p3.x, p3.y);
+  }
   if (d.generic) return;                        // very many rows: k_pass1 (generic) + k_rowstage write this slot
   const int tb = d.t - a.first_template;
 
