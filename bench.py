@@ -262,14 +262,15 @@ def spawn_ranks(args) -> int:
     return subprocess.call(cmd)
 
 
-STAGES = ("spectra", "pass1", "pass2")
+STAGES = ("spectra", "pass1", "pass2", "chisq_at_events")
 STAGE_TEXT = {
     "decimated": {
         "spectra": "k_correlate + k_bandpower + k_uspec (template phasors x data, coarse-grid band powers, U+); timed "
                    "serialised, run beside pass 1 on a side stream in gwmf_filter",
         "pass1": "k_pass1_eff (first FFT pass of every effective band: writes n complex fp32 per n-point transform) "
                  "[+ generic kernel + row stage for bands of > 512 input rows]",
-        "pass2": "k_pass2_eff (last FFT stage + rho/chi^2/trigger epilogue: reads n complex fp32 per n-point transform)"},
+        "pass2": "k_pass2_eff (last FFT stage + rho/chi^2/trigger epilogue: reads n complex fp32 per n-point transform)",
+        "chisq_at_events": "k_chisq_at (chi^2 on demand: Eq. 5 evaluated from its definition at every event's sample)"},
     "two_pass": {
         "spectra": "-",
         "pass1": "k_pass1_narrow (pruned column FFT + first row stage, writes p*N*8 B/template) with the low-volume kernels "
@@ -330,7 +331,8 @@ def run_gpu(args):
     Sn = w.psd
     T = len(w.masses)
 
-    f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}", path=args.path, batch=args.batch)
+    f = gwmf.Filter(w.n, w.p, w.window, T, rho_thresh=w.rho_thresh, device=f"cuda:{local}", path=args.path, batch=args.batch,
+                    chisq_on_demand=args.chisq_on_demand)
     path = f.path
     f.make_bank(w.masses)
     segs_dev = [torch.from_numpy(sg).to(dev) for sg in segs]
@@ -370,8 +372,8 @@ def run_gpu(args):
 
     # per-stage device times (events inside the library, on its stream, stages serialised)
     reps = 3
-    k_ms = np.zeros(3)
-    k_launch = np.zeros(3)
+    k_ms = np.zeros(4)
+    k_launch = np.zeros(4)
     for _ in range(reps):
         m3, n3 = f.filter_timed(first, count)
         k_ms += m3
@@ -419,6 +421,9 @@ def run_gpu(args):
     if rank == 0:
         line = base_line(args, w, value, ms / args.steps, "f32")
         line["config"]["path"] = path
+        if args.chisq_on_demand:
+            line["metric"] += " -- chi^2 ON DEMAND (evaluated at the event samples only; not the headline workload)"
+            line["config"]["chisq_mode"] = "on_demand"
         if nseg > 1:
             line["roofline_note"] = "per-stage times and bytes below are those of ONE segment (gwmf_filter_timed)"
         line["config"]["batch_templates_per_launch"] = float(count / max(k_launch[2], 1))
@@ -445,7 +450,7 @@ def run_gpu(args):
                 continue
             ent = {"kernel": STAGE_TEXT[path][st], "ms_per_step": float(k_ms[i]), "avg_launch_ms": float(k_ms[i] / k_launch[i]),
                    "share_of_step": float(k_ms[i] / k_ms.sum())}
-            if st != "spectra" and path != "fused":
+            if st in ("pass1", "pass2") and path != "fused":
                 ent["GB/s"] = bytes_step / (k_ms[i] * 1e-3) / 1e9
                 ent["frac"] = ent["GB/s"] / peak
             kernels[st] = ent
@@ -510,6 +515,9 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "two_pass", "fused", "decimated"],
                     help="gwmf_params::path: auto = the library's choice (decimated for n >= 2^15)")
     ap.add_argument("--batch", type=int, default=0, help="templates per launch (0 = library default)")
+    ap.add_argument("--chisq-on-demand", action="store_true",
+                    help="gwmf_params::chisq_mode = ON_DEMAND: one full-band transform per template, chi^2 evaluated only at "
+                         "the event samples (SURVEY.md 8(f)-2; a different workload from the headline's chi^2(t) at every sample)")
     ap.add_argument("--shard", default="segments", choices=["segments", "templates"],
                     help="N > 1: segments = every rank filters the whole bank against its own segment (weak scaling); "
                          "templates = one segment, the bank split by template id, events gathered (strong scaling)")

@@ -59,6 +59,17 @@ typedef enum {
   GWMF_PATH_DECIMATED = 3
 } gwmf_path;
 
+/* Where chi^2 is evaluated.  EVERY_SAMPLE: chi^2(t) at all n samples (the paper's pipeline; needed
+ * for gwmf_series).  ON_DEMAND (the pipeline with the chi^2 loop taken out of the
+ * hot path): one full-band transform per template gives rho(t) and the events; chi^2 is then evaluated only at each
+ * event's sample, directly from its definition z_l[j] = sum_{k in band l} Q[k] e^{2 pi i jk/n} (one pass over the
+ * template's bins per event).  The events carry the same rho, sample and chi^2 up to fp32 rounding.  Decimated path
+ * only; gwmf_series then returns rho(t) and leaves chi^2(t) = 0. */
+typedef enum {
+  GWMF_CHISQ_EVERY_SAMPLE = 0,
+  GWMF_CHISQ_ON_DEMAND = 1
+} gwmf_chisq_mode;
+
 typedef struct gwmf_ctx gwmf_ctx;                      /* opaque */
 
 typedef struct { double m1, m2; } gwmf_mass_pair;      /* solar masses, > 0, any order */
@@ -84,6 +95,7 @@ typedef struct {
                             to 64 templates per launch, as many as fit in it (it needs ~3, not p, transforms each) */
   int32_t path;          /* a gwmf_path; GWMF_PATH_AUTO (0) = the library's choice.  A path that does not support n
                             (FUSED: 2^15 .. 2^20, DECIMATED: >= 2^15) is GWMF_E_ARG                               */
+  int32_t chisq_mode;    /* a gwmf_chisq_mode; ON_DEMAND needs the decimated path (n >= 2^15), else GWMF_E_ARG     */
 } gwmf_params;
 
 /* Bytes of DEVICE memory the caller must provide to gwmf_create (0 if params are invalid). */
@@ -129,15 +141,16 @@ int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn);
  * maxima above threshold.  Trigger slots of those templates are reset first.  async. */
 int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
 
-/* Measurement: the same work as gwmf_filter, with CUDA events recorded on the context's stream around the three
- * stages of every batch.  host_ms: HOST array of 3 doubles, summed device time (ms) of
+/* Measurement: the same work as gwmf_filter, with CUDA events recorded on the context's stream around the
+ * stages of every batch.  host_ms: HOST array of 4 doubles, summed device time (ms) of
  *   [0] the spectra of the decimated path (correlate, coarse-grid band powers, U+), serialised on the main stream
  *       for this call (gwmf_filter runs them beside pass 1 on a side stream); 0 for the other paths, whose
  *       correlate step is inside [1];
  *   [1] pass 1: first FFT pass of every (effective) band -> band intermediate in HBM; for the spill-free path only
  *       the wide bands' kernels;
- *   [2] pass 2: last FFT stage + rho/chi^2/trigger epilogue (spill-free path: k_fused).
- * host_launches: HOST array of 3 int32, batches timed in each stage.  syncs. */
+ *   [2] pass 2: last FFT stage + rho/chi^2/trigger epilogue (spill-free path: k_fused);
+ *   [3] chi^2 at the event samples (chisq_mode = ON_DEMAND only, else 0).
+ * host_launches: HOST array of 4 int32, launches / batches timed in each stage.  syncs. */
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
                       int32_t* host_launches);
 

@@ -29,6 +29,9 @@ bool params_ok(const gwmf_params* p) {
   if (p->path < GWMF_PATH_AUTO || p->path > GWMF_PATH_DECIMATED) return false;
   if (p->path == GWMF_PATH_FUSED && (p->n < (1 << 15) || p->n > (1 << 20))) return false;
   if (p->path == GWMF_PATH_DECIMATED && p->n < (1 << 15)) return false;
+  if (p->chisq_mode != GWMF_CHISQ_EVERY_SAMPLE && p->chisq_mode != GWMF_CHISQ_ON_DEMAND) return false;
+  if (p->chisq_mode == GWMF_CHISQ_ON_DEMAND && (p->n < (1 << 15) || (p->path != GWMF_PATH_AUTO && p->path != GWMF_PATH_DECIMATED)))
+    return false;
   return true;
 }
 
@@ -384,7 +387,7 @@ static int ensure_mirror(Ctx* c) {
 // Q, W_l and U+ of a batch (decimated path), on stream st
 static cudaError_t launch_spectra(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   cudaError_t e = launch_correlate(c, first, count, parity, st);
-  if (e == cudaSuccess) e = launch_bandpower(c, first, count, parity, st);
+  if (e == cudaSuccess && c->prm.chisq_mode != GWMF_CHISQ_ON_DEMAND) e = launch_bandpower(c, first, count, parity, st);
   return e;
 }
 
@@ -475,6 +478,11 @@ static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t*
     }
     f0 += cnt;
   }
+  if (c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND) {
+    if (ev) CU(cudaEventRecord(ev[4 * counts.size()], c->stream));
+    CU(launch_chisq_at_events(c, first_template, n_templates));
+    if (ev) CU(cudaEventRecord(ev[4 * counts.size() + 1], c->stream));
+  }
   return end_segment_use(c);
 }
 
@@ -513,7 +521,7 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
     std::vector<cudaEvent_t> v;
     ~Events() { for (cudaEvent_t e : v) if (e) cudaEventDestroy(e); }
   } ev;
-  ev.v.assign((size_t)nb * 4, nullptr);
+  ev.v.assign((size_t)nb * 4 + 2, nullptr);
   for (auto& e : ev.v) CU(cudaEventCreate(&e));
   rc = run_batches(c, first_template, n_templates, ev.v.data(), counts);
   if (rc != GWMF_OK) return rc;
@@ -527,6 +535,14 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
     }
   host_launches[0] = c->path == GWMF_PATH_DECIMATED ? nb : 0;
   host_launches[1] = host_launches[2] = nb;
+  host_ms[3] = 0.0;
+  host_launches[3] = 0;
+  if (c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND) {
+    float m = 0.f;
+    CU(cudaEventElapsedTime(&m, ev.v[4 * nb], ev.v[4 * nb + 1]));
+    host_ms[3] = m;
+    host_launches[3] = 1;
+  }
   return GWMF_OK;
 }
 
@@ -629,7 +645,9 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
   if (rc != GWMF_OK) return rc;
   if ((rc = begin_segment_use(c)) != GWMF_OK) return rc;
   if (c->path == GWMF_PATH_DECIMATED) {
-    CU(decimated_batch(c, template_id, 1, 0, 0, 0, false, false, d_rho, d_chi, nullptr));
+    const bool on_demand = c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND;          // no chi^2(t) series in that mode
+    if (on_demand) CU(cudaMemsetAsync(d_chi, 0, sizeof(float) * (size_t)c->n, c->stream));
+    CU(decimated_batch(c, template_id, 1, 0, 0, 0, false, false, d_rho, on_demand ? nullptr : d_chi, nullptr));
   } else {
     CU(launch_pass1_filter(c, template_id, 1, 0, 0, 0, false));
     if (c->fused) CU(launch_fused_filter(c, template_id, 1, 0, false, d_rho, d_chi));

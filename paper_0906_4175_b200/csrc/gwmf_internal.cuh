@@ -41,6 +41,7 @@ struct TemplateMeta {
   int32_t n_eff;                 // effective bands of this template
   int32_t z_lo, z_hi;            // hull of the class-S bands, bins [z_lo, z_hi)
   int32_t u_hi;                  // support of U+: bins [0, u_hi), u_hi = widest class-S band
+  int32_t full_band;             // chi^2 on demand: the ONE effective band is the whole template [edges[0], k_high)
 };
 
 // One effective band: which spectrum it reads (kind) and the bins [e_lo, e_hi) it owns.
@@ -59,6 +60,7 @@ struct alignas(32) SlotDesc {
 #ifdef __CUDACC__
 __device__ __forceinline__ EffBand eff_band(const TemplateMeta* m, int e) {
   EffBand b;
+  if (m->full_band) { b.kind = kEffD; b.e_lo = m->edges[0]; b.e_hi = m->k_high; b.l = -1; return b; }
   if (m->s_mask) {
     if (e == 0) { b.kind = kEffZ; b.e_lo = m->z_lo; b.e_hi = m->z_hi; b.l = -1; return b; }
     if (e == 1) { b.kind = kEffU; b.e_lo = 0; b.e_hi = m->u_hi; b.l = -1; return b; }
@@ -164,6 +166,7 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
 cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
 cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
 cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi);
+cudaError_t launch_chisq_at_events(Ctx* c, int first, int count);      // chi^2 on demand: fills the slots' chi^2
 cudaError_t launch_reset_slots(Ctx* c, int first, int count);
 cudaError_t launch_compact(Ctx* c);
 

@@ -182,7 +182,8 @@ cudaError_t launch_weighted_spectrum(Ctx* c, int buf, cudaStream_t st) {
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ meta, uint32_t* __restrict__ masks,
                                                     const double* __restrict__ c_tab, int n_templates, int p, int k_low,
-                                                    int half_n, double four_df, int all_wide, int s_bins, int t_max) {
+                                                    int half_n, double four_df, int all_wide, int s_bins, int t_max,
+                                                    int on_demand) {
   // thread (l = threadIdx.x, template = 8 blockIdx.x + threadIdx.y): one band edge each, then the wide-band mask
   __shared__ int s_edges[8][kMaxBands + 1];
   const int l = threadIdx.x, ty = threadIdx.y;
@@ -255,6 +256,16 @@ __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ m
       meta[t].z_lo = s_mask ? z_lo : 0;
       meta[t].z_hi = z_hi;
       meta[t].u_hi = u_hi;
+      meta[t].full_band = 0;
+      if (on_demand) {                          // one transform over the whole template; chi^2 comes later, per event
+        const int k0 = s_edges[ty][0];
+        const int rows_all = ((k_high - 1) >> kLogN2) - (k0 >> kLogN2) + 1;
+        meta[t].s_mask = 0;
+        meta[t].d_mask = 0;
+        meta[t].gen_mask = rows_all > 32 * t_max ? 1u : 0u;
+        meta[t].n_eff = 1;
+        meta[t].full_band = 1;
+      }
     }
   }
   if (l == 0) {
@@ -323,7 +334,8 @@ cudaError_t launch_bank_setup(Ctx* c) {
   const bool decim = c->path == GWMF_PATH_DECIMATED;
   k_bank_setup<<<(c->n_templates + 7) / 8, dim3(32, 8), 0, c->stream>>>(
       ws_ptr<TemplateMeta>(c, c->lay.meta), ws_ptr<uint32_t>(c, c->lay.masks), ws_ptr<double>(c, c->lay.c_tab),
-      c->n_templates, c->prm.p, c->k_low, (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1, decim ? c->s_bins : 0, c->t_max);
+      c->n_templates, c->prm.p, c->k_low, (int)(c->n / 2), 4.0 * c->df, c->nb == 32 ? 0 : 1, decim ? c->s_bins : 0, c->t_max,
+      c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND ? 1 : 0);
   c->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;

@@ -73,6 +73,79 @@ __global__ void __launch_bounds__(256) k_emit(const Slot* __restrict__ slots, co
   }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// chi^2 on demand (gwmf_params::chisq_mode = GWMF_CHISQ_ON_DEMAND).  The filter has left, per
+// (template, window), the maximum of rho and its sample j; chi^2 is wanted at that sample only (reading 12), so
+// it is evaluated from the definition, Eq. 5 with
+//     z_l[j] = sum_{k in band l} Q[k] e^{2 pi i jk/n},   Q[k] = wq[k] e^{i Psi0(f_k)}        (Eq. 1)
+// one CTA per event, one pass over the template's bins: the phasor exactly as in k_correlate (fp64 Horner, reduced to
+// one turn), the Fourier factor from jk mod n (exact in integers), fp32 sums per thread and a fixed-order block
+// reduction per band (bit-reproducible).  Cost O(k_high - k_low) per event against O(p n log n) per template.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_chisq_at(Slot* __restrict__ slots, const TemplateMeta* __restrict__ meta,
+                                                  const float2* __restrict__ wq, const double* __restrict__ u_tab, int p,
+                                                  int n_windows, int log_n) {
+  __shared__ float2 red[8];
+  __shared__ int s_edges[kMaxBands + 1];
+  const int t = blockIdx.y, w = blockIdx.x;
+  Slot* sl = slots + (size_t)t * n_windows + w;
+  const unsigned long long key = sl->key;
+  if (key == 0ull) return;                                    // no event in this window (uniform over the CTA)
+  const unsigned j = 0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull);
+  const TemplateMeta* m = meta + t;
+  if (threadIdx.x <= p) s_edges[threadIdx.x] = m->edges[threadIdx.x];
+  __syncthreads();
+  const unsigned nmask = (1u << log_n) - 1u;
+  const float inv_n2 = 2.0f / (float)(1u << log_n);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const double c0 = m->c0, c2 = m->c2, c3 = m->c3, c4 = m->c4;
+  float zx = 0.f, zy = 0.f, q = 0.f;                          // sum_l z_l and sum_l |z_l|^2 (thread 0)
+  for (int l = 0; l < p; ++l) {
+    float ax = 0.f, ay = 0.f;
+    for (int k = s_edges[l] + threadIdx.x; k < s_edges[l + 1]; k += 256) {
+      const double u = u_tab[k];
+      double ph = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
+      ph -= rint(ph);
+      // total angle in turns: Psi0/2pi + (jk mod n)/n, both in [-1/2, 1): one sincospif
+      const float turns = 2.0f * (float)ph + (float)((j * (unsigned)k) & nmask) * inv_n2;
+      float sn, cs;
+      sincospif(turns, &sn, &cs);
+      const float2 v = wq[k];
+      ax = fmaf(v.x, cs, fmaf(-v.y, sn, ax));
+      ay = fmaf(v.x, sn, fmaf(v.y, cs, ay));
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+      ax += __shfl_down_sync(0xFFFFFFFFu, ax, d);
+      ay += __shfl_down_sync(0xFFFFFFFFu, ay, d);
+    }
+    if (lane == 0) red[warp] = make_float2(ax, ay);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      float sx = 0.f, sy = 0.f;
+      for (int i = 0; i < 8; ++i) { sx += red[i].x; sy += red[i].y; }
+      zx += sx;
+      zy += sy;
+      q = fmaf(sx, sx, fmaf(sy, sy, q));
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const float z2 = fmaf(zx, zx, zy * zy);
+    const float chi = fmaxf(q - z2 / (float)p, 0.f) * ((float)p * m->scale_rho2);    // Eq. 5
+    sl->aux = (unsigned long long)__float_as_uint(chi);
+  }
+}
+
+cudaError_t launch_chisq_at_events(Ctx* c, int first, int count) {
+  if (count <= 0) return cudaSuccess;
+  k_chisq_at<<<dim3(c->n_windows, count), 256, 0, c->stream>>>(
+      ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows, ws_ptr<TemplateMeta>(c, c->lay.meta) + first,
+      wq_buf(c, c->front), ws_ptr<double>(c, c->lay.u_tab), c->prm.p, c->n_windows, c->log_n);
+  c->launches++;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_reset_slots(Ctx* c, int first, int count) {
   size_t n = (size_t)count * c->n_windows;
   if (n == 0) return cudaSuccess;

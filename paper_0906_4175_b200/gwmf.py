@@ -30,7 +30,7 @@ EXPORTS = [
 class Params(C.Structure):
     _fields_ = [("n", C.c_int64), ("fs", C.c_double), ("f_low", C.c_double), ("p", C.c_int32),
                 ("rho_thresh", C.c_double), ("window", C.c_int32), ("max_templates", C.c_int32),
-                ("batch", C.c_int32), ("path", C.c_int32)]
+                ("batch", C.c_int32), ("path", C.c_int32), ("chisq_mode", C.c_int32)]
 
 
 class MassPair(C.Structure):
@@ -87,9 +87,10 @@ def load_library():
     return L
 
 
-def workspace_bytes(n, p, window, max_templates, fs=4096.0, f_low=40.0, rho_thresh=6.0, batch=0, path="auto") -> int:
+def workspace_bytes(n, p, window, max_templates, fs=4096.0, f_low=40.0, rho_thresh=6.0, batch=0, path="auto",
+                    chisq_on_demand=False) -> int:
     prm = Params(int(n), float(fs), float(f_low), int(p), float(rho_thresh), int(window), int(max_templates), int(batch),
-                 PATHS[path])
+                 PATHS[path], 1 if chisq_on_demand else 0)
     return int(load_library().gwmf_workspace_bytes(C.byref(prm)))
 
 
@@ -97,7 +98,7 @@ class Filter:
     """One gwmf context: a device workspace, a stream, a bank and the current segment."""
 
     def __init__(self, n, p, window, max_templates, rho_thresh=6.0, fs=4096.0, f_low=40.0, batch=0,
-                 device="cuda:0", stream=None, path="auto"):
+                 device="cuda:0", stream=None, path="auto", chisq_on_demand=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("gwmf needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -106,7 +107,7 @@ class Filter:
         self.device = torch.device(device)
         self.n, self.p, self.window = int(n), int(p), int(window)
         self.params = Params(int(n), float(fs), float(f_low), int(p), float(rho_thresh), int(window),
-                             int(max_templates), int(batch), PATHS[path])
+                             int(max_templates), int(batch), PATHS[path], 1 if chisq_on_demand else 0)
         nbytes = int(self._L.gwmf_workspace_bytes(C.byref(self.params)))
         if nbytes == 0:
             raise GwmfError(E_ARG, "invalid parameters")
@@ -194,13 +195,13 @@ class Filter:
         self._check(self._L.gwmf_filter(self._h, int(first), int(count)))
 
     def filter_timed(self, first=0, count=None):
-        """As filter(), returning ((ms_spectra, ms_pass1, ms_pass2), (batches timed in each)); syncs."""
+        """As filter(), returning ((ms_spectra, ms_pass1, ms_pass2, ms_chisq_at_events), (launches timed in each)); syncs."""
         if count is None:
             count = self.n_templates - first
-        ms = (C.c_double * 3)()
-        nl = (C.c_int32 * 3)()
+        ms = (C.c_double * 4)()
+        nl = (C.c_int32 * 4)()
         self._check(self._L.gwmf_filter_timed(self._h, int(first), int(count), ms, nl))
-        return (ms[0], ms[1], ms[2]), (nl[0], nl[1], nl[2])
+        return tuple(ms), tuple(nl)
 
     def triggers(self, capacity=None) -> np.ndarray:
         if capacity is None:

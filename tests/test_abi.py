@@ -34,7 +34,7 @@ def test_header_symbols_exported(lib):
 
 def test_struct_layouts_match_header():
     from paper_0906_4175_b200 import gwmf
-    assert ctypes.sizeof(gwmf.Params) == 56       # int64, 2 doubles, int32(+pad), double, 3 int32 (+pad)
+    assert ctypes.sizeof(gwmf.Params) == 64       # int64, 2 doubles, int32(+pad), double, 5 int32 (+pad)
     assert ctypes.sizeof(gwmf.MassPair) == 16
     assert gwmf.TRIGGER_DTYPE.itemsize == 16
 
@@ -62,7 +62,7 @@ def test_null_arguments_are_rejected_without_a_gpu(lib):
     assert lib.gwmf_triggers(None, None, 0, ctypes.byref(n)) == -1
     h = ctypes.c_void_p()
     from paper_0906_4175_b200 import gwmf
-    prm = gwmf.Params(1 << 14, 4096.0, 40.0, 4, 6.0, 4096, 8, 0, 0)
+    prm = gwmf.Params(1 << 14, 4096.0, 40.0, 4, 6.0, 4096, 8, 0, 0, 0)
     assert lib.gwmf_create(ctypes.byref(prm), None, 0, None, ctypes.byref(h)) == -1     # no workspace
 
 

@@ -290,6 +290,37 @@ def test_config4_long_segment_64_templates(gw, ocache, path4):
         parity.assert_series(rho_g, chi_g, rho_o.astype(np.float64), chi_o.astype(np.float64), w.p, f"config 4 template {i}")
 
 
+@pytest.mark.parametrize("config", [1, 2])
+def test_chisq_on_demand_matches_oracle_and_every_sample_mode(gw, ocache, config):
+    # SURVEY 8(f)-2 / PAPER.md:164: rho(t) from ONE full-band transform per template, chi^2 evaluated from its
+    # definition at the event samples only.  Every event (rho, sample, chi^2) against the oracle over the whole bank,
+    # and against the chi^2-at-every-sample run of the same library.
+    w = inputs.workload(config)
+    s = inputs.segment(w).astype(np.float32)
+    s64 = s.astype(np.float64)
+    Sn = w.psd
+    out = ocache.bank_out(f"c{config}", s64, Sn, w.masses, w.p, w.window, w.rho_thresh)
+    f = gw.Filter(w.n, w.p, w.window, len(w.masses), rho_thresh=w.rho_thresh, chisq_on_demand=True)
+    f.make_bank(w.masses)
+    f.load_segment(s, Sn)
+    assert np.all(f.transform_counts() == 1)
+    f.filter()
+    trig = f.triggers()
+    compared, exempt = parity.assert_triggers(trig, out, w.rho_thresh, w.window, w.p)
+    assert compared >= 3
+    ref = _run_gpu(gw, w, s, Sn).triggers()
+    a = {(int(t["template_id"]), int(t["sample"])): t for t in trig}
+    b = {(int(t["template_id"]), int(t["sample"])): t for t in ref}
+    common = set(a) & set(b)
+    assert len(common) >= 0.98 * max(len(a), len(b))      # cells within fp32 rounding of the threshold / a tie may differ
+    for key in common:
+        assert abs(float(a[key]["rho"]) - float(b[key]["rho"])) <= 1e-4 * float(b[key]["rho"])
+        assert abs(float(a[key]["chisq"]) - float(b[key]["chisq"])) <= 1e-3 * float(b[key]["chisq"]) + 1e-3
+    rho_g, chi_g = f.series(3)                             # rho(t) is still available; chi^2(t) is not formed
+    rho_o, _ = ocache.template_series((f"c{config}", 3), s64, Sn, w.masses[3][0], w.masses[3][1], w.p)
+    assert np.max(np.abs(rho_g - rho_o) - (1e-3 + 1e-4 * rho_o)) <= 0 and np.all(chi_g == 0.0)
+
+
 def test_noise_statistics_at_full_size(gw):
     # in stationary Gaussian noise rho^2 is chi^2 with 2 degrees of freedom and the veto
     # statistic chi^2 with 2p - 2, whatever the template: properties that hold at any size, checked at the
