@@ -237,7 +237,10 @@ struct P2EArgs {
   int batch;
 };
 
-template <bool SERIES>
+// SINGLE: every template of the launch has exactly one effective band (p = 1, or chi^2 on demand): z is that band's
+// transform, no sums over bands are kept, and the epilogue is one compare of |z|^2 against the threshold per sample
+// (chi^2 is 0 by definition for p = 1 and is filled in later by k_chisq_at in the on-demand mode).
+template <bool SERIES, bool SINGLE>
 __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
   const P2Args& a = ea.b;
   extern __shared__ __align__(128) float2 smem2[];
@@ -315,6 +318,24 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
         if (lane == 0) prefetch();
         advance();
       }
+      if constexpr (SINGLE) {
+        // ---- the row's only band: epilogue straight from the transform (steps a4, a5 without chi^2) ----
+        const float scale = __ldg(&a.meta[tb].scale_rho2);
+        const float thr_z2 = a.thresh * a.thresh * 0.999f / scale;            // rho^2 > thr^2  <=>  |z|^2 > thr^2 / scale
+        Slot* slots_t = a.slots ? a.slots + (size_t)tb * a.n_windows : nullptr;
+#pragma unroll
+        for (int jc = 0; jc < 32; ++jc) {
+          const float z2 = fmaf(x[jc].x, x[jc].x, x[jc].y * x[jc].y);
+          if constexpr (SERIES) {
+            const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
+            if (a.series_rho) a.series_rho[j] = sqrtf(z2 * scale);
+            if (a.series_chi) a.series_chi[j] = 0.f;
+          }
+          if (z2 > thr_z2 && slots_t)
+            emit_candidate(slots_t, (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1), z2 * scale, 0.f, a.thresh, a.log_w);
+        }
+        continue;
+      }
       if (has_s && e == 0) {                    // Z
 #pragma unroll
         for (int jc = 0; jc < 32; ++jc) az[jc] = cadd(az[jc], x[jc]);
@@ -330,6 +351,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
         }
       }
     }
+    if constexpr (SINGLE) continue;
     // ---- epilogue of one row: rho, chi^2 and the trigger slots (steps a4, a5) ----
     const float scale = __ldg(&a.meta[tb].scale_rho2);
     const float fp_scale = (float)a.p * scale, inv_p = 1.0f / (float)a.p;
@@ -584,8 +606,10 @@ cudaError_t configure_pass2() {
   cudaError_t e = cudaFuncSetAttribute(k_pass2<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
   return e;
@@ -662,8 +686,13 @@ cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, fl
   a.thresh = (float)c->prm.rho_thresh;
   ea.slot_base = c->h_eff[first];
   ea.batch = count;
-  if (series_rho || series_chi) k_pass2_eff<true><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(ea);
-  else k_pass2_eff<false><<<p2_grid(c, a.n_rows), kP2Warps * 32, kP2Smem, c->stream>>>(ea);
+  const bool single = c->h_eff[first + count] - c->h_eff[first] == count;     // one effective band per template
+  const bool series = series_rho || series_chi;
+  const dim3 grid(p2_grid(c, a.n_rows));
+  if (single && series) k_pass2_eff<true, true><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
+  else if (single) k_pass2_eff<false, true><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
+  else if (series) k_pass2_eff<true, false><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
+  else k_pass2_eff<false, false><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
   c->launches++;
   return cudaGetLastError();
 }
