@@ -92,7 +92,8 @@ typedef struct {
   int32_t batch;         /* most templates filtered per kernel launch, 0 .. 64; sizes the band-intermediate
                             buffer, batch * p * n * 8 bytes, and the correlated spectra, 2 * batch * n * 4 bytes.
                             0 = library default: a band buffer of about 2 GiB; the decimated path then takes up
-                            to 64 templates per launch, as many as fit in it (it needs ~3, not p, transforms each) */
+                            to 64 templates per launch, as many as fit in it (it needs ~3, not p, transforms each).
+                            The decimated path processes templates in pairs: an odd value is rounded up            */
   int32_t path;          /* a gwmf_path; GWMF_PATH_AUTO (0) = the library's choice.  A path that does not support n
                             (FUSED: 2^15 .. 2^20, DECIMATED: >= 2^15) is GWMF_E_ARG                               */
   int32_t chisq_mode;    /* a gwmf_chisq_mode; ON_DEMAND needs the decimated path (n >= 2^15), else GWMF_E_ARG     */

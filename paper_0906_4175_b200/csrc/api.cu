@@ -71,6 +71,12 @@ Layout make_layout(const gwmf_params* p) {
     if (L.y_slots < p->p) L.y_slots = p->p;
   }
   if (L.batch > p->max_templates) L.batch = p->max_templates;
+  if (path == GWMF_PATH_DECIMATED && (L.batch & 1)) {
+    // templates are processed in pairs (2i, 2i+1 share one transform, segment.cu:k_pairing): a launch holds whole
+    // pairs, so an odd limit is rounded up
+    L.batch += 1;
+    if (L.y_slots < L.batch * p->p && p->batch > 0) L.y_slots = L.batch * p->p;
+  }
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
   L.u_tab = take(half * sizeof(double));
@@ -397,62 +403,75 @@ static bool any_generic(const Ctx* c, int first, int count) {
   return false;
 }
 
-// One batch of the decimated path.  Main stream: pass 1 of the effective bands, pass 2.  Side stream (high
-// priority, between a fork and a join): the generic kernel for the very wide bands of THIS batch, then the spectra
-// (correlate, band powers) of the NEXT batch into the other half of the double buffers.
+// One batch of the decimated path: [bfirst, bfirst + bcount) is pair-aligned (whole pairs 2i, 2i+1: spectra and pass 1
+// run for all of it), pass 2 processes the rows of [first, first + count) inside it.  Main stream: pass 1 of the
+// effective bands, pass 2.  Side stream (high priority, between a fork and a join): the generic kernel for the very
+// wide bands of THIS batch, then the spectra (correlate, band powers) of the NEXT batch into the other half of the
+// double buffers.
 //   ev: optional 4 events (timed mode: everything serialised on the main stream) recorded before the spectra,
 //   before pass 1, before pass 2 and after pass 2.
-static cudaError_t decimated_batch(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool ready,
-                                   bool update_slots, float* series_rho, float* series_chi, cudaEvent_t* ev) {
+struct Batch { int bfirst, bcount, first, count; };
+
+static cudaError_t decimated_batch(Ctx* c, const Batch& b, const Batch* nx, int parity, bool ready, bool update_slots,
+                                   float* series_rho, float* series_chi, cudaEvent_t* ev) {
   cudaError_t e;
-  const bool gen = any_generic(c, first, count);
+  const bool gen = any_generic(c, b.bfirst, b.bcount);
   if (ev) {
     if ((e = cudaEventRecord(ev[0], c->stream)) != cudaSuccess) return e;
-    if ((e = launch_spectra(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+    if ((e = launch_spectra(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
     if ((e = cudaEventRecord(ev[1], c->stream)) != cudaSuccess) return e;
-    if (gen && (e = launch_pass1_generic_eff(c, first, count, parity, c->stream)) != cudaSuccess) return e;
-    if ((e = launch_pass1_eff(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+    if (gen && (e = launch_pass1_generic_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
+    if ((e = launch_pass1_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
     if ((e = cudaEventRecord(ev[2], c->stream)) != cudaSuccess) return e;
-    if ((e = launch_pass2_eff(c, first, count, update_slots, series_rho, series_chi)) != cudaSuccess) return e;
+    if ((e = launch_pass2_eff(c, b.bfirst, b.bcount, b.first, b.count, update_slots, series_rho, series_chi)) != cudaSuccess) return e;
     return cudaEventRecord(ev[3], c->stream);
   }
-  if (!ready && (e = launch_spectra(c, first, count, parity, c->stream)) != cudaSuccess) return e;
-  const bool side_work = gen || next_count > 0;
+  if (!ready && (e = launch_spectra(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
+  const bool side_work = gen || nx != nullptr;
   if (side_work) {
     // fork: everything enqueued so far on the main stream (this batch's spectra, the previous batch's pass 2, which
     // read the band buffer and the other half of the spectra buffers) precedes the side work
     if ((e = cudaEventRecord(c->ev_fork, c->stream)) != cudaSuccess) return e;
     if ((e = cudaStreamWaitEvent(c->side, c->ev_fork, 0)) != cudaSuccess) return e;
-    if (gen && (e = launch_pass1_generic_eff(c, first, count, parity, c->side)) != cudaSuccess) return e;
-    if (next_count > 0 && (e = launch_spectra(c, next_first, next_count, parity ^ 1, c->side)) != cudaSuccess) return e;
+    if (gen && (e = launch_pass1_generic_eff(c, b.bfirst, b.bcount, parity, c->side)) != cudaSuccess) return e;
+    if (nx && (e = launch_spectra(c, nx->bfirst, nx->bcount, parity ^ 1, c->side)) != cudaSuccess) return e;
     if ((e = cudaEventRecord(c->ev_join, c->side)) != cudaSuccess) return e;
   }
-  if ((e = launch_pass1_eff(c, first, count, parity, c->stream)) != cudaSuccess) return e;
+  if ((e = launch_pass1_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
   if (side_work && (e = cudaStreamWaitEvent(c->stream, c->ev_join, 0)) != cudaSuccess) return e;
-  return launch_pass2_eff(c, first, count, update_slots, series_rho, series_chi);
+  return launch_pass2_eff(c, b.bfirst, b.bcount, b.first, b.count, update_slots, series_rho, series_chi);
 }
 
 // Cut [first, first + n) into launches: at most lay.batch templates each and, on the decimated path, at most
-// lay.y_slots n-point transforms (the band buffer's capacity); needs the host mirror.
-static void partition(const Ctx* c, int first, int n, std::vector<int>& counts) {
-  counts.clear();
-  int t = first;
+// lay.y_slots n-point transforms (the band buffer's capacity) over whole pairs of templates; needs the host mirror.
+static void partition(const Ctx* c, int first, int n, std::vector<Batch>& out) {
+  out.clear();
   const int end = first + n;
+  if (c->path != GWMF_PATH_DECIMATED) {
+    for (int t = first; t < end; t += c->lay.batch) {
+      const int cnt = end - t < c->lay.batch ? end - t : c->lay.batch;
+      out.push_back(Batch{t, cnt, t, cnt});
+    }
+    return;
+  }
+  const int T = c->n_templates;
+  int t = first & ~1;                                 // pair-aligned start
   while (t < end) {
     int cnt = 0;
-    if (c->path == GWMF_PATH_DECIMATED) {
-      while (t + cnt < end && cnt < c->lay.batch && c->h_eff[t + cnt + 1] - c->h_eff[t] <= c->lay.y_slots) ++cnt;
-      if (cnt == 0) cnt = 1;                      // cannot happen: n_eff <= p <= y_slots
-    } else {
-      cnt = end - t < c->lay.batch ? end - t : c->lay.batch;
+    while (t + cnt < end && cnt + 2 <= c->lay.batch) {
+      const int step = t + cnt + 2 <= T ? 2 : 1;      // the last template of an odd bank stands alone
+      if (c->h_eff[t + cnt + step] - c->h_eff[t] > c->lay.y_slots) break;
+      cnt += step;
     }
-    counts.push_back(cnt);
+    if (cnt == 0) cnt = t + 2 <= T ? 2 : 1;           // cannot happen: a pair needs at most 2 p <= y_slots
+    const int lo = t > first ? t : first, hi = t + cnt < end ? t + cnt : end;
+    out.push_back(Batch{t, cnt, lo, hi - lo});
     t += cnt;
   }
 }
 
 // All batches of [first_template, first_template + n_templates).  ev: 4 events per batch (timed mode) or nullptr.
-static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t* ev, const std::vector<int>& counts) {
+static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t* ev, const std::vector<Batch>& batches) {
   int rc = begin_segment_use(c);
   if (rc != GWMF_OK) return rc;
   if (c->pending_reset) {                       // first filter call on a new segment: forget the previous segment's events
@@ -460,28 +479,27 @@ static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t*
     c->pending_reset = false;
   }
   CU(launch_reset_slots(c, first_template, n_templates));
-  int parity = 0, f0 = first_template;
-  for (size_t b = 0; b < counts.size(); ++b, parity ^= 1) {
-    const int cnt = counts[b];
-    const int next = b + 1 < counts.size() ? counts[b + 1] : 0;
+  int parity = 0;
+  for (size_t b = 0; b < batches.size(); ++b, parity ^= 1) {
+    const Batch& bt = batches[b];
+    const Batch* nx = b + 1 < batches.size() ? &batches[b + 1] : nullptr;
     cudaEvent_t* evb = ev ? ev + 4 * b : nullptr;
     if (c->path == GWMF_PATH_DECIMATED) {
-      CU(decimated_batch(c, f0, cnt, f0 + cnt, next, parity, b > 0, true, nullptr, nullptr, evb));
+      CU(decimated_batch(c, bt, nx, parity, b > 0, true, nullptr, nullptr, evb));
     } else {
       if (evb) CU(cudaEventRecord(evb[0], c->stream));
       if (evb) CU(cudaEventRecord(evb[1], c->stream));
-      CU(launch_pass1_filter(c, f0, cnt, f0 + cnt, next, parity, b > 0));
+      CU(launch_pass1_filter(c, bt.first, bt.count, nx ? nx->first : 0, nx ? nx->count : 0, parity, b > 0));
       if (evb) CU(cudaEventRecord(evb[2], c->stream));
-      if (c->fused) CU(launch_fused_filter(c, f0, cnt, parity, true, nullptr, nullptr));
-      else CU(launch_pass2_filter(c, f0, cnt, true, nullptr, nullptr));
+      if (c->fused) CU(launch_fused_filter(c, bt.first, bt.count, parity, true, nullptr, nullptr));
+      else CU(launch_pass2_filter(c, bt.first, bt.count, true, nullptr, nullptr));
       if (evb) CU(cudaEventRecord(evb[3], c->stream));
     }
-    f0 += cnt;
   }
   if (c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND) {
-    if (ev) CU(cudaEventRecord(ev[4 * counts.size()], c->stream));
+    if (ev) CU(cudaEventRecord(ev[4 * batches.size()], c->stream));
     CU(launch_chisq_at_events(c, first_template, n_templates));
-    if (ev) CU(cudaEventRecord(ev[4 * counts.size() + 1], c->stream));
+    if (ev) CU(cudaEventRecord(ev[4 * batches.size() + 1], c->stream));
   }
   return end_segment_use(c);
 }
@@ -500,9 +518,9 @@ int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates) {
   if (n_templates == 0) return GWMF_OK;
   int rc = ensure_mirror(c);
   if (rc != GWMF_OK) return rc;
-  std::vector<int> counts;
-  partition(c, first_template, n_templates, counts);
-  return run_batches(c, first_template, n_templates, nullptr, counts);
+  std::vector<Batch> batches;
+  partition(c, first_template, n_templates, batches);
+  return run_batches(c, first_template, n_templates, nullptr, batches);
 }
 
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
@@ -514,16 +532,16 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
   if (!range_ok(c, first_template, n_templates) || n_templates < 1) return GWMF_E_ARG;
   int rc = ensure_mirror(c);
   if (rc != GWMF_OK) return rc;
-  std::vector<int> counts;
-  partition(c, first_template, n_templates, counts);
-  const int nb = (int)counts.size();
+  std::vector<Batch> batches;
+  partition(c, first_template, n_templates, batches);
+  const int nb = (int)batches.size();
   struct Events {                                   // destroyed on every exit path
     std::vector<cudaEvent_t> v;
     ~Events() { for (cudaEvent_t e : v) if (e) cudaEventDestroy(e); }
   } ev;
   ev.v.assign((size_t)nb * 4 + 2, nullptr);
   for (auto& e : ev.v) CU(cudaEventCreate(&e));
-  rc = run_batches(c, first_template, n_templates, ev.v.data(), counts);
+  rc = run_batches(c, first_template, n_templates, ev.v.data(), batches);
   if (rc != GWMF_OK) return rc;
   CU(cudaStreamSynchronize(c->stream));
   host_ms[0] = host_ms[1] = host_ms[2] = 0.0;
@@ -647,7 +665,9 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
   if (c->path == GWMF_PATH_DECIMATED) {
     const bool on_demand = c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND;          // no chi^2(t) series in that mode
     if (on_demand) CU(cudaMemsetAsync(d_chi, 0, sizeof(float) * (size_t)c->n, c->stream));
-    CU(decimated_batch(c, template_id, 1, 0, 0, 0, false, false, d_rho, on_demand ? nullptr : d_chi, nullptr));
+    std::vector<Batch> one;
+    partition(c, template_id, 1, one);                                         // the template's pair, rows of the template
+    CU(decimated_batch(c, one[0], nullptr, 0, false, false, d_rho, on_demand ? nullptr : d_chi, nullptr));
   } else {
     CU(launch_pass1_filter(c, template_id, 1, 0, 0, 0, false));
     if (c->fused) CU(launch_fused_filter(c, template_id, 1, 0, false, d_rho, d_chi));

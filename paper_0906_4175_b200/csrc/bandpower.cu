@@ -150,11 +150,7 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
 }
 
 // U+[tb][m] = sum over the class-S bands, ascending l (fixed order: bit-reproducible), 0 <= m < u_hi
-__global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wbuf,
-                                               float2* __restrict__ ubuf, int p) {
-  const int tb = blockIdx.y, m = blockIdx.x * 256 + threadIdx.x;
-  const TemplateMeta* mt = meta + tb;
-  if (m >= mt->u_hi) return;
+__device__ __forceinline__ float2 usum(const TemplateMeta* mt, const float2* __restrict__ wbuf, int tb, int p, int m) {
   float2 acc = make_float2(0.f, 0.f);
   unsigned s = mt->s_mask;
   while (s) {
@@ -166,7 +162,31 @@ __global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ 
       acc.y += v.y;
     }
   }
-  ubuf[(size_t)tb * kUCap + m] = acc;
+  return acc;
+}
+
+// Unpaired template: ubuf[tb][m] = U+[m] (one-sided, doubled for m > 0: its transform's real part is u).
+// Owner of a pair (tb, tb + 1): the two ubuf rows hold the pair spectrum P[m] = U_A[m] + i U_B[m], -up_hi < m < up_hi,
+// with bin 0 at the start of the guest's row; U_X[m] = U+_X[m] / 2 for m > 0, U_X[-m] = conj(U_X[m]) (two-sided
+// spectrum of a real series), so that ONE transform returns u_A + i u_B.
+__global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wbuf,
+                                               float2* __restrict__ ubuf, int p) {
+  const int tb = blockIdx.y, m = blockIdx.x * 256 + threadIdx.x;
+  const TemplateMeta* mt = meta + tb;
+  if (mt->pair == 2 || !mt->s_mask) return;               // a guest's spectrum is written by its owner
+  if (mt->pair == 0) {
+    if (m < mt->u_hi) ubuf[(size_t)tb * kUCap + m] = usum(mt, wbuf, tb, p, m);
+    return;
+  }
+  if (m >= mt->up_hi) return;
+  const float2 ua = usum(mt, wbuf, tb, p, m), ub = usum(mt + 1, wbuf, tb + 1, p, m);
+  float2* bin0 = ubuf + (size_t)(tb + 1) * kUCap;
+  if (m == 0) {
+    bin0[0] = make_float2(ua.x, ub.x);                    // both are real at m = 0
+  } else {
+    bin0[m] = make_float2(0.5f * (ua.x - ub.y), 0.5f * (ua.y + ub.x));        // (U_A + i U_B) / 2
+    bin0[-m] = make_float2(0.5f * (ua.x + ub.y), 0.5f * (ub.x - ua.y));       // (conj U_A + i conj U_B) / 2
+  }
 }
 
 cudaError_t configure_bandpower() {

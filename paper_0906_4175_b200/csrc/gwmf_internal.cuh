@@ -32,7 +32,10 @@ struct TemplateMeta {
   uint16_t row_off[kMaxBands + 2];  // band-separated spectrum Qb: rows of narrow band l start at row_off[l] (k_fused)
   // ---- decimated path: the template's EFFECTIVE bands (n-point transforms that are really run) ----
   //   if s_mask != 0:  e = 0: Z = the union of the class-S bands (one transform, gives their share of z)
-  //                    e = 1: U = one-sided spectrum of sum_{l in S} |z_l|^2 (real part of its transform)
+  //                    e = 1: U = one-sided spectrum of sum_{l in S} |z_l|^2 (real part of its transform), or, for
+  //                           the OWNER of a pair (pair == 1), UP = U_A + i U_B, the two-sided spectra of this template
+  //                           and of the next one: ONE transform returns u_A + i u_B.  The GUEST (pair == 2) has no
+  //                           U band of its own and reads the imaginary part of its owner's.
   //   then one per class-D band in ascending l (z_l itself: contributes to z and to sum |z_l|^2)
   uint32_t s_mask;               // bit l: band l is class S (0 < bins <= s_bins)
   uint32_t d_mask;               // bit l: band l is class D (bins > s_bins)
@@ -42,10 +45,12 @@ struct TemplateMeta {
   int32_t z_lo, z_hi;            // hull of the class-S bands, bins [z_lo, z_hi)
   int32_t u_hi;                  // support of U+: bins [0, u_hi), u_hi = widest class-S band
   int32_t full_band;             // chi^2 on demand: the ONE effective band is the whole template [edges[0], k_high)
+  int32_t pair;                  // 0: unpaired, 1: owner of the pair (t even, t + 1 is its guest), 2: guest
+  int32_t up_hi;                 // owner: support of the pair spectrum, bins (-up_hi, up_hi)
 };
 
 // One effective band: which spectrum it reads (kind) and the bins [e_lo, e_hi) it owns.
-enum EffKind { kEffZ = 0, kEffU = 1, kEffD = 2 };
+enum EffKind { kEffZ = 0, kEffU = 1, kEffD = 2, kEffUP = 3 };
 struct EffBand { int kind, e_lo, e_hi, l; };
 // The same, one record per slot of the whole bank (slot = eff_prefix[t] + e), written once per bank setup so that a
 // pass-1 CTA finds its work with ONE 32-byte load instead of a search through the template records.
@@ -63,8 +68,17 @@ __device__ __forceinline__ EffBand eff_band(const TemplateMeta* m, int e) {
   if (m->full_band) { b.kind = kEffD; b.e_lo = m->edges[0]; b.e_hi = m->k_high; b.l = -1; return b; }
   if (m->s_mask) {
     if (e == 0) { b.kind = kEffZ; b.e_lo = m->z_lo; b.e_hi = m->z_hi; b.l = -1; return b; }
-    if (e == 1) { b.kind = kEffU; b.e_lo = 0; b.e_hi = m->u_hi; b.l = -1; return b; }
-    e -= 2;
+    if (m->pair == 2) {
+      e -= 1;                                    // the guest of a pair has no U band of its own
+    } else {
+      if (e == 1) {
+        b.l = -1;
+        if (m->pair == 1) { b.kind = kEffUP; b.e_lo = 1 - m->up_hi; b.e_hi = m->up_hi; }
+        else { b.kind = kEffU; b.e_lo = 0; b.e_hi = m->u_hi; }
+        return b;
+      }
+      e -= 2;
+    }
   }
   unsigned d = m->d_mask;
   for (int i = 0; i < e; ++i) d &= d - 1;
@@ -165,7 +179,8 @@ cudaError_t configure_bandpower();
 cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st);      // W_l, then U+
 cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
 cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
-cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi);
+cudaError_t launch_pass2_eff(Ctx* c, int bfirst, int bcount, int first, int count, bool update_slots, float* series_rho,
+                             float* series_chi);
 cudaError_t launch_chisq_at_events(Ctx* c, int first, int count);      // chi^2 on demand: fills the slots' chi^2
 cudaError_t launch_reset_slots(Ctx* c, int first, int count);
 cudaError_t launch_compact(Ctx* c);

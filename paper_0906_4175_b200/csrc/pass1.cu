@@ -379,7 +379,7 @@ struct EffSrc {
 // (the band's first and last row are only partly inside); a masked element is zero-filled (src-size 0).
 template <bool HOLES>
 __device__ __forceinline__ void eff_request(const EffSrc& es, float2* slot, int k1, int k2, int fr, int lr) {
-  const int k = (k1 << kLogN2) + k2;
+  const int k = k1 * kN2 + k2;                  // k1 is negative for the lower half of a pair spectrum
   bool ok = k1 >= fr && k1 <= lr;
   if constexpr (HOLES) {
     for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
@@ -406,7 +406,7 @@ __device__ __forceinline__ void eff_request_round(const EffSrc& es, float2* stag
 // the transform are still free.
 template <bool HOLES>
 __device__ __forceinline__ float2 eff_load(const EffSrc& es, int k1, int k2, int fr, int lr) {
-  const int k = (k1 << kLogN2) + k2;
+  const int k = k1 * kN2 + k2;                  // k1 is negative for the lower half of a pair spectrum
   bool ok = k1 >= fr && k1 <= lr;
   if constexpr (HOLES) {
     for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
@@ -534,7 +534,9 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
   es.e_hi = d.e_hi;
   es.holes = s_holes;
   es.n_holes = d.n_holes;
-  es.src = d.kind == kEffU ? a.ubuf + (size_t)tb * kUCap : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
+  es.src = d.kind == kEffU    ? a.ubuf + (size_t)tb * kUCap
+           : d.kind == kEffUP ? a.ubuf + (size_t)(tb + 1) * kUCap              // bin 0 of the pair spectrum; bins run negative
+                              : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
   const int row_lo = es.e_lo >> kLogN2;
 
   if (d.n_holes > 0) {                          // rare: class-D bands inside the hull of Z

@@ -232,63 +232,74 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 // bulk copies, across band and row boundaries.
 // ---------------------------------------------------------------------------------------------------
 struct P2EArgs {
-  P2Args b;
+  P2Args b;                   // b.meta: first template of the (pair-aligned) batch; b.n_rows: rows of [t_begin, t_begin + count)
   int slot_base;              // eff_prefix of the first template of the batch
-  int batch;
+  int batch;                  // templates of the batch (spectra and pass 1 were run for all of them)
+  int t_begin;                // first template of the batch whose rows this launch processes (batch-relative)
 };
 
 // SINGLE: every template of the launch has exactly one effective band (p = 1, or chi^2 on demand): z is that band's
 // transform, no sums over bands are kept, and the epilogue is one compare of |z|^2 against the threshold per sample
 // (chi^2 is 0 by definition for p = 1 and is filled in later by k_chisq_at in the on-demand mode).
+constexpr int kP2EWarps = 12;     // k_pass2_eff: 12 warps per SM with a ring of 2 rows each (192 KB): the kernel is bound by the
+constexpr int kP2ERing = 2;       // latency of its per-row chains, not by HBM, once a template needs ~2 transforms
+
 template <bool SERIES, bool SINGLE>
-__global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
+__global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea) {
   const P2Args& a = ea.b;
   extern __shared__ __align__(128) float2 smem2[];
-  __shared__ int s_slot0[kMaxBatch];          // first slot of template tb (batch-relative)
-  __shared__ int s_neff[kMaxBatch];           // n_eff | has_s << 8
+  __shared__ int s_slot0[kMaxBatch + 2];      // first slot of template tb (batch-relative)
+  __shared__ int s_neff[kMaxBatch + 2];       // rows to read | has_s << 8 | guest of a pair << 9
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float2* tw_s = smem2;                                               // [c][jm]
-  float2* bufs = smem2 + 1024 + warp * (kP2Ring * kN2);
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2Warps * kP2Ring * kN2) + kP2Ring * warp;
+  float2* bufs = smem2 + 1024 + warp * (kP2ERing * kN2);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2EWarps * kP2ERing * kN2) + kP2ERing * warp;
   for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
   for (int t = threadIdx.x; t < ea.batch; t += blockDim.x) {
     s_slot0[t] = a.meta[t].eff_prefix - ea.slot_base;
-    s_neff[t] = a.meta[t].n_eff | (a.meta[t].s_mask ? 256 : 0);
+    const bool guest = a.meta[t].pair == 2;     // reads one row more than it owns: the pair band of template t - 1
+    s_neff[t] = (a.meta[t].n_eff + (guest ? 1 : 0)) | (a.meta[t].s_mask ? 256 : 0) | (guest ? 512 : 0);
   }
   __syncthreads();                                                    // the only CTA-wide barrier
 
-  const int total_warps = gridDim.x * kP2Warps;
-  const int first_row = blockIdx.x * kP2Warps + warp;
+  const int total_warps = gridDim.x * kP2EWarps;
+  const int first_row = blockIdx.x * kP2EWarps + warp;
   if (first_row >= a.n_rows) return;                                  // warps are independent: no CTA barrier below
   const int n1_mask = a.n1 - 1;
 
-  unsigned long long policy;
+  unsigned long long policy, policy_keep;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+  // a pair band is read twice, by the guest's row first (rows are walked downwards) and about one row-time later by
+  // its owner's: the first read keeps it in L2, the second one releases it
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(policy_keep));
 
   // Rows are walked from the END of the band buffer: what pass 1 wrote last is still in L2.
   const int last_row = a.n_rows - 1 - first_row;
   int pf_item = 0, pf_e = 0, pf_row = last_row;                       // prefetch cursor (next item to request)
   auto prefetch = [&]() {
     // caller: lane 0 only, and only after every lane has consumed the buffer being refilled
-    const int tb = pf_row >> a.log_n1, j1 = pf_row & n1_mask;
-    const float2* src = a.y + ((size_t)(s_slot0[tb] + pf_e) * a.n1 + j1) * kN2;
-    const int b = pf_item % kP2Ring;
+    const int tb = ea.t_begin + (pf_row >> a.log_n1), j1 = pf_row & n1_mask;
+    // item e of a row -> slot: a guest's item 1 is the pair band of its owner (slot 1 of template tb - 1)
+    const int slot = (s_neff[tb] & 512) ? (pf_e == 1 ? s_slot0[tb - 1] + 1 : s_slot0[tb] + pf_e - (pf_e > 1 ? 1 : 0))
+                                        : s_slot0[tb] + pf_e;
+    const float2* src = a.y + ((size_t)slot * a.n1 + j1) * kN2;
+    const int b = pf_item % kP2ERing;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     mbar_expect_tx(&bars[b], kRowBytes);
-    bulk_load_row(bufs + b * kN2, src, kRowBytes, &bars[b], policy);
+    bulk_load_row(bufs + b * kN2, src, kRowBytes, &bars[b], ((s_neff[tb] & 512) && pf_e == 1) ? policy_keep : policy);
   };
   auto advance = [&]() {
     ++pf_item;
-    if (++pf_e == (s_neff[pf_row >> a.log_n1] & 255)) { pf_e = 0; pf_row -= total_warps; }
+    if (++pf_e == (s_neff[ea.t_begin + (pf_row >> a.log_n1)] & 255)) { pf_e = 0; pf_row -= total_warps; }
   };
   if (lane == 0) {
 #pragma unroll
-    for (int b = 0; b < kP2Ring; ++b) mbar_init(&bars[b], 1);
+    for (int b = 0; b < kP2ERing; ++b) mbar_init(&bars[b], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncwarp();
 #pragma unroll 1
-  for (int b = 0; b < kP2Ring && pf_row >= 0; ++b) {
+  for (int b = 0; b < kP2ERing && pf_row >= 0; ++b) {
     if (lane == 0) prefetch();
     advance();
   }
@@ -301,14 +312,14 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
   int item = 0;
 #pragma unroll 1
   for (int row = last_row; row >= 0; row -= total_warps) {
-    const int tb = row >> a.log_n1, j1 = row & n1_mask;
+    const int tb = ea.t_begin + (row >> a.log_n1), j1 = row & n1_mask;
     const int ne = s_neff[tb] & 255;
-    const bool has_s = (s_neff[tb] & 256) != 0;
+    const bool has_s = (s_neff[tb] & 256) != 0, guest = (s_neff[tb] & 512) != 0;
 #pragma unroll 1
     for (int e = 0; e < ne; ++e, ++item) {
-      const int b = item % kP2Ring;
+      const int b = item % kP2ERing;
       const float2* cur = bufs + b * kN2;
-      mbar_wait(&bars[b], (item / kP2Ring) & 1);
+      mbar_wait(&bars[b], (item / kP2ERing) & 1);
       float2 x[32];
 #pragma unroll
       for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(cur[32 * c + lane], tw_s[32 * c + lane]);     // lane = jm
@@ -339,9 +350,14 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2_eff(P2EArgs ea) {
       if (has_s && e == 0) {                    // Z
 #pragma unroll
         for (int jc = 0; jc < 32; ++jc) az[jc] = cadd(az[jc], x[jc]);
-      } else if (has_s && e == 1) {             // U
+      } else if (has_s && e == 1) {             // U: real part; the guest of a pair owns the imaginary part
+        if (guest) {
 #pragma unroll
-        for (int jc = 0; jc < 32; ++jc) aq[jc] += x[jc].x;
+          for (int jc = 0; jc < 32; ++jc) aq[jc] += x[jc].y;
+        } else {
+#pragma unroll
+          for (int jc = 0; jc < 32; ++jc) aq[jc] += x[jc].x;
+        }
       } else {                                  // D
 #pragma unroll
         for (int jc = 0; jc < 32; ++jc) {
@@ -600,16 +616,17 @@ cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool u
 }
 
 constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
+constexpr size_t kP2ESmem = (size_t)(1024 + kP2EWarps * kP2ERing * kN2) * sizeof(float2) + kP2EWarps * kP2ERing * sizeof(unsigned long long);
 
 // Opt-in to > 48 KB of dynamic shared memory on the CURRENT device (gwmf_create calls this for every context).
 cudaError_t configure_pass2() {
   cudaError_t e = cudaFuncSetAttribute(k_pass2<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2Smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2ESmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2ESmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2ESmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass2_eff<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP2ESmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
   return e;
@@ -665,13 +682,15 @@ cudaError_t launch_pass2_dense(Ctx* c, const float2* d_mid, float2* d_out, cudaS
   return cudaGetLastError();
 }
 
-cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, float* series_rho, float* series_chi) {
+// batch = [bfirst, bfirst + bcount) (pair-aligned: spectra and pass 1 ran for all of it); rows of [first, first + count)
+cudaError_t launch_pass2_eff(Ctx* c, int bfirst, int bcount, int first, int count, bool update_slots, float* series_rho,
+                             float* series_chi) {
   P2EArgs ea;
   P2Args& a = ea.b;
   a.y = ws_ptr<float2>(c, c->lay.y);
   a.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
-  a.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
-  a.slots = update_slots ? ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows : nullptr;
+  a.meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + bfirst;
+  a.slots = update_slots ? ws_ptr<Slot>(c, c->lay.slots) + (size_t)bfirst * c->n_windows : nullptr;
   a.series_rho = series_rho;
   a.series_chi = series_chi;
   a.dense_out = nullptr;
@@ -684,15 +703,17 @@ cudaError_t launch_pass2_eff(Ctx* c, int first, int count, bool update_slots, fl
   a.n_windows = c->n_windows;
   a.n_rows = count * c->n1;
   a.thresh = (float)c->prm.rho_thresh;
-  ea.slot_base = c->h_eff[first];
-  ea.batch = count;
-  const bool single = c->h_eff[first + count] - c->h_eff[first] == count;     // one effective band per template
+  ea.slot_base = c->h_eff[bfirst];
+  ea.batch = bcount;
+  ea.t_begin = first - bfirst;
+  const bool single = c->prm.p == 1 || c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND;   // one effective band per template
   const bool series = series_rho || series_chi;
-  const dim3 grid(p2_grid(c, a.n_rows));
-  if (single && series) k_pass2_eff<true, true><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
-  else if (single) k_pass2_eff<false, true><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
-  else if (series) k_pass2_eff<true, false><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
-  else k_pass2_eff<false, false><<<grid, kP2Warps * 32, kP2Smem, c->stream>>>(ea);
+  const int want = (a.n_rows + kP2EWarps - 1) / kP2EWarps;
+  const dim3 grid(want < c->n_sms ? want : c->n_sms);       // persistent: at most one CTA per SM
+  if (single && series) k_pass2_eff<true, true><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
+  else if (single) k_pass2_eff<false, true><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
+  else if (series) k_pass2_eff<true, false><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
+  else k_pass2_eff<false, false><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
   c->launches++;
   return cudaGetLastError();
 }

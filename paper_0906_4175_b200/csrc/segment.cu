@@ -257,6 +257,8 @@ __global__ void __launch_bounds__(256) k_bank_setup(TemplateMeta* __restrict__ m
       meta[t].z_hi = z_hi;
       meta[t].u_hi = u_hi;
       meta[t].full_band = 0;
+      meta[t].pair = 0;
+      meta[t].up_hi = 0;
       if (on_demand) {                          // one transform over the whole template; chi^2 comes later, per event
         const int k0 = s_edges[ty][0];
         const int rows_all = ((k_high - 1) >> kLogN2) - (k0 >> kLogN2) + 1;
@@ -303,6 +305,22 @@ __global__ void __launch_bounds__(1024) k_eff_scan(TemplateMeta* __restrict__ me
   }
 }
 
+// Pairs (decimated path): templates 2i and 2i+1 share ONE transform for their two real series sum_l |z_l|^2 when
+// both have narrow bands: the owner (2i) carries the band UP = U_A + i U_B, the guest loses its U band.  Pairs are
+// fixed by the bank index, so a template's result does not depend on how the bank is cut into launches.
+__global__ void k_pairing(TemplateMeta* __restrict__ meta, int n_templates) {
+  const int t = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+  if (t + 1 >= n_templates) return;
+  TemplateMeta* a = meta + t;
+  TemplateMeta* b = meta + t + 1;
+  if (!a->s_mask || !b->s_mask || a->full_band || b->full_band) return;
+  a->pair = 1;
+  a->up_hi = a->u_hi > b->u_hi ? a->u_hi : b->u_hi;
+  b->pair = 2;
+  b->n_eff -= 1;
+  b->gen_mask = (b->gen_mask >> 2) << 1;          // its class-D bands move from e >= 2 to e >= 1
+}
+
 // slot table of the whole bank: one thread per (template, effective band)
 __global__ void __launch_bounds__(256) k_slot_table(const TemplateMeta* __restrict__ meta, SlotDesc* __restrict__ tab,
                                                     int n_templates) {
@@ -342,6 +360,8 @@ cudaError_t launch_bank_setup(Ctx* c) {
   c->mirror_ready = false;
   if (decim) {
     int32_t* d_eff = ws_ptr<int32_t>(c, c->lay.eff);
+    k_pairing<<<(c->n_templates / 2 + 255) / 256 + 1, 256, 0, c->stream>>>(ws_ptr<TemplateMeta>(c, c->lay.meta), c->n_templates);
+    c->launches++;
     k_eff_scan<<<1, 1024, 0, c->stream>>>(ws_ptr<TemplateMeta>(c, c->lay.meta), d_eff, c->n_templates);
     k_slot_table<<<(c->n_templates + 7) / 8, 256, 0, c->stream>>>(ws_ptr<TemplateMeta>(c, c->lay.meta),
                                                                     ws_ptr<SlotDesc>(c, c->lay.slot_tab), c->n_templates);
