@@ -463,11 +463,14 @@ def run_gpu(args):
             # the spill-free kernel moves (almost) no HBM bytes: it is bound by the FP32 pipes and shared memory
             flops_unit = 5.0 * w.n * np.log2(w.n) * w.p            # p * 5 N log2 N per template-segment
             apeak, asrc = alu_peak()
+            measured_alu = gwmf.fma_peak(5, f.stream)            # FFMA2 chains, libgwmf.so's own probe kernel
             tfl = flops_unit * count / (k_ms[2] * 1e-3) / 1e12
             tr, tr_src = traffic_record(path, args.workload, "pass2")
             line["roofline"] = {
                 "bound": "alu", "kernel": STAGE_TEXT[path]["pass2"], "achieved": float(tfl), "peak": apeak, "unit": "TFLOP/s",
-                "frac": float(tfl / apeak), "peak_source": asrc, "flops": "dense-FFT equivalent (p*5N*log2N per unit), not executed flops",
+                "frac": float(tfl / apeak), "peak_source": asrc, "peak_measured": measured_alu,
+                "frac_of_measured": float(tfl / measured_alu), "peak_measured_source": "gwmf_fma_peak: packed fma.rn.f32x2 chains",
+                "flops": "dense-FFT equivalent (p*5N*log2N per unit), not executed flops",
                 "traffic": tr * count / k_launch[2] if tr else None, "traffic_source": tr_src,
                 "avg_launch_ms": float(k_ms[2] / k_launch[2]), "kernels": kernels, "hbm_model_equivalent": hbm_model}
         else:
@@ -518,10 +521,17 @@ def main():
     ap.add_argument("--chisq-on-demand", action="store_true",
                     help="gwmf_params::chisq_mode = ON_DEMAND: one full-band transform per template, chi^2 evaluated only at "
                          "the event samples (SURVEY.md 8(f)-2; a different workload from the headline's chi^2(t) at every sample)")
+    ap.add_argument("--peak", action="store_true", help="print the measured FP32 (packed FFMA2) peak of the device and exit")
     ap.add_argument("--shard", default="segments", choices=["segments", "templates"],
                     help="N > 1: segments = every rank filters the whole bank against its own segment (weak scaling); "
                          "templates = one segment, the bank split by template id, events gathered (strong scaling)")
     args = ap.parse_args()
+    if args.peak:
+        from paper_0906_4175_b200 import gwmf
+        derived, src = alu_peak()
+        print(json.dumps({"fp32_peak_tflops_measured": gwmf.fma_peak(10), "how": "gwmf_fma_peak: packed fma.rn.f32x2 chains, best of 10",
+                          "fp32_peak_tflops_derived": derived, "derived_from": src}))
+        return 0
     if args.impl == "reference":
         return run_reference(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

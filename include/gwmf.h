@@ -198,6 +198,11 @@ int gwmf_uses_fused(const gwmf_ctx* ctx);
 /* The gwmf_path this context filters with (GWMF_PATH_AUTO resolved at gwmf_create); GWMF_E_ARG for a null ctx. */
 int gwmf_path_in_use(const gwmf_ctx* ctx);
 
+/* Measurement: FP32 (non-tensor) peak of the current device in TFLOP/s, measured with chains of packed
+ * fma.rn.f32x2 -- the instruction the hot kernels' butterflies are made of -- on the given stream (a cudaStream_t;
+ * NULL = default stream); best of `repeats` >= 1 timed launches after one warm-up.  Needs no context.  syncs. */
+int gwmf_fma_peak(void* cuda_stream, int32_t repeats, double* host_tflops);
+
 /* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
 int64_t gwmf_launch_count(const gwmf_ctx* ctx);
 
