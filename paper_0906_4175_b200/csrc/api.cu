@@ -392,7 +392,7 @@ static int ensure_mirror(Ctx* c) {
 
 // Q, W_l and U+ of a batch (decimated path), on stream st
 static cudaError_t launch_spectra(Ctx* c, int first, int count, int parity, cudaStream_t st) {
-  cudaError_t e = launch_correlate(c, first, count, parity, st);
+  cudaError_t e = launch_correlate(c, first, count, parity, st, true);
   if (e == cudaSuccess && c->prm.chisq_mode != GWMF_CHISQ_ON_DEMAND) e = launch_bandpower(c, first, count, parity, st);
   return e;
 }

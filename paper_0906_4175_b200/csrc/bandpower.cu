@@ -60,7 +60,6 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
   int log_l = kLogLMin;
   while ((1 << log_l) < 2 * B) ++log_l;
   if (log_l != LOG_L) return;
-  const float2* __restrict__ qband = q + (size_t)tb * half_n + e_lo;
   float2* __restrict__ wout = wbuf + ((size_t)tb * p + l) * kUCap;
   const int tid = threadIdx.x;
   float2* twl = sm + L + (L >> 4);
@@ -71,7 +70,17 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
   tw.hi = twh;
   tw.lo = twl;
 
-  for (int i = tid; i < L; i += kBpThreads) sm[pad16(i)] = i < B ? qband[i] : make_float2(0.f, 0.f);
+  // the band's bins -> shared memory.  Q is stored c-major inside each row of 1024 bins (cm_pos): walk the band's rows
+  // position by position (coalesced) and scatter to the bin's place
+  for (int i = B + tid; i < L; i += kBpThreads) sm[pad16(i)] = make_float2(0.f, 0.f);
+  {
+    const int row_lo = e_lo >> kLogN2, n_rows = ((e_lo + B - 1) >> kLogN2) - row_lo + 1;
+    const float2* __restrict__ qrows = q + (size_t)tb * half_n + (size_t)row_lo * kN2;
+    for (int idx = tid; idx < n_rows * kN2; idx += kBpThreads) {
+      const int i = ((row_lo + (idx >> kLogN2)) << kLogN2) + cm_pos(idx & (kN2 - 1)) - e_lo;
+      if (i >= 0 && i < B) sm[pad16(i)] = qrows[idx];
+    }
+  }
   __syncthreads();
   // ---- inverse transform, decimation in frequency: stage 1 (inputs i >= L/2 are zero since L >= 2B)
 #pragma unroll 1
@@ -174,8 +183,10 @@ __global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ 
   const int tb = blockIdx.y, m = blockIdx.x * 256 + threadIdx.x;
   const TemplateMeta* mt = meta + tb;
   if (mt->pair == 2 || !mt->s_mask) return;               // a guest's spectrum is written by its owner
+  // rows of 1024 bins are stored c-major (cm_pos), as pass 1 reads them; bin -m sits in row floor(-m / 1024)
+  const int mp = (m & ~(kN2 - 1)) + cm_pos(m & (kN2 - 1));
   if (mt->pair == 0) {
-    if (m < mt->u_hi) ubuf[(size_t)tb * kUCap + m] = usum(mt, wbuf, tb, p, m);
+    if (m < mt->u_hi) ubuf[(size_t)tb * kUCap + mp] = usum(mt, wbuf, tb, p, m);
     return;
   }
   if (m >= mt->up_hi) return;
@@ -184,8 +195,9 @@ __global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ 
   if (m == 0) {
     bin0[0] = make_float2(ua.x, ub.x);                    // both are real at m = 0
   } else {
-    bin0[m] = make_float2(0.5f * (ua.x - ub.y), 0.5f * (ua.y + ub.x));        // (U_A + i U_B) / 2
-    bin0[-m] = make_float2(0.5f * (ua.x + ub.y), 0.5f * (ub.x - ua.y));       // (conj U_A + i conj U_B) / 2
+    const int km = -m, kmp = (km & ~(kN2 - 1)) + cm_pos(km & (kN2 - 1));        // (km & ~1023) = 1024 floor(km / 1024) < 0
+    bin0[mp] = make_float2(0.5f * (ua.x - ub.y), 0.5f * (ua.y + ub.x));        // (U_A + i U_B) / 2
+    bin0[kmp] = make_float2(0.5f * (ua.x + ub.y), 0.5f * (ub.x - ua.y));       // (conj U_A + i conj U_B) / 2
   }
 }
 

@@ -19,6 +19,9 @@ constexpr int kSBinsMax = 8192;
 constexpr int kLMax = 16384;
 constexpr int kLogLMin = 11;     // smallest coarse grid (2048 points)
 constexpr int kUCap = kSBinsMax; // entries of the one-sided power spectrum U+ kept per template
+// C-major order inside a row of 1024 bins: bin k2 = 32 m + c sits at position 32 c + m (an involution).  The spectra
+// the decimated path's first pass reads (Q, U+) are stored this way: its warps read with lane = m.
+__host__ __device__ __forceinline__ int cm_pos(int k2) { return ((k2 & 31) << 5) | (k2 >> 5); }
 
 // Per-template record (device).  Phase in TURNS: psi(u) = (((c0 u^2 + c2) u + c3) u + c4) u - 1/8 with
 // u = f^(-1/3); this is Psi0/(2 pi) of the 2PN SPA phase (BASELINE.json:configs[0]).
@@ -157,7 +160,7 @@ cudaError_t launch_psd_tables(Ctx* c, cudaStream_t st);                // sn -> 
 cudaError_t launch_weighted_spectrum(Ctx* c, int buf, cudaStream_t st); // scratch spectrum, sn, c_tab -> wq[buf]
 cudaError_t launch_bank_setup(Ctx* c);
 cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, int next_count, int parity, bool q_ready);
-cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st);
+cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st, bool c_major = false);
 cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cudaStream_t st);
 inline int qb_rows_cap(const Ctx* c) { return c->n1 / 2 + kMaxBands + 2; }   // rows of Qb per template
 cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid, cudaStream_t st);

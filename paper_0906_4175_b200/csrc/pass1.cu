@@ -142,7 +142,8 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
             if constexpr (DENSE) {
               q = a.dense_in[k];
             } else {
-              q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + k];      // Q_I[k] from k_correlate
+              // Q_I[k] from k_correlate (decimated path: rows stored c-major)
+              q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + (a.eff ? (k - k2) + cm_pos(k2) : k)];
             }
             if constexpr (G > 1) {
               if (r > 0) q = cmul(q, a.tw_n1[(r * aa * NB) % n1]);         // w_NA^{r a}
@@ -238,6 +239,43 @@ __global__ void __launch_bounds__(256) k_correlate(const TemplateMeta* __restric
   float sn, cs;
   sincospif(2.0f * (float)t, &sn, &cs);
   q[(size_t)blockIdx.y * half_n + k] = cmul(wq[k], make_float2(cs, sn));
+}
+
+// The same values with every row of 1024 bins stored C-MAJOR (bin 32 m + c at position 32 c + m, cm_pos): the layout
+// the decimated path's first pass reads with lane = m.  One CTA per (row, template); the row is transposed through
+// shared memory so that both the reads of wq / u_tab and the writes of Q are coalesced.
+__global__ void __launch_bounds__(256) k_correlate_cm(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wq,
+                                                      const double* __restrict__ u_tab, float2* __restrict__ q, int half_n,
+                                                      int row_first) {
+  __shared__ float2 sq[kN2 + 32];
+  const TemplateMeta* m = meta + blockIdx.y;
+  const int row = row_first + blockIdx.x;
+  const int k_lo = m->edges[0], k_hi = m->k_high;
+  if ((row + 1) * kN2 <= k_lo || row * kN2 >= k_hi) return;            // CTA-uniform
+  const double c0 = m->c0, c2 = m->c2, c3 = m->c3, c4 = m->c4;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int k2 = threadIdx.x + 256 * i, k = row * kN2 + k2;
+    float2 v = make_float2(0.f, 0.f);
+    if (k >= k_lo && k < k_hi) {
+      // correlate: template phasor times weighted data bin (Eq. 1 integrand)
+      const double u = u_tab[k];
+      double t = fma(fma(fma(fma(c0, u * u, c2), u, c3), u, c4), u, -0.125);   // Psi0 / 2 pi, turns
+      t -= rint(t);
+      float sn, cs;
+      sincospif(2.0f * (float)t, &sn, &cs);
+      v = cmul(wq[k], make_float2(cs, sn));
+    }
+    const int pos = cm_pos(k2);
+    sq[pos + (pos >> 5)] = v;
+  }
+  __syncthreads();
+  float2* out = q + (size_t)blockIdx.y * half_n + (size_t)row * kN2;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int pos = threadIdx.x + 256 * i, k = row * kN2 + cm_pos(pos);
+    if (k >= k_lo && k < k_hi) out[pos] = sq[pos + (pos >> 5)];
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -359,173 +397,141 @@ __global__ void __launch_bounds__(256, 3) k_pass1_narrow(P1Args a) {
 // ---------------------------------------------------------------------------------------------------
 // Decimated path: first pass of the n-point transform of an EFFECTIVE band (gwmf_internal.cuh: Z = union of the
 // narrow bands read from Q, U = one-sided power spectrum read from ubuf, D = one wide band read from Q), any number
-// of input rows.  Same CTA shape and phases as k_pass1_narrow; what is new is the sum over the input rows that share
-// a residue b' = (k1 - row_lo) mod 32: with k1 = row_lo + b' + 32 t,
-//     sum_t X[k_t] e^{2 pi i ja k_t/n} = e^{2 pi i ja k_0/n} sum_t X[k_t] g^t,  g = e^{2 pi i ja 32 * 1024/n} = e^{2 pi i ja/NA},
-// evaluated by Horner's rule with the CTA-constant g: ceil(R/32) complex multiply-adds per (b', column), then the
-// same 32-point transform over b'.  Bands of at most 16 rows keep the pruned variants.  Bins of class-D bands that
-// lie inside the hull of Z ("holes": only with unusual spectra) are masked out.
+// of input rows.  WARP-AUTONOMOUS: a CTA owns one ja and 8 values of c (one per warp); a warp owns the 32 columns
+// k2 = 32 m + c, m = lane, and runs both the column transform and the first stage of the row transform on them
+// with no CTA barrier at all:
+//   phase 1, lane = m:  for every residue b' = (k1 - row_lo) mod 32, with k1 = row_lo + b' + 32 t,
+//         v[b'] = TW[b'] sum_t X[k1][k2] g^t,   g = e^{2 pi i ja/NA},  TW[i] = e^{2 pi i ja (row_lo + i)/n1}
+//       (Horner's rule over the rounds t, highest first; bands of <= 16 rows use pruned variants), then the 32-point
+//       transform over b' -> jb, and the lane writes ITS column of the warp's 32 x 32 tile.
+//   phase 2, lane = jb: reads ITS row of the tile (all m), multiplies by the twiddle
+//         e^{2 pi i [c j1 + (n/32) jb b0 + (jb n1 + 32 ja) m]/n} = S w^m,   j1 = ja + NA jb, b0 = row_lo mod 32
+//       (column twiddle e^{2 pi i j1 k2/n}, rotation w_32^{jb b0}, and the twiddle between the two 32-point stages of
+//       the row transform; geometric in m: w^m = w8^(m >> 3) w^(m & 7), two exact angles per lane, no table),
+//       32-point transform over m -> jm, and stages the 256 B piece A[j1][c][0..31] in the SAME row of the tile, from
+//       where one bulk copy (cp.async.bulk shared -> global, issued by the lane itself) takes it to the band buffer.
+// A lane only ever re-writes tile cells it was the last to read, so one __syncwarp() between the phases is all the
+// synchronisation there is.  The input spectra are stored C-MAJOR inside each row of 1024 bins (bin 32 m + c at
+// position 32 c + m, cm_pos) so that the 32 lanes of a warp read 256 contiguous bytes.
+// Bins of class-D bands that lie inside the hull of Z ("holes": only with unusual spectra) are masked out.
 // ---------------------------------------------------------------------------------------------------
 struct EffSrc {
-  const float2* src;      // spectrum indexed by absolute bin k (Q of the template, or U+ of the template)
+  const float2* src;      // spectrum, rows of 1024 bins in c-major order: bin k at src[(k & ~1023) + cm_pos(k & 1023)]
   int e_lo, e_hi;
   int n_holes;            // Z only
   const int* holes;       // shared memory: [2h] = first bin of hole h, [2h+1] = one past its last bin
 };
 
-// Input of thread (column k2) from row k1, staged through shared memory by an 8-byte cp.async (LDGSTS): no
-// register is tied up while the load is in flight, so a whole round of 32 rows is requested at once.  Rows strictly
-// inside the band need no bin test: fr / lr are the first / last row whose bin in THIS column belongs to the band
-// (the band's first and last row are only partly inside); a masked element is zero-filled (src-size 0).
-template <bool HOLES>
-__device__ __forceinline__ void eff_request(const EffSrc& es, float2* slot, int k1, int k2, int fr, int lr) {
-  const int k = k1 * kN2 + k2;                  // k1 is negative for the lower half of a pair spectrum
-  bool ok = k1 >= fr && k1 <= lr;
-  if constexpr (HOLES) {
-    for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
-  }
-  const float2* src = es.src + (ok ? k : es.e_lo);                 // always a valid address
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((unsigned)__cvta_generic_to_shared(slot)), "l"(src),
-               "r"(ok ? 8 : 0)
-               : "memory");
-}
+constexpr int kWStride = 34;                      // float2 per row of a warp's tile (272 B: 16-byte aligned, conflict-free)
+constexpr int kWTile = 32 * kWStride;             // float2 per warp
+constexpr size_t kP1WSmem = (size_t)(8 * kWTile + 8 * 32) * sizeof(float2);     // tiles + per-warp TW tables
+
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// First round of requests of a thread (rows row_lo + i + 32 (T-1), i < RMAX), issued BEFORE the CTA builds its
-// twiddle tables so that their latency overlaps that work.  stage: [32 rows][256 columns] aliasing the exchange tile;
-// a thread only ever touches its own column of it.
-template <int RMAX, bool HOLES>
-__device__ __forceinline__ void eff_request_round(const EffSrc& es, float2* stage_col, int row0, int k2, int fr, int lr) {
-#pragma unroll
-  for (int i = 0; i < RMAX; ++i) eff_request<HOLES>(es, stage_col + i * 256, row0 + i, k2, fr, lr);
-  cp_async_commit();
-}
-
-// Plain (register) load of the same element, for the round that is requested first of all, while the registers of
-// the transform are still free.
 template <bool HOLES>
-__device__ __forceinline__ float2 eff_load(const EffSrc& es, int k1, int k2, int fr, int lr) {
-  const int k = k1 * kN2 + k2;                  // k1 is negative for the lower half of a pair spectrum
+__device__ __forceinline__ bool eff_ok(const EffSrc& es, int k1, int k2, int fr, int lr) {
   bool ok = k1 >= fr && k1 <= lr;
   if constexpr (HOLES) {
+    const int k = k1 * kN2 + k2;
     for (int h = 0; h < es.n_holes; ++h) ok = ok && !(k >= es.holes[2 * h] && k < es.holes[2 * h + 1]);
   }
-  float2 val = make_float2(0.f, 0.f);
-  if (ok) val = __ldg(es.src + k);
-  return val;
+  return ok;
 }
 
-// Phase 1 of a CTA: thread (m, ci) owns column k2 and forms, for every residue b' = (k1 - row_lo) mod 32,
-//     v[b'] = TW[b'] sum_t X[row_lo + b' + 32 t][k2] g^t        (Horner, g = e^{2 pi i ja/NA})
-// then the 32-point transform over b', the T1 twiddle, and writes its column of the exchange tile.
-// TW[i] = e^{2 pi i ja (row_lo + i)/n1} (shared, CTA constant).  The column part e^{2 pi i ja k2/n} of the twiddle is
-// split off: its m part rides on the T1 table (built per CTA), its c part on the per-thread twiddle of phase 2.
-// Latency: round t = 0 is loaded straight into the registers v[] at the very top (they are free until the transform),
-// the last round t = T-1 (if T > 1) goes through cp.async into the staging area at the same time; both are in flight
-// while the CTA builds its tables.  Only bands of more than 64 rows have further rounds, requested one after the other.
+// predicated 8-byte load (no branch): 0 where !ok
+__device__ __forceinline__ float2 ldg_pred(const float2* p, bool ok) {
+  float2 v = make_float2(0.f, 0.f);
+  asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\t@p ld.global.nc.v2.f32 {%0, %1}, [%2];\n\t}"
+      : "+f"(v.x), "+f"(v.y)
+      : "l"(p), "r"((int)ok));
+  return v;
+}
+// the same element through an 8-byte cp.async into shared memory (zero-filled where !ok): no register is tied up
+__device__ __forceinline__ void ldgsts_pred(float2* slot, const float2* p, bool ok) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((unsigned)__cvta_generic_to_shared(slot)), "l"(p),
+               "r"(ok ? 8 : 0)
+               : "memory");
+}
+
+// Phase 1 of a warp (lane = m, column k2 = 32 lane + c): leaves v[jb], jb = 0..31 in natural order.
+// col: the lane's column of the warp's tile (tile + lane), rows i at stride kWStride -- used as the landing zone of the
+// cp.async rounds, a lane only touches its own column.  TW: the warp's table (shared).
 template <int RMAX, bool HOLES>
-__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, float2* __restrict__ T1, float2* __restrict__ TW,
-                                           float2* __restrict__ tile, int ja, int cg) {
-  const int tid = threadIdx.x;
-  const unsigned nmask = (1u << a.log_n) - 1u;
-  const int n1m = a.n1 - 1;
+__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float2* __restrict__ TW,
+                                           float2* __restrict__ col, int ja, int c, int lane, float2 (&v)[32]) {
   const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
-  const int T = (R + 31) >> 5;
-  const int ci = tid & 7, m = tid >> 3;
-  const int k2 = 32 * m + 8 * cg + ci;
-  const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);
+  const int T = RMAX < 32 ? 1 : (R + 31) >> 5;
+  const int k2 = 32 * lane + c;
+  const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);       // first / last row whose bin in THIS column is in the band
   const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
-  float2* stage_col = tile + tid;               // [i][256]: column tid = m * 8 + ci of the staging area
+  const float2* __restrict__ base = es.src + c * 32 + lane;            // + k1 * 1024 (k1 < 0 in the lower half of a pair spectrum)
+  const float2* safe = es.src + (size_t)(row_lo < 0 ? 0 : row_lo) * kN2;
 
-  float2 v[32];
-  const bool preload = RMAX < 32 || T <= 2;     // CTA-uniform
-  if (preload) {
+  // top round (t = T - 1) straight into the registers of the transform; the one below it through cp.async at the same time
+  {
+    const int r0 = row_lo + 32 * (T - 1);
 #pragma unroll
-    for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = eff_load<HOLES>(es, row_lo + i, k2, fr, lr);        // round 0
+    for (int i = 0; i < RMAX; ++i) {
+      const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
+      v[brev<32>(i)] = ldg_pred(base + (ptrdiff_t)(r0 + i) * kN2, ok);
+    }
   }
-  if constexpr (RMAX == 32) {
-    if (T > 1) eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * (T - 1), k2, fr, lr);          // round T-1
-  }
-  if (tid < 32) TW[tid] = a.tw_n1[(ja * (row_lo + tid)) & n1m];
-  __syncthreads();                              // T1 (built by the caller before the slot was known) and TW are ready
-
   if constexpr (RMAX == 32) {
     if (T > 1) {
-      const tw4 g = make_tw4(a.tw_n1[(ja * 32) & n1m]);                          // e^{2 pi i ja/NA}
-      cp_async_wait_all();                                                       // round T-1 has landed (own column only)
-      if (preload) {                                                             // T == 2: v = stage g + v
+      auto request = [&](int t) {
+        const int r0 = row_lo + 32 * t;
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
-          const float2 hi = stage_col[i * 256], val = v[brev<32>(i)];
-          v[brev<32>(i)] = unpk(fma2(pk(-hi.y, hi.x), g.yy, fma2(pk(hi), g.xx, pk(val))));
+          const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
+          ldgsts_pred(col + i * kWStride, ok ? base + (ptrdiff_t)(r0 + i) * kN2 : safe, ok);
         }
-      } else {                                                                   // more than 64 rows: round after round
-#pragma unroll
-        for (int i = 0; i < 32; ++i) v[brev<32>(i)] = stage_col[i * 256];
+        cp_async_commit();
+      };
+      request(T - 2);
+      const tw4 g = make_tw4(a.tw_n1[(ja * 32) & (a.n1 - 1)]);                    // e^{2 pi i ja/NA}
 #pragma unroll 1
-        for (int t = T - 2; t >= 0; --t) {
-          eff_request_round<32, HOLES>(es, stage_col, row_lo + 32 * t, k2, fr, lr);
-          cp_async_wait_all();
+      for (int t = T - 2; t >= 0; --t) {
+        cp_async_wait_all();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            const float2 val = stage_col[i * 256], w = v[brev<32>(i)];
-            v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
-          }
+        for (int i = 0; i < 32; ++i) {
+          const float2 val = col[i * kWStride], w = v[brev<32>(i)];
+          v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
         }
+        if (t > 0) request(t - 1);
       }
     }
   }
 #pragma unroll
   for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(v[brev<32>(i)], TW[i]);
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
-  if constexpr (RMAX == 32) __syncthreads();   // every thread has consumed its staged inputs: the tile may be written
-  const float4* __restrict__ t1 = reinterpret_cast<const float4*>(T1 + m * kT1Stride);
-#pragma unroll
-  for (int jb = 0; jb < 32; jb += 2) {
-    const float4 w = t1[jb >> 1];
-    tile[jb * kTileStride + m * 8 + ci] = cmul(v[jb], make_float2(w.x, w.y));
-    tile[(jb + 1) * kTileStride + m * 8 + ci] = cmul(v[jb + 1], make_float2(w.z, w.w));
-  }
 }
 
 template <bool HOLES>
-__device__ __forceinline__ void eff_cta(const P1Args& a, const EffSrc& es, float2* tile, float2* T1, float2* TW, int ja, int cg) {
+__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float2* TW, float2* col, int ja, int c, int lane,
+                                         float2 (&v)[32]) {
   const int R = ((es.e_hi - 1) >> kLogN2) - (es.e_lo >> kLogN2) + 1;
-  if (R <= 4) eff_phase1<4, HOLES>(a, es, T1, TW, tile, ja, cg);
-  else if (R <= 8) eff_phase1<8, HOLES>(a, es, T1, TW, tile, ja, cg);
-  else if (R <= 16) eff_phase1<16, HOLES>(a, es, T1, TW, tile, ja, cg);
-  else eff_phase1<32, HOLES>(a, es, T1, TW, tile, ja, cg);
+  if (R <= 4) eff_phase1<4, HOLES>(a, es, TW, col, ja, c, lane, v);
+  else if (R <= 8) eff_phase1<8, HOLES>(a, es, TW, col, ja, c, lane, v);
+  else if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, col, ja, c, lane, v);
+  else eff_phase1<32, HOLES>(a, es, TW, col, ja, c, lane, v);
 }
 
 __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
   extern __shared__ __align__(128) float2 smem[];
-  float2* tile = smem;                          // [32][kStageStride] (phase 1: stride kTileStride; before that: input staging)
-  float2* T1 = smem + 32 * kStageStride;        // [32 m][kT1Stride]  e^{2 pi i (jb/1024 + 32 ja/n) m}
-  __shared__ float2 TW[32];                     // e^{2 pi i ja (row_lo + i)/n1}
   __shared__ int s_holes[2 * kMaxBands];
 
-  const int tid = threadIdx.x;
-  const int na = a.n1 >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  float2* tile = smem + warp * kWTile;          // this warp's [32][kWStride] tile
+  float2* TW = smem + 8 * kWTile + warp * 32;   // this warp's e^{2 pi i ja (row_lo + i)/n1}
+  const int na = a.n1 >> 5, n1m = a.n1 - 1;
   const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
+  const int c = 8 * cg + warp;
   const int slot = blockIdx.y;                  // batch-relative
   const unsigned nmask = (1u << a.log_n) - 1u;
 
   const SlotDesc d = slot_tab[a.slot_base + slot];      // one 32-byte load, same address in every thread
-  {
-    // While the descriptor is on its way: T1 row m for jb = 4 ci .. 4 ci + 3 times this thread's m part of the column
-    // twiddle, e^{2 pi i ja 32 m/n} (depends on ja only)
-    const int ci = tid & 7, m = tid >> 3;
-    const float2 Am = cis_frac(((unsigned)ja * 32u * (unsigned)m) & nmask, a.log_n);
-    const float4* src4 = reinterpret_cast<const float4*>(a.tw_p2 + m * 32 + 4 * ci);
-    const float4 w0 = __ldg(src4), w1 = __ldg(src4 + 1);
-    float4* dst = reinterpret_cast<float4*>(T1 + m * kT1Stride + 4 * ci);
-    const float2 p0 = cmul(make_float2(w0.x, w0.y), Am), p1 = cmul(make_float2(w0.z, w0.w), Am);
-    const float2 p2 = cmul(make_float2(w1.x, w1.y), Am), p3 = cmul(make_float2(w1.z, w1.w), Am);
-    dst[0] = make_float4(p0.x, p0.y, p1.x, p1.y);
-    dst[1] = make_float4(p2.x, p2.y, p3.x, p3.y);
-  }
   if (d.generic) return;                        // very many rows: k_pass1 (generic) + k_rowstage write this slot
   const int tb = d.t - a.first_template;
 
@@ -538,8 +544,11 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
            : d.kind == kEffUP ? a.ubuf + (size_t)(tb + 1) * kUCap              // bin 0 of the pair spectrum; bins run negative
                               : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
   const int row_lo = es.e_lo >> kLogN2;
+  TW[lane] = __ldg(&a.tw_n1[(ja * (row_lo + lane)) & n1m]);
+  __syncwarp();
 
-  if (d.n_holes > 0) {                          // rare: class-D bands inside the hull of Z
+  float2 v[32];
+  if (d.n_holes > 0) {                          // rare: class-D bands inside the hull of Z (CTA-uniform branch)
     if (tid == 0) {
       const TemplateMeta* mt = a.meta + tb;
       int nh = 0;
@@ -551,37 +560,64 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
       }
     }
     __syncthreads();
-    eff_cta<true>(a, es, tile, T1, TW, ja, cg);
+    eff_warp<true>(a, es, TW, tile + lane, ja, c, lane, v);
   } else {
-    eff_cta<false>(a, es, tile, T1, TW, ja, cg);
+    eff_warp<false>(a, es, TW, tile + lane, ja, c, lane, v);
   }
-  __syncthreads();
-
-  float2* out0 = a.y + ((size_t)slot * a.n1 + (size_t)ja) * kN2 + cg * 256;   // row jb adds jb * na * 1024
-  const size_t row_stride = (size_t)na * kN2;
-  // ---- phase 2: thread (jb = lane, ci = warp)
-  {
-    const int jb = tid & 31, cw = tid >> 5;
-    const int c = 8 * cg + cw;
-    // e^{2 pi i jb (c + 1024 b0)/32768} (rest of the column twiddle e^{2 pi i NA jb k2/n} and the rotation w_32^{jb b0})
-    // times the c part of e^{2 pi i ja k2/n}: one angle, exact in integers mod n
-    const unsigned num = ((unsigned)jb * (unsigned)(c + 1024 * (row_lo & 31)) * (unsigned)na + (unsigned)ja * (unsigned)c) & nmask;
-    const tw4 S = make_tw4(cis_frac(num, a.log_n));
-    float2 x[32];
+  // the lane's column of the tile: tile[jb][m = lane]
 #pragma unroll
-    for (int mm = 0; mm < 32; ++mm) x[brev<32>(mm)] = cmul_tw(tile[jb * kTileStride + mm * 8 + cw], S);
-    fft_dit<32>(x);                                   // over m -> jm
-    __syncthreads();                                  // the tile has been read by everyone: reuse it as staging
-    float4* st = reinterpret_cast<float4*>(tile + jb * kStageStride + cw * 32);
+  for (int jb = 0; jb < 32; ++jb) tile[jb * kWStride + lane] = v[jb];
+  __syncwarp();
+
+  // ---- phase 2: lane = jb, row j1 = ja + NA jb
+  const int jb = lane;
+  const unsigned j1 = (unsigned)ja + (unsigned)na * (unsigned)jb;
+  // S = e^{2 pi i [c j1 + (n/32) jb b0]/n},  w = e^{2 pi i (jb n1 + 32 ja)/n}: exact angles in integers mod n
+  const unsigned num_s = ((unsigned)c * j1 + (((unsigned)jb * (unsigned)(row_lo & 31)) << (a.log_n - 5))) & nmask;
+  const unsigned num_w = ((unsigned)jb * (unsigned)a.n1 + 32u * (unsigned)ja) & nmask;
+  const float2 S = cis_frac(num_s, a.log_n);
+  const float2 w1 = cis_frac(num_w, a.log_n);
+  const float2 w8 = cis_frac((8u * num_w) & nmask, a.log_n);
+  // W[lo] = w^lo, lo < 8 (chain from w); B[hi] = S w8^hi, hi < 4
+  tw4 B[4];
+  {
+    float2 b = S;
+    B[0] = make_tw4(b);
+#pragma unroll
+    for (int hi = 1; hi < 4; ++hi) { b = cmul(b, w8); B[hi] = make_tw4(b); }
+  }
+  float2 x[32];
+  {
+    const float4* __restrict__ row = reinterpret_cast<const float4*>(tile + jb * kWStride);
+    float2 wl = make_float2(1.f, 0.f);
+#pragma unroll
+    for (int lo = 0; lo < 8; lo += 2) {
+      const tw4 Wa = make_tw4(wl);
+      wl = cmul(wl, w1);
+      const tw4 Wb = make_tw4(wl);
+      if (lo < 6) wl = cmul(wl, w1);
+#pragma unroll
+      for (int hi = 0; hi < 4; ++hi) {
+        const int m = 8 * hi + lo;
+        const float4 t = row[m >> 1];                                  // tile[jb][m], tile[jb][m + 1]
+        const float2 t0 = make_float2(t.x, t.y), t1 = make_float2(t.z, t.w);
+        x[brev<32>(m)] = cmul_tw(lo == 0 ? t0 : cmul_tw(t0, Wa), B[hi]);
+        x[brev<32>(m + 1)] = cmul_tw(cmul_tw(t1, Wb), B[hi]);
+      }
+    }
+  }
+  fft_dit<32>(x);                                   // over m -> jm
+  // stage the 256 B piece A[j1][c][0..31] in the lane's own row of the tile and send it off
+  {
+    float4* st = reinterpret_cast<float4*>(tile + jb * kWStride);
 #pragma unroll
     for (int jm = 0; jm < 32; jm += 2) st[jm >> 1] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic writes -> visible to the bulk copy engine
-  __syncthreads();
-  if (tid < 32) {
-    const unsigned src = (unsigned)__cvta_generic_to_shared(tile + tid * kStageStride);
-    float2* dst = out0 + (size_t)tid * row_stride;
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], 2048;" ::"l"(dst), "r"(src) : "memory");
+  {
+    float2* dst = a.y + ((size_t)slot * a.n1 + (size_t)j1) * kN2 + c * 32;
+    const unsigned src = (unsigned)__cvta_generic_to_shared(tile + jb * kWStride);
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], 256;" ::"l"(dst), "r"(src) : "memory");
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the copy's reads
   }
@@ -677,18 +713,25 @@ cudaError_t launch_correlate_bands(Ctx* c, int first, int count, int parity, cud
   return cudaGetLastError();
 }
 
-cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+cudaError_t launch_correlate(Ctx* c, int first, int count, int parity, cudaStream_t st, bool c_major) {
   const int half = (int)(c->n / 2);
   // only the bins some template of the batch owns: k_low .. the batch's largest k_high (host-side bank scalars)
   int kh = 0;
   for (int t = first; t < first + count; ++t) kh = c->h_meta[t].k_high > kh ? c->h_meta[t].k_high : kh;
+  float2* q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half;
+  if (c_major) {
+    const int row_first = c->k_low >> kLogN2, rows = ((kh - 1) >> kLogN2) - row_first + 1;
+    if (rows <= 0) return cudaSuccess;
+    k_correlate_cm<<<dim3(rows, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, wq_buf(c, c->front),
+                                                      ws_ptr<double>(c, c->lay.u_tab), q, half, row_first);
+    c->launches++;
+    return cudaGetLastError();
+  }
   const int k_first = c->k_low & ~255;
   const int blocks = (kh - k_first + 255) / 256;
   if (blocks <= 0) return cudaSuccess;
   k_correlate<<<dim3(blocks, count), 256, 0, st>>>(ws_ptr<TemplateMeta>(c, c->lay.meta) + first, wq_buf(c, c->front),
-                                                  ws_ptr<double>(c, c->lay.u_tab),
-                                                  ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half, half,
-                                                  k_first);
+                                                  ws_ptr<double>(c, c->lay.u_tab), q, half, k_first);
   c->launches++;
   return cudaGetLastError();
 }
@@ -817,7 +860,7 @@ cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStrea
   fill_eff_args(c, args, first, count, parity);
   const int n_slots = c->h_eff[first + count] - c->h_eff[first];
   if (n_slots <= 0) return cudaSuccess;
-  k_pass1_eff<<<dim3(4 * c->na, n_slots), 256, kNarrowSmem, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab));
+  k_pass1_eff<<<dim3(4 * c->na, n_slots), 256, kP1WSmem, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab));
   c->launches++;
   return cudaGetLastError();
 }
@@ -843,7 +886,7 @@ static cudaError_t configure_p1_one() {
 // for each context: the attribute is per device, not per process).
 cudaError_t configure_pass1(int /*path*/) {
   cudaError_t e = cudaFuncSetAttribute(k_pass1_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNarrowSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass1_eff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNarrowSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass1_eff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kP1WSmem);
   if (e == cudaSuccess) e = configure_p1_one<1, 16>();
   if (e == cudaSuccess) e = configure_p1_one<1, 32>();
   if (e == cudaSuccess) e = configure_p1_one<2, 32>();
