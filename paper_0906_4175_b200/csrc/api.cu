@@ -243,7 +243,8 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->ev_last_load = nullptr;
   for (int b = 0; b < 2; ++b) { c->h_stage[b] = nullptr; c->ev_seg_ready[b] = c->ev_seg_free[b] = c->ev_stage_free[b] = nullptr; }
   // > 48 KB of dynamic shared memory is an opt-in per function AND per device: do it for this context's device
-  if (configure_pass1(c->path) != cudaSuccess || configure_pass2() != cudaSuccess || configure_bandpower() != cudaSuccess) {
+  if (configure_pass1(c->path) != cudaSuccess || configure_pass2() != cudaSuccess || configure_bandpower() != cudaSuccess ||
+      (c->path == GWMF_PATH_DECIMATED && make_band_tensor_map(c) != cudaSuccess)) {
     delete c;
     return GWMF_E_CUDA;
   }

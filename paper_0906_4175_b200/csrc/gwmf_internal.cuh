@@ -1,5 +1,6 @@
 // gwmf_internal.cuh -- shared declarations of the CUDA side (not part of the C ABI).
 #pragma once
+#include <cuda.h>           // CUtensorMap (type only; no driver library is linked)
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
@@ -129,6 +130,7 @@ struct Ctx {
   int path;                      // GWMF_PATH_TWO_PASS / _FUSED / _DECIMATED (resolved from gwmf_params::path at create)
   bool fused;                    // path == GWMF_PATH_FUSED
   int device;                    // CUDA device the context lives on
+  CUtensorMap band_tmap;         // decimated path: the band buffer [tile = slot * NA + ja][c][jb][256 B] as a 4-d tensor (pass 2's row gather)
   int s_bins;                    // decimated path: class-S threshold in bins = min(kSBinsMax, n / 16)
   int t_max;                     // decimated path: effective bands of more than 32 * t_max input rows use the generic kernel
   int32_t* h_eff;                // host mirror (pinned): eff_prefix[0 .. n_templates], then one "has generic band" flag per template
@@ -178,6 +180,7 @@ inline cudaError_t launch_fft_dense(Ctx* c, const float2* d_in, float2* d_mid, f
 // decimated path
 cudaError_t configure_pass1(int path);
 cudaError_t configure_pass2();
+cudaError_t make_band_tensor_map(Ctx* c);   // needs lay.y, n1 (gwmf_create)
 cudaError_t configure_bandpower();
 cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st);      // W_l, then U+
 cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);

@@ -35,6 +35,7 @@ struct P1Args {
   int eff;                    // 0: y is indexed by tb * p + l (two-pass / spill-free paths)
   int slot_base;              // eff_prefix of the first template of the batch
   int first_template;         // bank index of the first template of the batch
+  int ja_per_cta;             // k_pass1_eff: consecutive ja values a CTA walks over
   const float2* ubuf;         // [batch][kUCap] one-sided power spectra U+ (bandpower.cu)
 };
 
@@ -170,10 +171,18 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) v[b] = S[m * SROW + b * C + c];
       fft_dif<NB>(v);
-      float2* out = a.y + ((size_t)band_index * n1 + (size_t)(G * m + r)) * kN2 + k2;
+      if (a.eff) {
+        // decimated path: the band buffer is [slot][ja][c][jb][.] (k_pass1_eff); Y[j1][32 mm + cc] goes to cell mm of
+        // the piece (ja, cc, jb), where the row stage (k_rowstage, mode 2) transforms it in place
+        float2* out = a.y + ((((size_t)band_index * NA + (size_t)(G * m + r)) * 32 + (k2 & 31)) << 10) + (k2 >> 5);
 #pragma unroll
-      for (int jb = 0; jb < NB; ++jb)
-        out[(size_t)jb * NA * kN2] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
+        for (int jb = 0; jb < NB; ++jb) out[jb * 32] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
+      } else {
+        float2* out = a.y + ((size_t)band_index * n1 + (size_t)(G * m + r)) * kN2 + k2;
+#pragma unroll
+        for (int jb = 0; jb < NB; ++jb)
+          out[(size_t)jb * NA * kN2] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
+      }
     }
     __syncthreads();                            // S, A, Bt are rewritten by the next item
   }
@@ -207,6 +216,23 @@ __global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const 
   for (long long row = (long long)blockIdx.x * 8 + warp; row < total_rows; row += (long long)gridDim.x * 8) {
     const int w = (int)(row >> log_n1), j1 = (int)(row & ((1 << log_n1) - 1));
     const int band = use_mask ? s_list[w] : w;
+    if (use_mask == 2) {
+      // decimated path: lane = c owns the 256 B piece (ja, c, jb) of the slot, j1 = ja + NA jb; the result is stored
+      // with the 16-byte chunks swizzled as k_pass1_eff stores them (chunk ch at ch ^ (jb & 15))
+      const int log_na = log_n1 - 5, ja = j1 & ((1 << log_na) - 1), jb = j1 >> log_na;
+      float4* P = reinterpret_cast<float4*>(y + ((((((size_t)band << log_na) + ja) * 32 + lane) * 32 + jb) << 5));
+      float2 x[32];
+#pragma unroll
+      for (int m = 0; m < 32; m += 2) {
+        const float4 t = P[m >> 1];
+        x[brev<32>(m)] = make_float2(t.x, t.y);
+        x[brev<32>(m + 1)] = make_float2(t.z, t.w);
+      }
+      fft_dit<32>(x);                                                      // over m -> jm
+#pragma unroll
+      for (int jm = 0; jm < 32; jm += 2) P[(jm >> 1) ^ (jb & 15)] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
+      continue;
+    }
     float2* Y = y + (((size_t)band << log_n1) + (size_t)j1) * kN2;
     float2 x[32];
 #pragma unroll
@@ -422,10 +448,57 @@ struct EffSrc {
   const int* holes;       // shared memory: [2h] = first bin of hole h, [2h+1] = one past its last bin
 };
 
-constexpr int kWStride = 34;                      // float2 per row of a warp's tile (272 B: 16-byte aligned, conflict-free)
-constexpr int kWTile = 32 * kWStride;             // float2 per warp
-constexpr size_t kP1WSmem = (size_t)(8 * kWTile + 8 * 32) * sizeof(float2);     // tiles + per-warp TW tables
+// A warp's tile: 32 rows (jb) of 256 B, no padding; the 16-byte chunk ch of row r sits at chunk ch ^ (r & 15) (wz), which
+// makes the column writes of phase 1, the row reads / writes of phase 2 (16 bytes per lane) and the bulk copy's linear
+// read all conflict-free.  The tile reaches the band buffer as it is (pass 2 undoes the swizzle when it reads).
+constexpr int kWTile = 32 * 32;                   // float2 per warp (8 KB)
+#ifndef GWMF_P1_WARPS
+#define GWMF_P1_WARPS 4
+#endif
+#ifndef GWMF_P1_CTAS
+#define GWMF_P1_CTAS 4
+#endif
+#ifndef GWMF_P1_JA
+#define GWMF_P1_JA 4
+#endif
+constexpr int kP1Warps = GWMF_P1_WARPS;           // warps (values of c) per CTA of k_pass1_eff
+constexpr int kP1Groups = 32 / kP1Warps;          // CTAs (column groups cg) per ja
+constexpr size_t kP1WSmem = (size_t)(kP1Warps * kWTile + kP1Warps * 32) * sizeof(float2);     // tiles + per-warp TW tables
+__device__ __forceinline__ int wz(int r, int m) { return r * 32 + (m ^ ((r & 15) << 1)); }   // cell (row r, element m)
 
+// 16-byte shared-memory access at (addr ^ x): the XOR is part of the asm so that the 16 addresses of a row are formed
+// where they are used instead of being kept in registers
+__device__ __forceinline__ float4 lds128_x(unsigned addr, unsigned x) {
+  float4 v;
+  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %4, %5;\n\tld.shared.v4.f32 {%0, %1, %2, %3}, [a];\n\t}"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+               : "r"(addr), "r"(x));
+  return v;
+}
+__device__ __forceinline__ void sts128_x(unsigned addr, unsigned x, float4 v) {
+  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %0, %1;\n\tst.shared.v4.f32 [a], {%2, %3, %4, %5};\n\t}" ::"r"(addr), "r"(x),
+               "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w)
+               : "memory");
+}
+// 8-byte accesses to cell (row i, element m = lane) of a warp's swizzled tile: byte address ((col ^ x) + off) with
+// col = tile | lane * 8, x = (i & 15) << 4, off = i * 256 (the XOR and the offset are part of the asm: nothing is hoisted)
+__device__ __forceinline__ void sts64_xo(unsigned col, unsigned x, unsigned off, float2 v) {
+  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %0, %1;\n\tadd.u32 a, a, %2;\n\tst.shared.v2.f32 [a], {%3, %4};\n\t}" ::"r"(col), "r"(x),
+               "r"(off), "f"(v.x), "f"(v.y)
+               : "memory");
+}
+__device__ __forceinline__ float2 lds64_xo(unsigned col, unsigned x, unsigned off) {
+  float2 v;
+  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %2, %3;\n\tadd.u32 a, a, %4;\n\tld.shared.v2.f32 {%0, %1}, [a];\n\t}"
+               : "=f"(v.x), "=f"(v.y)
+               : "r"(col), "r"(x), "r"(off));
+  return v;
+}
+__device__ __forceinline__ void ldgsts_xo(unsigned col, unsigned x, unsigned off, const float2* p, bool ok) {
+  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %0, %1;\n\tadd.u32 a, a, %2;\n\tcp.async.ca.shared.global [a], [%3], 8, %4;\n\t}" ::"r"(col),
+               "r"(x), "r"(off), "l"(p), "r"(ok ? 8 : 0)
+               : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -455,11 +528,11 @@ __device__ __forceinline__ void ldgsts_pred(float2* slot, const float2* p, bool 
 }
 
 // Phase 1 of a warp (lane = m, column k2 = 32 lane + c): leaves v[jb], jb = 0..31 in natural order.
-// col: the lane's column of the warp's tile (tile + lane), rows i at stride kWStride -- used as the landing zone of the
+// tile: the warp's tile; the lane's column of it (cells wz(i, lane)) is used as the landing zone of the
 // cp.async rounds, a lane only touches its own column.  TW: the warp's table (shared).
 template <int RMAX, bool HOLES>
 __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float2* __restrict__ TW,
-                                           float2* __restrict__ col, int ja, int c, int lane, float2 (&v)[32]) {
+                                           float2* __restrict__ tile, int ja, int c, int lane, float2 (&v)[32]) {
   const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
   const int T = RMAX < 32 ? 1 : (R + 31) >> 5;
@@ -468,24 +541,30 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
   const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
   const float2* __restrict__ base = es.src + c * 32 + lane;            // + k1 * 1024 (k1 < 0 in the lower half of a pair spectrum)
   const float2* safe = es.src + (size_t)(row_lo < 0 ? 0 : row_lo) * kN2;
+  const unsigned col = (unsigned)__cvta_generic_to_shared(tile) | ((unsigned)lane << 3);     // the tile is 256 B aligned
 
   // top round (t = T - 1) straight into the registers of the transform; the one below it through cp.async at the same time
   {
     const int r0 = row_lo + 32 * (T - 1);
+    const float2* __restrict__ p0 = base + (ptrdiff_t)r0 * kN2;
 #pragma unroll
     for (int i = 0; i < RMAX; ++i) {
       const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
-      v[brev<32>(i)] = ldg_pred(base + (ptrdiff_t)(r0 + i) * kN2, ok);
+      v[brev<32>(i)] = ldg_pred(p0 + i * kN2, ok);
     }
   }
+  // the previous tile's bulk store must have read the tile before anything is written to it
+  if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+  __syncwarp();
   if constexpr (RMAX == 32) {
     if (T > 1) {
       auto request = [&](int t) {
         const int r0 = row_lo + 32 * t;
+        const float2* __restrict__ p0 = base + (ptrdiff_t)r0 * kN2;
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
           const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
-          ldgsts_pred(col + i * kWStride, ok ? base + (ptrdiff_t)(r0 + i) * kN2 : safe, ok);
+          ldgsts_xo(col, (i & 15) << 4, i * 256, ok ? p0 + i * kN2 : safe, ok);
         }
         cp_async_commit();
       };
@@ -496,7 +575,7 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
         cp_async_wait_all();
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
-          const float2 val = col[i * kWStride], w = v[brev<32>(i)];
+          const float2 val = lds64_xo(col, (i & 15) << 4, i * 256), w = v[brev<32>(i)];
           v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
         }
         if (t > 0) request(t - 1);
@@ -509,25 +588,26 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
 }
 
 template <bool HOLES>
-__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float2* TW, float2* col, int ja, int c, int lane,
+__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float2* TW, float2* tile, int ja, int c, int lane,
                                          float2 (&v)[32]) {
   const int R = ((es.e_hi - 1) >> kLogN2) - (es.e_lo >> kLogN2) + 1;
-  if (R <= 4) eff_phase1<4, HOLES>(a, es, TW, col, ja, c, lane, v);
-  else if (R <= 8) eff_phase1<8, HOLES>(a, es, TW, col, ja, c, lane, v);
-  else if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, col, ja, c, lane, v);
-  else eff_phase1<32, HOLES>(a, es, TW, col, ja, c, lane, v);
+  if (R <= 4) eff_phase1<4, HOLES>(a, es, TW, tile, ja, c, lane, v);
+  else if (R <= 8) eff_phase1<8, HOLES>(a, es, TW, tile, ja, c, lane, v);
+  else if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, tile, ja, c, lane, v);
+  else eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
 }
 
-__global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
-  extern __shared__ __align__(128) float2 smem[];
+__global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
+  extern __shared__ __align__(1024) float2 smem[];
   __shared__ int s_holes[2 * kMaxBands];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  float2* tile = smem + warp * kWTile;          // this warp's [32][kWStride] tile
-  float2* TW = smem + 8 * kWTile + warp * 32;   // this warp's e^{2 pi i ja (row_lo + i)/n1}
+  float2* tile = smem + warp * kWTile;          // this warp's swizzled [32][32] tile (wz)
+  float2* TW = smem + kP1Warps * kWTile + warp * 32;   // this warp's e^{2 pi i ja (row_lo + i)/n1}
   const int na = a.n1 >> 5, n1m = a.n1 - 1;
-  const int cg = blockIdx.x & 3, ja = blockIdx.x >> 2;
-  const int c = 8 * cg + warp;
+  const int cg = blockIdx.x % kP1Groups, ja0 = (blockIdx.x / kP1Groups) * a.ja_per_cta;
+  const int ja1 = ja0 + a.ja_per_cta < na ? ja0 + a.ja_per_cta : na;
+  const int c = kP1Warps * cg + warp;
   const int slot = blockIdx.y;                  // batch-relative
   const unsigned nmask = (1u << a.log_n) - 1u;
 
@@ -544,10 +624,6 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
            : d.kind == kEffUP ? a.ubuf + (size_t)(tb + 1) * kUCap              // bin 0 of the pair spectrum; bins run negative
                               : a.q + (size_t)tb * (size_t)(1u << (a.log_n - 1));
   const int row_lo = es.e_lo >> kLogN2;
-  TW[lane] = __ldg(&a.tw_n1[(ja * (row_lo + lane)) & n1m]);
-  __syncwarp();
-
-  float2 v[32];
   if (d.n_holes > 0) {                          // rare: class-D bands inside the hull of Z (CTA-uniform branch)
     if (tid == 0) {
       const TemplateMeta* mt = a.meta + tb;
@@ -560,13 +636,22 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
       }
     }
     __syncthreads();
-    eff_warp<true>(a, es, TW, tile + lane, ja, c, lane, v);
-  } else {
-    eff_warp<false>(a, es, TW, tile + lane, ja, c, lane, v);
   }
+  // The warp walks over its ja values.  The bulk store of a tile is only waited for when the tile is written again
+  // (eff_phase1, after the next tile's loads have been issued); TW of the next ja is fetched one iteration ahead.
+  float2 tw_next = __ldg(&a.tw_n1[(ja0 * (row_lo + lane)) & n1m]);
+#pragma unroll 1
+  for (int ja = ja0; ja < ja1; ++ja) {
+  TW[lane] = tw_next;
+  __syncwarp();
+  if (ja + 1 < ja1) tw_next = __ldg(&a.tw_n1[((ja + 1) * (row_lo + lane)) & n1m]);
+  float2 v[32];
+  if (d.n_holes > 0) eff_warp<true>(a, es, TW, tile, ja, c, lane, v);
+  else eff_warp<false>(a, es, TW, tile, ja, c, lane, v);
   // the lane's column of the tile: tile[jb][m = lane]
+  const unsigned col = (unsigned)__cvta_generic_to_shared(tile) | ((unsigned)lane << 3);
 #pragma unroll
-  for (int jb = 0; jb < 32; ++jb) tile[jb * kWStride + lane] = v[jb];
+  for (int jb = 0; jb < 32; ++jb) sts64_xo(col, (jb & 15) << 4, jb * 256, v[jb]);
   __syncwarp();
 
   // ---- phase 2: lane = jb, row j1 = ja + NA jb
@@ -588,7 +673,8 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
   }
   float2 x[32];
   {
-    const float4* __restrict__ row = reinterpret_cast<const float4*>(tile + jb * kWStride);
+    // chunk ch of the lane's row sits at ch ^ (jb & 15): one XOR on the byte address per access
+    const unsigned row = (unsigned)__cvta_generic_to_shared(tile + jb * 32) | ((unsigned)(jb & 15) << 4);
     float2 wl = make_float2(1.f, 0.f);
 #pragma unroll
     for (int lo = 0; lo < 8; lo += 2) {
@@ -599,7 +685,7 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
 #pragma unroll
       for (int hi = 0; hi < 4; ++hi) {
         const int m = 8 * hi + lo;
-        const float4 t = row[m >> 1];                                  // tile[jb][m], tile[jb][m + 1]
+        const float4 t = lds128_x(row, (unsigned)(m >> 1) << 4);        // tile[jb][m], tile[jb][m + 1]
         const float2 t0 = make_float2(t.x, t.y), t1 = make_float2(t.z, t.w);
         x[brev<32>(m)] = cmul_tw(lo == 0 ? t0 : cmul_tw(t0, Wa), B[hi]);
         x[brev<32>(m + 1)] = cmul_tw(cmul_tw(t1, Wb), B[hi]);
@@ -607,20 +693,23 @@ __global__ void __launch_bounds__(256, 3) k_pass1_eff(P1Args a, const SlotDesc* 
     }
   }
   fft_dit<32>(x);                                   // over m -> jm
-  // stage the 256 B piece A[j1][c][0..31] in the lane's own row of the tile and send it off
+  // stage the 256 B piece A[j1][c][0..31] in the lane's own row of the tile (same swizzle); the whole 8 KB tile then
+  // leaves with ONE bulk copy: the band buffer is [slot][ja][c][jb][jm]
   {
-    float4* st = reinterpret_cast<float4*>(tile + jb * kWStride);
+    const unsigned row = (unsigned)__cvta_generic_to_shared(tile + jb * 32) | ((unsigned)(jb & 15) << 4);
 #pragma unroll
-    for (int jm = 0; jm < 32; jm += 2) st[jm >> 1] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
+    for (int jm = 0; jm < 32; jm += 2) sts128_x(row, (unsigned)(jm >> 1) << 4, make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y));
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic writes -> visible to the bulk copy engine
-  {
-    float2* dst = a.y + ((size_t)slot * a.n1 + (size_t)j1) * kN2 + c * 32;
-    const unsigned src = (unsigned)__cvta_generic_to_shared(tile + jb * kWStride);
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], 256;" ::"l"(dst), "r"(src) : "memory");
+  __syncwarp();
+  if (lane == 0) {
+    float2* dst = a.y + ((((size_t)slot * na + ja) * 32 + c) << 10);
+    const unsigned src = (unsigned)__cvta_generic_to_shared(tile);
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], 8192;" ::"l"(dst), "r"(src) : "memory");
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the copy's reads
   }
+  }   // ja
+  if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the copy's reads
 }
 
 constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 32 * kT1Stride) * sizeof(float2);
@@ -756,6 +845,7 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   args.eff = 0;
   args.slot_base = 0;
   args.first_template = 0;
+  args.ja_per_cta = 1;
   args.ubuf = nullptr;
   args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   args.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
@@ -828,6 +918,7 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid, cudaSt
   args.eff = 0;
   args.slot_base = 0;
   args.first_template = 0;
+  args.ja_per_cta = 1;
   args.ubuf = nullptr;
   return dispatch_p1<true>(c, args, st);
 }
@@ -851,6 +942,7 @@ static void fill_eff_args(Ctx* c, P1Args& args, int first, int count, int parity
   args.eff = 1;
   args.slot_base = c->h_eff[first];
   args.first_template = first;
+  args.ja_per_cta = 1;
   args.ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
 }
 
@@ -860,7 +952,8 @@ cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStrea
   fill_eff_args(c, args, first, count, parity);
   const int n_slots = c->h_eff[first + count] - c->h_eff[first];
   if (n_slots <= 0) return cudaSuccess;
-  k_pass1_eff<<<dim3(4 * c->na, n_slots), 256, kP1WSmem, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab));
+  args.ja_per_cta = c->na >= GWMF_P1_JA ? GWMF_P1_JA : c->na;
+  k_pass1_eff<<<dim3(kP1Groups * (c->na / args.ja_per_cta), n_slots), kP1Warps * 32, kP1WSmem, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab));
   c->launches++;
   return cudaGetLastError();
 }

@@ -16,6 +16,10 @@
 // reach HBM.  Samples with rho > threshold race for their (template, window) slot with a 128-bit
 // compare-and-swap on (rho, -index | chi^2): the result is the maximum, lowest index on ties,
 // whatever the order of arrival.
+#include <string.h>
+
+#include <cuda.h>          // CUtensorMap (types only: the encoder is fetched through cudaGetDriverEntryPoint)
+
 #include "fft_reg.cuh"
 #include "gwmf_internal.cuh"
 
@@ -104,6 +108,17 @@ __device__ __forceinline__ void bulk_load_row(void* dst, const void* src, unsign
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
           smem_u32(dst)),
       "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+
+// one row (ja, jb) of a slot of the decimated path's band buffer [slot][ja][c][jb][jm]: 32 pieces of 256 B, 8 KB apart,
+// gathered by ONE tensor copy (box {jm: 256 B, jb: 1, c: 32, tile: 1}); lands as [c][256 B] (SASS: UTMALDG)
+__device__ __forceinline__ void tensor_load_row(void* dst, const CUtensorMap* tmap, int jb, int tile, unsigned long long* bar,
+                                                unsigned long long policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4, %5}], [%6], %7;" ::"r"(
+          smem_u32(dst)),
+      "l"(tmap), "r"(0), "r"(jb), "r"(0), "r"(tile), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
 
@@ -234,6 +249,7 @@ __global__ void __launch_bounds__(kP2Warps * 32, 1) k_pass2(P2Args a) {
 struct P2EArgs {
   P2Args b;                   // b.meta: first template of the (pair-aligned) batch; b.n_rows: rows of [t_begin, t_begin + count)
   int slot_base;              // eff_prefix of the first template of the batch
+  int log_na;                 // log2(n1 / 32): j1 = ja + NA jb
   int batch;                  // templates of the batch (spectra and pass 1 were run for all of them)
   int t_begin;                // first template of the batch whose rows this launch processes (batch-relative)
 };
@@ -245,7 +261,7 @@ constexpr int kP2EWarps = 12;     // k_pass2_eff: 12 warps per SM with a ring of
 constexpr int kP2ERing = 2;       // latency of its per-row chains, not by HBM, once a template needs ~2 transforms
 
 template <bool SERIES, bool SINGLE>
-__global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea) {
+__global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, const __grid_constant__ CUtensorMap tmap) {
   const P2Args& a = ea.b;
   extern __shared__ __align__(128) float2 smem2[];
   __shared__ int s_slot0[kMaxBatch + 2];      // first slot of template tb (batch-relative)
@@ -282,11 +298,12 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea) {
     // item e of a row -> slot: a guest's item 1 is the pair band of its owner (slot 1 of template tb - 1)
     const int slot = (s_neff[tb] & 512) ? (pf_e == 1 ? s_slot0[tb - 1] + 1 : s_slot0[tb] + pf_e - (pf_e > 1 ? 1 : 0))
                                         : s_slot0[tb] + pf_e;
-    const float2* src = a.y + ((size_t)slot * a.n1 + j1) * kN2;
     const int b = pf_item % kP2ERing;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     mbar_expect_tx(&bars[b], kRowBytes);
-    bulk_load_row(bufs + b * kN2, src, kRowBytes, &bars[b], ((s_neff[tb] & 512) && pf_e == 1) ? policy_keep : policy);
+    // j1 = ja + NA jb: tile (slot, ja), row jb of each of its 32 pieces
+    tensor_load_row(bufs + b * kN2, &tmap, j1 >> ea.log_na, (slot << ea.log_na) + (j1 & ((1 << ea.log_na) - 1)), &bars[b],
+                    ((s_neff[tb] & 512) && pf_e == 1) ? policy_keep : policy);
   };
   auto advance = [&]() {
     ++pf_item;
@@ -322,7 +339,9 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea) {
       mbar_wait(&bars[b], (item / kP2ERing) & 1);
       float2 x[32];
 #pragma unroll
-      for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(cur[32 * c + lane], tw_s[32 * c + lane]);     // lane = jm
+      // pass 1 stores the 16-byte chunk ch of a 256 B piece at chunk ch ^ (jb & 15)
+      const int sl = lane ^ (((j1 >> ea.log_na) & 15) << 1);
+      for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(cur[32 * c + sl], tw_s[32 * c + lane]);       // lane = jm
       fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
       __syncwarp();                                                         // every lane holds its 32 values
       if (pf_row >= 0) {
@@ -632,6 +651,30 @@ cudaError_t configure_pass2() {
   return e;
 }
 
+// The band buffer of the decimated path as a tensor of fp32: dims (fastest first) {64 floats = 32 jm, 32 jb, 32 c,
+// tiles = y_slots * NA}; pass 2 fetches row (ja, jb) of a slot with the box {64, 1, 32, 1} = 8 KB.  cuTensorMapEncodeTiled
+// is fetched from the driver at run time (no libcuda at link time).
+cudaError_t make_band_tensor_map(Ctx* c) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess) return e;
+  if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+  const int na = c->n1 / 32;
+  if (na < 1) { memset(&c->band_tmap, 0, sizeof(c->band_tmap)); return cudaSuccess; }     // n = 2^14 never takes this path
+  const cuuint64_t dims[4] = {64, 32, 32, (cuuint64_t)c->lay.y_slots * (cuuint64_t)na};
+  const cuuint64_t strides[3] = {256, 8192, 262144};                                       // bytes, dims 1..3
+  const cuuint32_t box[4] = {64, 1, 32, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUresult r = reinterpret_cast<EncodeFn>(fn)(&c->band_tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->ws + c->lay.y, dims, strides,
+                                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 static int p2_grid(const Ctx* c, int n_rows) {
   const int want = (n_rows + kP2Warps - 1) / kP2Warps;
   return want < c->n_sms ? want : c->n_sms;               // persistent: at most one CTA per SM
@@ -704,16 +747,17 @@ cudaError_t launch_pass2_eff(Ctx* c, int bfirst, int bcount, int first, int coun
   a.n_rows = count * c->n1;
   a.thresh = (float)c->prm.rho_thresh;
   ea.slot_base = c->h_eff[bfirst];
+  ea.log_na = c->log_n - kLogN2 - 5;
   ea.batch = bcount;
   ea.t_begin = first - bfirst;
   const bool single = c->prm.p == 1 || c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND;   // one effective band per template
   const bool series = series_rho || series_chi;
   const int want = (a.n_rows + kP2EWarps - 1) / kP2EWarps;
   const dim3 grid(want < c->n_sms ? want : c->n_sms);       // persistent: at most one CTA per SM
-  if (single && series) k_pass2_eff<true, true><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
-  else if (single) k_pass2_eff<false, true><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
-  else if (series) k_pass2_eff<true, false><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
-  else k_pass2_eff<false, false><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea);
+  if (single && series) k_pass2_eff<true, true><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea, c->band_tmap);
+  else if (single) k_pass2_eff<false, true><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea, c->band_tmap);
+  else if (series) k_pass2_eff<true, false><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea, c->band_tmap);
+  else k_pass2_eff<false, false><<<grid, kP2EWarps * 32, kP2ESmem, c->stream>>>(ea, c->band_tmap);
   c->launches++;
   return cudaGetLastError();
 }
