@@ -104,8 +104,9 @@ Layout make_layout(const gwmf_params* p) {
   L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
   L.qb = take(path == GWMF_PATH_FUSED ? 2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2) : 256);   // band-separated copy (k_fused)
   // decimated path: per-band one-sided power spectra W_l and their sum U+, double-buffered across batches
-  L.wbuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * (size_t)p->p * kUCap * sizeof(float2) : 256);
+  L.wbuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * (size_t)p->p * kSubMax * kUCap * sizeof(float2) : 256);
   L.ubuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * kUCap * sizeof(float2) : 256);
+  L.bp_jobs = take(path == GWMF_PATH_DECIMATED ? bp_jobs_bytes() : 256);
   size_t yb = (size_t)L.y_slots * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;
@@ -117,6 +118,15 @@ Layout make_layout(const gwmf_params* p) {
 bool create_upload_side(Ctx* c) {
   if (cudaStreamCreateWithFlags(&c->upload, cudaStreamNonBlocking) != cudaSuccess) return false;
   if (cudaEventCreateWithFlags(&c->ev_last_load, cudaEventDisableTiming) != cudaSuccess) return false;
+  if (cudaEventCreateWithFlags(&c->ev_bp_fork, cudaEventDisableTiming) != cudaSuccess) return false;
+  {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);
+    for (int i = 0; i < 3; ++i) {
+      if (cudaStreamCreateWithPriority(&c->bp[i], cudaStreamNonBlocking, hi) != cudaSuccess) return false;
+      if (cudaEventCreateWithFlags(&c->ev_bp_join[i], cudaEventDisableTiming) != cudaSuccess) return false;
+    }
+  }
   for (int b = 0; b < 2; ++b) {
     if (cudaMallocHost((void**)&c->h_stage[b], sizeof(float) * (size_t)c->n) != cudaSuccess) return false;
     if (cudaEventCreateWithFlags(&c->ev_seg_ready[b], cudaEventDisableTiming) != cudaSuccess) return false;
@@ -129,6 +139,11 @@ bool create_upload_side(Ctx* c) {
 void destroy_upload_side(Ctx* c) {
   if (c->upload) { cudaStreamSynchronize(c->upload); cudaStreamDestroy(c->upload); c->upload = nullptr; }
   if (c->ev_last_load) cudaEventDestroy(c->ev_last_load);
+  if (c->ev_bp_fork) cudaEventDestroy(c->ev_bp_fork);
+  for (int i = 0; i < 3; ++i) {
+    if (c->bp[i]) { cudaStreamSynchronize(c->bp[i]); cudaStreamDestroy(c->bp[i]); c->bp[i] = nullptr; }
+    if (c->ev_bp_join[i]) cudaEventDestroy(c->ev_bp_join[i]);
+  }
   for (int b = 0; b < 2; ++b) {
     if (c->h_stage[b]) cudaFreeHost(c->h_stage[b]);
     if (c->ev_seg_ready[b]) cudaEventDestroy(c->ev_seg_ready[b]);
@@ -241,6 +256,8 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->pending_reset = false;
   c->upload = nullptr;
   c->ev_last_load = nullptr;
+  c->ev_bp_fork = nullptr;
+  for (int i = 0; i < 3; ++i) { c->bp[i] = nullptr; c->ev_bp_join[i] = nullptr; }
   for (int b = 0; b < 2; ++b) { c->h_stage[b] = nullptr; c->ev_seg_ready[b] = c->ev_seg_free[b] = c->ev_stage_free[b] = nullptr; }
   // > 48 KB of dynamic shared memory is an opt-in per function AND per device: do it for this context's device
   if (configure_pass1(c->path) != cudaSuccess || configure_pass2() != cudaSuccess || configure_bandpower() != cudaSuccess ||

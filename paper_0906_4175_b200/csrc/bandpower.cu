@@ -27,6 +27,7 @@ namespace gwmf {
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }        // one float2 of padding per 16: the
                                                                             // stride-1 groups of the last stage become conflict-free
 constexpr int kBpThreads = 256;
+constexpr int kBpSubThreads = 512;   // sub-grid CTAs (one per SM, 140 KB of shared memory): twice the threads
 constexpr int kTwLo = 128;            // e^{2 pi i t/L} = TWH[t >> 7] * TWL[t & 127]: two small shared tables instead of one
                                       // scattered 8-byte global load per twiddle (every lane in its own sector)
 constexpr size_t bp_smem(int log_l) {
@@ -42,60 +43,153 @@ struct BpTw {
   }
 };
 
+// Job lists of a batch, one per kernel: class 0..3 = bands on a grid of 2^11..2^14 points, class 4 = the sub-grid jobs
+// (band, r) of the bands on 2^15 / 2^16 points.  jobs[class][i] = tb << 16 | l << 8 | r.  The order inside a list is
+// whatever the atomics give: every job writes rows of its own, so the results do not depend on it.
+constexpr int kBpJobCap = kMaxBatch * kMaxBands * kSubMax;
+constexpr int kBpClasses = 5;
+__global__ void __launch_bounds__(1024) k_bp_jobs(const TemplateMeta* __restrict__ meta, int p, int count, int* __restrict__ jobs,
+                                                  int* __restrict__ n_jobs) {
+  __shared__ int s_n[kBpClasses];
+  if (threadIdx.x < kBpClasses) s_n[threadIdx.x] = 0;
+  __syncthreads();
+  for (int i = threadIdx.x; i < count * p; i += blockDim.x) {
+    const int tb = i / p, l = i - tb * p;
+    const TemplateMeta* mt = meta + tb;
+    if (!((mt->s_mask >> l) & 1u)) continue;
+    const int B = mt->edges[l + 1] - mt->edges[l];
+    int log_l = kLogLMin;
+    while ((1 << log_l) < 2 * B) ++log_l;
+    if (log_l <= 14) {
+      jobs[(log_l - kLogLMin) * kBpJobCap + atomicAdd(&s_n[log_l - kLogLMin], 1)] = (tb << 16) | (l << 8);
+    } else {
+      const int sub = 1 << (log_l - 14);
+      const int at = atomicAdd(&s_n[4], sub);
+      for (int r = 0; r < sub; ++r) jobs[4 * kBpJobCap + at + r] = (tb << 16) | (l << 8) | r;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < kBpClasses) n_jobs[threadIdx.x] = s_n[threadIdx.x];
+}
+
 // grid (p, templates of the batch), one kernel per coarse-grid size L = 2^LOG_L (a CTA whose band wants another size
 // exits at once): W[tb][l][m] = one-sided power spectrum of class-S band l, 0 <= m < B_l.
-template <int LOG_L>
-__global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
+// The CTAs of a launch walk over the job list of their class (k_bp_jobs): only CTAs with work are started.
+// SUB (LOG_L = 14 only): the band needs a grid of LT = 2^15 or 2^16 points.  CTA r = blockIdx.z < D = LT / L takes the
+// interleaved sub-grid j' = r + D j'':
+//     y[r + D j''] = sum_{i' < L} X_r[i'] e^{2 pi i j'' i'/L},   X_r[i'] = sum_q Q[e_l + i' + q L] e^{2 pi i r (i' + q L)/LT}
+// (the band's bins with the sub-grid's phase ramp, folded modulo L), and its share of the LT-point forward transform,
+//     U_l[m] += (1/LT) e^{-2 pi i r m/LT} W_r[m mod L],   W_r = L-point forward transform of |y[r + D j'']|^2,
+// goes to row r of the band's rows of wbuf; k_uspec adds the rows in a fixed order.
+template <int LOG_L, bool SUB>
+__global__ void __launch_bounds__(SUB ? kBpSubThreads : kBpThreads, LOG_L == 14 ? 1 : 2)
     k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q, const float2* __restrict__ tw_l,
-                float2* __restrict__ wbuf, int p, int half_n) {
+                float2* __restrict__ wbuf, int p, int half_n, const int* __restrict__ jobs, const int* __restrict__ n_jobs) {
   constexpr int L = 1 << LOG_L;
+  constexpr int NT = SUB ? kBpSubThreads : kBpThreads;
   constexpr int R3 = L / 1024;                    // last radix: 2, 4, 8, 16
   constexpr int S1 = L / 32;                      // stride of the first radix-32 stage
   constexpr int TWS = kLMax / L;                  // tw_l[t * TWS] = e^{2 pi i t / L}
+  constexpr int CLS = SUB ? 4 : LOG_L - kLogLMin; // job class (k_bp_jobs)
   extern __shared__ __align__(16) float2 sm[];
-  const int l = blockIdx.x, tb = blockIdx.y;
-  const TemplateMeta* mt = meta + tb;
-  if (!((mt->s_mask >> l) & 1u)) return;
-  const int e_lo = mt->edges[l], B = mt->edges[l + 1] - e_lo;
-  int log_l = kLogLMin;
-  while ((1 << log_l) < 2 * B) ++log_l;
-  if (log_l != LOG_L) return;
-  float2* __restrict__ wout = wbuf + ((size_t)tb * p + l) * kUCap;
+  __shared__ float2 s_fine[4];
+  const int n_job = n_jobs[CLS];
+  if ((int)blockIdx.x >= n_job) return;
   const int tid = threadIdx.x;
   float2* twl = sm + L + (L >> 4);
   float2* twh = twl + kTwLo;
-  for (int i = tid; i < kTwLo; i += kBpThreads) twl[i] = tw_l[i * TWS];
-  for (int i = tid; i < L / kTwLo; i += kBpThreads) twh[i] = tw_l[i * kTwLo * TWS];
+  for (int i = tid; i < kTwLo; i += NT) twl[i] = tw_l[i * TWS];
+  for (int i = tid; i < L / kTwLo; i += NT) twh[i] = tw_l[i * kTwLo * TWS];
   BpTw<LOG_L> tw;
   tw.hi = twh;
   tw.lo = twl;
 
+#pragma unroll 1
+  for (int job = blockIdx.x; job < n_job; job += gridDim.x) {
+  const int jd = jobs[CLS * kBpJobCap + job];     // tb << 16 | l << 8 | sub-grid r
+  const int tb = jd >> 16, l = (jd >> 8) & 255, r = jd & 255;
+  const TemplateMeta* mt = meta + tb;
+  const int e_lo = mt->edges[l], B = mt->edges[l + 1] - e_lo;
+  int log_lt = kLogLMin;                          // the band's whole grid LT = 2^log_lt (= L unless SUB)
+  while ((1 << log_lt) < 2 * B) ++log_lt;
+  float2* __restrict__ wout = wbuf + (((size_t)tb * p + l) * kSubMax + r) * kUCap;
+  __syncthreads();                                // the previous job of this CTA is done with shared memory; tables are in place
+
+  // e^{2 pi i t/LT}, LT = 2^15 or 2^16 (SUB): t = (t >> sh) on the L-point table times the few finer steps below it
+  const int sh = log_lt - LOG_L;                  // 1 or 2
+  if constexpr (SUB) {
+    if (tid < 4) {
+      float sn, cs;
+      sincospif(2.0f * (float)tid / (float)(1u << log_lt), &sn, &cs);
+      s_fine[tid] = make_float2(cs, sn);
+    }
+    __syncthreads();                              // twl / twh / s_fine are in place
+  }
+  auto sub_tw = [&](unsigned t) -> float2 {
+    t &= (1u << log_lt) - 1u;
+    const float2 coarse = tw((int)(t >> sh));
+    const unsigned lo = t & ((1u << sh) - 1u);
+    return lo ? cmul(coarse, s_fine[lo]) : coarse;
+  };
   // the band's bins -> shared memory.  Q is stored c-major inside each row of 1024 bins (cm_pos): walk the band's rows
   // position by position (coalesced) and scatter to the bin's place
-  for (int i = B + tid; i < L; i += kBpThreads) sm[pad16(i)] = make_float2(0.f, 0.f);
   {
     const int row_lo = e_lo >> kLogN2, n_rows = ((e_lo + B - 1) >> kLogN2) - row_lo + 1;
     const float2* __restrict__ qrows = q + (size_t)tb * half_n + (size_t)row_lo * kN2;
-    for (int idx = tid; idx < n_rows * kN2; idx += kBpThreads) {
-      const int i = ((row_lo + (idx >> kLogN2)) << kLogN2) + cm_pos(idx & (kN2 - 1)) - e_lo;
-      if (i >= 0 && i < B) sm[pad16(i)] = qrows[idx];
+    if constexpr (!SUB) {
+      for (int i = B + tid; i < L; i += NT) sm[pad16(i)] = make_float2(0.f, 0.f);
+      for (int idx = tid; idx < n_rows * kN2; idx += NT) {
+        const int i = ((row_lo + (idx >> kLogN2)) << kLogN2) + cm_pos(idx & (kN2 - 1)) - e_lo;
+        if (i >= 0 && i < B) sm[pad16(i)] = qrows[idx];
+      }
+    } else {
+      // X_r[i mod L] += Q[e_l + i] e^{2 pi i r i/LT}: a cell receives at most two terms (B <= LT / 2 = 2 L), so the
+      // shared-memory adds commute and the result does not depend on their order
+      for (int i = tid; i < L; i += NT) sm[pad16(i)] = make_float2(0.f, 0.f);
+      __syncthreads();
+      for (int idx0 = tid; idx0 < n_rows * kN2; idx0 += 4 * NT) {
+        float2 v[4];
+        int ii[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {                                      // four loads in flight
+          const int idx = idx0 + u * NT;
+          ii[u] = ((row_lo + (idx >> kLogN2)) << kLogN2) + cm_pos(idx & (kN2 - 1)) - e_lo;
+          if (idx >= n_rows * kN2 || ii[u] >= B) ii[u] = -1;
+          v[u] = ii[u] >= 0 ? __ldg(qrows + idx) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (ii[u] < 0) continue;
+          const float2 t = r ? cmul(v[u], sub_tw((unsigned)r * (unsigned)ii[u])) : v[u];
+          float* dst = reinterpret_cast<float*>(&sm[pad16(ii[u] & (L - 1))]);
+          atomicAdd(dst, t.x);
+          atomicAdd(dst + 1, t.y);
+        }
+      }
     }
   }
   __syncthreads();
-  // ---- inverse transform, decimation in frequency: stage 1 (inputs i >= L/2 are zero since L >= 2B)
+  // ---- inverse transform, decimation in frequency: stage 1 (!SUB: inputs i >= L/2 are zero since L >= 2B)
 #pragma unroll 1
-  for (int o = tid; o < S1; o += kBpThreads) {
+  for (int o = tid; o < S1; o += NT) {
     float2 x[32];
 #pragma unroll
-    for (int qq = 0; qq < 16; ++qq) x[brev<32>(qq)] = sm[pad16(o + S1 * qq)];
-    fft_dit<32, 16>(x);
+    if constexpr (!SUB) {
+#pragma unroll
+      for (int qq = 0; qq < 16; ++qq) x[brev<32>(qq)] = sm[pad16(o + S1 * qq)];
+      fft_dit<32, 16>(x);
+    } else {                                      // a folded band fills the whole sub-grid spectrum
+#pragma unroll
+      for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pad16(o + S1 * qq)];
+      fft_dit<32>(x);
+    }
 #pragma unroll
     for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = k == 0 ? x[0] : cmul(x[k], tw((o * k) & (L - 1)));
   }
   __syncthreads();
   // ---- stage 2: inside each block k1 of S1 = 32 R3 points
 #pragma unroll 1
-  for (int g = tid; g < S1; g += kBpThreads) {
+  for (int g = tid; g < S1; g += NT) {
     const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
     float2 x[32];
 #pragma unroll
@@ -107,7 +201,7 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
   __syncthreads();
   // ---- stage 3 (R3 points, stride 1), |y|^2, and the first stage of the way back (same groups, no twiddle)
 #pragma unroll 1
-  for (int g = tid; g < 1024; g += kBpThreads) {
+  for (int g = tid; g < 1024; g += NT) {
     const int base = g * R3;
     float2 x[R3];
 #pragma unroll
@@ -123,7 +217,7 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
   __syncthreads();
   // ---- decimation in time: twiddle first, then the radix-32 transform (transposes of stages 2 and 1)
 #pragma unroll 1
-  for (int g = tid; g < S1; g += kBpThreads) {
+  for (int g = tid; g < S1; g += NT) {
     const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
     float2 x[32];
 #pragma unroll
@@ -137,9 +231,9 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
   }
   __syncthreads();
   // last stage: only the outputs m = o + S1 k < B <= L/2 are wanted, i.e. k < 16; they leave straight to global memory
-  const float inv_l = 1.0f / (float)L;
+  const float inv_l = 1.0f / (float)(1u << log_lt);
 #pragma unroll 1
-  for (int o = tid; o < S1; o += kBpThreads) {
+  for (int o = tid; o < S1; o += NT) {
     float2 x[32];
 #pragma unroll
     for (int qq = 0; qq < 32; ++qq) {
@@ -147,65 +241,133 @@ __global__ void __launch_bounds__(kBpThreads, LOG_L == 14 ? 1 : 2)
       x[brev<32>(qq)] = qq == 0 ? v : cmul(v, tw((o * qq) & (L - 1)));
     }
     fft_dit<32>(x);
+    if constexpr (!SUB) {
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int m = o + S1 * k;
-      if (m < B) {
-        const float sc = m == 0 ? inv_l : 2.0f * inv_l;                  // one-sided: U+[m] = 2 U[m] for m > 0
-        wout[m] = make_float2(x[k].x * sc, -x[k].y * sc);               // conj: forward transform of a real series
+      for (int k = 0; k < 16; ++k) {
+        const int m = o + S1 * k;
+        if (m < B) {
+          const float sc = m == 0 ? inv_l : 2.0f * inv_l;                  // one-sided: U+[m] = 2 U[m] for m > 0
+          wout[m] = make_float2(x[k].x * sc, -x[k].y * sc);               // conj: forward transform of a real series
+        }
+      }
+    } else {
+      // W_r is periodic in m with period L: every m = m' + fold L < B gets conj(x) e^{-2 pi i r m/LT}
+#pragma unroll
+      for (int k = 0; k < 32; ++k) {
+        const float2 wc = make_float2(x[k].x, -x[k].y);                    // conj: forward transform of a real series
+        for (int m = o + S1 * k; m < B; m += L) {
+          const float sc = m == 0 ? inv_l : 2.0f * inv_l;                  // one-sided: U+[m] = 2 U[m] for m > 0
+          const float2 t = sub_tw((unsigned)r * (unsigned)m);
+          const float2 v = r ? cmul(wc, make_float2(t.x, -t.y)) : wc;      // e^{-2 pi i r m/LT}
+          wout[m] = make_float2(v.x * sc, v.y * sc);
+        }
       }
     }
   }
+  }   // job
 }
 
-// U+[tb][m] = sum over the class-S bands, ascending l (fixed order: bit-reproducible), 0 <= m < u_hi
-__device__ __forceinline__ float2 usum(const TemplateMeta* mt, const float2* __restrict__ wbuf, int tb, int p, int m) {
-  float2 acc = make_float2(0.f, 0.f);
-  unsigned s = mt->s_mask;
-  while (s) {
-    const int l = __ffs(s) - 1;
-    s &= s - 1;
-    if (m < mt->edges[l + 1] - mt->edges[l]) {
-      const float2 v = wbuf[((size_t)tb * p + l) * kUCap + m];
-      acc.x += v.x;
-      acc.y += v.y;
+// U+[tb][m] = sum over the rows of wbuf of the class-S bands, ascending (l, sub-grid): a fixed order, bit-reproducible.
+// The rows in use and their lengths are listed in shared memory once per CTA.
+constexpr int kUsEntries = kMaxBands * kSubMax;
+// called by one whole warp (lane = band)
+__device__ __forceinline__ void uspec_list(const TemplateMeta* mt, int tb, int p, int* s_row, int* s_len, int* s_n) {
+  const int l = threadIdx.x & 31;
+  const bool is_s = (mt->s_mask >> l) & 1u;
+  const int B = is_s ? mt->edges[l + 1] - mt->edges[l] : 0;
+  const int sub = !is_s ? 0 : B > kLMax ? 4 : B > kLMax / 2 ? 2 : 1;      // grid 2^16, 2^15, <= 2^14: rows of wbuf in use
+  int incl = sub;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (l >= d) incl += v;
+  }
+  for (int r = 0; r < sub; ++r) { s_row[incl - sub + r] = (tb * p + l) * kSubMax + r; s_len[incl - sub + r] = B; }
+  if (l == 31) *s_n = incl;
+}
+__device__ __forceinline__ void uspec_sum(const float2* __restrict__ wbuf, const int* s_row, const int* s_len, int n, int m0,
+                                          float2 (&acc)[4]) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) acc[i] = make_float2(0.f, 0.f);
+  for (int e = 0; e < n; ++e) {
+    const float2* __restrict__ row = wbuf + (size_t)s_row[e] * kUCap;
+    const int B = s_len[e];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int m = m0 + 256 * i;
+      if (m < B) {
+        const float2 v = __ldg(row + m);
+        acc[i].x += v.x;
+        acc[i].y += v.y;
+      }
     }
   }
-  return acc;
 }
 
 // Unpaired template: ubuf[tb][m] = U+[m] (one-sided, doubled for m > 0: its transform's real part is u).
 // Owner of a pair (tb, tb + 1): the two ubuf rows hold the pair spectrum P[m] = U_A[m] + i U_B[m], -up_hi < m < up_hi,
 // with bin 0 at the start of the guest's row; U_X[m] = U+_X[m] / 2 for m > 0, U_X[-m] = conj(U_X[m]) (two-sided
 // spectrum of a real series), so that ONE transform returns u_A + i u_B.
+// A CTA owns the 1024 bins m = 1024 b .. 1024 b + 1023 of one template (pair); the rows of 1024 bins are stored
+// c-major (cm_pos), as pass 1 reads them, so the results are transposed through shared memory and leave coalesced.
+// Bin -m sits in row floor(-m / 1024): row -b for m = 1024 b, row -b - 1 for the other 1023.
 __global__ void __launch_bounds__(256) k_uspec(const TemplateMeta* __restrict__ meta, const float2* __restrict__ wbuf,
                                                float2* __restrict__ ubuf, int p) {
-  const int tb = blockIdx.y, m = blockIdx.x * 256 + threadIdx.x;
+  __shared__ int s_row[2][kUsEntries], s_len[2][kUsEntries], s_n[2];
+  __shared__ float2 s_pos[kN2 + 32], s_neg[kN2 + 32];
+  const int tb = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
   const TemplateMeta* mt = meta + tb;
-  if (mt->pair == 2 || !mt->s_mask) return;               // a guest's spectrum is written by its owner
-  // rows of 1024 bins are stored c-major (cm_pos), as pass 1 reads them; bin -m sits in row floor(-m / 1024)
-  const int mp = (m & ~(kN2 - 1)) + cm_pos(m & (kN2 - 1));
-  if (mt->pair == 0) {
-    if (m < mt->u_hi) ubuf[(size_t)tb * kUCap + mp] = usum(mt, wbuf, tb, p, m);
-    return;
+  const int pair = mt->pair;
+  if (pair == 2 || !mt->s_mask) return;                   // a guest's spectrum is written by its owner
+  const int hi = pair ? mt->up_hi : mt->u_hi;
+  if (b * kN2 >= hi) return;
+  if (tid < 32) uspec_list(mt, tb, p, s_row[0], s_len[0], &s_n[0]);
+  else if (tid < 64 && pair) uspec_list(mt + 1, tb + 1, p, s_row[1], s_len[1], &s_n[1]);
+  __syncthreads();
+  const int m0 = b * kN2 + tid;
+  float2 ua[4], ub[4];
+  uspec_sum(wbuf, s_row[0], s_len[0], s_n[0], m0, ua);
+  if (pair) uspec_sum(wbuf, s_row[1], s_len[1], s_n[1], m0, ub);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int k2 = tid + 256 * i, pp = cm_pos(k2);
+    if (!pair) {
+      s_pos[pp + (pp >> 5)] = ua[i];
+    } else {
+      const int kn = (kN2 - k2) & (kN2 - 1), pn = cm_pos(kn);              // bin -m has k2' = (-m) mod 1024
+      float2 vp, vn;
+      if (m0 + 256 * i == 0) {
+        vp = vn = make_float2(ua[i].x, ub[i].x);                          // both are real at m = 0
+      } else {
+        vp = make_float2(0.5f * (ua[i].x - ub[i].y), 0.5f * (ua[i].y + ub[i].x));        // (U_A + i U_B) / 2
+        vn = make_float2(0.5f * (ua[i].x + ub[i].y), 0.5f * (ub[i].x - ua[i].y));        // (conj U_A + i conj U_B) / 2
+      }
+      s_pos[pp + (pp >> 5)] = vp;
+      s_neg[pn + (pn >> 5)] = vn;
+    }
   }
-  if (m >= mt->up_hi) return;
-  const float2 ua = usum(mt, wbuf, tb, p, m), ub = usum(mt + 1, wbuf, tb + 1, p, m);
-  float2* bin0 = ubuf + (size_t)(tb + 1) * kUCap;
-  if (m == 0) {
-    bin0[0] = make_float2(ua.x, ub.x);                    // both are real at m = 0
-  } else {
-    const int km = -m, kmp = (km & ~(kN2 - 1)) + cm_pos(km & (kN2 - 1));        // (km & ~1023) = 1024 floor(km / 1024) < 0
-    bin0[mp] = make_float2(0.5f * (ua.x - ub.y), 0.5f * (ua.y + ub.x));        // (U_A + i U_B) / 2
-    bin0[kmp] = make_float2(0.5f * (ua.x + ub.y), 0.5f * (ub.x - ua.y));       // (conj U_A + i conj U_B) / 2
+  __syncthreads();
+  float2* bin0 = ubuf + (size_t)(pair ? tb + 1 : tb) * kUCap;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int pos = tid + 256 * i, k2 = cm_pos(pos);
+    if (b * kN2 + k2 < hi) bin0[b * kN2 + pos] = s_pos[pos + (pos >> 5)];
+    if (pair) {
+      // k2' = k2: bin -(1024 b + 1024 - k2) for k2 >= 1 (row -b - 1); k2' = 0 is bin -1024 b (row -b; bin 0 itself for b = 0)
+      const int m = k2 ? (b + 1) * kN2 - k2 : b * kN2;
+      if (m < hi && m > 0) bin0[-(k2 ? b + 1 : b) * kN2 + pos] = s_neg[pos + (pos >> 5)];
+    }
   }
 }
 
+size_t bp_jobs_bytes() { return 2 * (size_t)(kBpClasses * kBpJobCap + 8) * sizeof(int); }
+
 cudaError_t configure_bandpower() {
-  cudaError_t e = cudaFuncSetAttribute(k_bandpower<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(11));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(12));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(13));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<14>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(14));
+  cudaError_t e = cudaFuncSetAttribute(k_bandpower<11, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(11));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<12, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(12));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<13, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(13));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<14, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(14));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bandpower<14, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bp_smem(14));
   return e;
 }
 
@@ -214,17 +376,41 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
   const size_t half = (size_t)(c->n / 2);
   const TemplateMeta* meta = ws_ptr<TemplateMeta>(c, c->lay.meta) + first;
   const float2* q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * half;
-  float2* wbuf = ws_ptr<float2>(c, c->lay.wbuf) + (size_t)parity * c->lay.batch * p * kUCap;
+  float2* wbuf = ws_ptr<float2>(c, c->lay.wbuf) + (size_t)parity * c->lay.batch * p * kSubMax * kUCap;
   float2* ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
   const float2* tw_l = ws_ptr<float2>(c, c->lay.tw_l);
-  const dim3 grid(p, count);
-  // one launch per coarse-grid size that the class threshold allows (a band of B bins uses L = 2^ceil(log2 2B) >= 2048)
-  k_bandpower<11><<<grid, kBpThreads, bp_smem(11), st>>>(meta, q, tw_l, wbuf, p, (int)half);
+  // job lists of the batch (one per kernel), then one launch per coarse-grid size that the class threshold allows (a band
+  // of B bins uses L = 2^ceil(log2 2B) >= 2048).  The kernels are independent and each fills only part of the device, so
+  // they run side by side: the larger grids on streams of their own between a fork and a join on st.
+  int* jobs = ws_ptr<int>(c, c->lay.bp_jobs) + (size_t)parity * (kBpClasses * kBpJobCap + 8);
+  int* n_jobs = jobs + kBpClasses * kBpJobCap;
+  k_bp_jobs<<<1, 1024, 0, st>>>(meta, p, count, jobs, n_jobs);
   c->launches++;
-  if (c->s_bins > 1024) { k_bandpower<12><<<grid, kBpThreads, bp_smem(12), st>>>(meta, q, tw_l, wbuf, p, (int)half); c->launches++; }
-  if (c->s_bins > 2048) { k_bandpower<13><<<grid, kBpThreads, bp_smem(13), st>>>(meta, q, tw_l, wbuf, p, (int)half); c->launches++; }
-  if (c->s_bins > 4096) { k_bandpower<14><<<grid, kBpThreads, bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half); c->launches++; }
-  k_uspec<<<dim3(c->s_bins / 256, count), 256, 0, st>>>(meta, wbuf, ubuf, p);
+  cudaError_t e;
+  const bool fork = c->s_bins > 1024;
+  if (fork && (e = cudaEventRecord(c->ev_bp_fork, st)) != cudaSuccess) return e;
+  const int g2 = 2 * c->n_sms, g1 = c->n_sms;     // resident CTAs of a kernel (2 per SM; 1 per SM for the 2^14-point grids)
+  k_bandpower<11, false><<<g2, kBpThreads, bp_smem(11), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+  c->launches++;
+  int used = 0;
+  auto side = [&](int i) -> cudaStream_t {
+    cudaStreamWaitEvent(c->bp[i], c->ev_bp_fork, 0);
+    used |= 1 << i;
+    return c->bp[i];
+  };
+  if (c->s_bins > 1024) { k_bandpower<12, false><<<g2, kBpThreads, bp_smem(12), side(0)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  if (c->s_bins > 2048) { k_bandpower<13, false><<<g2, kBpThreads, bp_smem(13), side(1)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  if (c->s_bins > 4096) { k_bandpower<14, false><<<g1, kBpThreads, bp_smem(14), side(2)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  if (c->s_bins > kLMax / 2) {                    // bands on grids of 2^15 or 2^16 points: up to kSubMax sub-grid jobs each
+    k_bandpower<14, true><<<g1, kBpSubThreads, bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+    c->launches++;
+  }
+  for (int i = 0; i < 3; ++i) {
+    if (!(used & (1 << i))) continue;
+    if ((e = cudaEventRecord(c->ev_bp_join[i], c->bp[i])) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(st, c->ev_bp_join[i], 0)) != cudaSuccess) return e;
+  }
+  k_uspec<<<dim3((c->s_bins + kN2 - 1) / kN2, count), 256, 0, st>>>(meta, wbuf, ubuf, p);
   c->launches++;
   return cudaGetLastError();
 }

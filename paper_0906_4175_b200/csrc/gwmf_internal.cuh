@@ -16,9 +16,10 @@ constexpr int kColsPerCta = 8;   // pass-1 column tile: 8 columns x 8 B = 64 B s
 constexpr int kP2Warps = 8;      // pass-2 rows (j1 values) per CTA, one warp each
 // Decimated path: a band of at most kSBinsMax bins is transformed on a coarse grid of L <= kLMax points (class S);
 // wider bands keep their own n-point transform (class D).  See bandpower.cu.
-constexpr int kSBinsMax = 8192;
-constexpr int kLMax = 16384;
+constexpr int kSBinsMax = 32768; // widest class-S band (bins)
+constexpr int kLMax = 16384;     // largest coarse grid one CTA transforms in shared memory
 constexpr int kLogLMin = 11;     // smallest coarse grid (2048 points)
+constexpr int kSubMax = 4;       // a band that needs L = 2^15 or 2^16 > kLMax points is done as L / kLMax interleaved sub-grids
 constexpr int kUCap = kSBinsMax; // entries of the one-sided power spectrum U+ kept per template
 // C-major order inside a row of 1024 bins: bin k2 = 32 m + c sits at position 32 c + m (an involution).  The spectra
 // the decimated path's first pass reads (Q, U+) are stored this way: its warps read with lane = m.
@@ -104,7 +105,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, total;
+         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, bp_jobs, total;
   size_t y_bytes;
   int batch;                     // most templates per launch
   int y_slots;                   // n-point transforms (n complex fp32 each) the band buffer holds
@@ -125,6 +126,8 @@ struct Ctx {
   cudaStream_t stream;
   cudaStream_t side;             // high-priority side stream for the low-volume pass-1 kernels
   cudaEvent_t ev_fork, ev_join;
+  cudaStream_t bp[3];            // decimated path: the band-power kernels of the larger coarse grids run side by side
+  cudaEvent_t ev_bp_fork, ev_bp_join[3];
   int n_templates;
   bool have_bank, have_segment;
   int path;                      // GWMF_PATH_TWO_PASS / _FUSED / _DECIMATED (resolved from gwmf_params::path at create)
@@ -182,6 +185,7 @@ cudaError_t configure_pass1(int path);
 cudaError_t configure_pass2();
 cudaError_t make_band_tensor_map(Ctx* c);   // needs lay.y, n1 (gwmf_create)
 cudaError_t configure_bandpower();
+size_t bp_jobs_bytes();                      // workspace of the band-power job lists (two batches)
 cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st);      // W_l, then U+
 cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
 cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);

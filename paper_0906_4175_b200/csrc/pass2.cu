@@ -22,6 +22,12 @@
 
 #include "fft_reg.cuh"
 #include "gwmf_internal.cuh"
+#ifndef GWMF_P2_TW4
+#define GWMF_P2_TW4 1
+#endif
+#ifndef GWMF_P2_EPI
+#define GWMF_P2_EPI 1
+#endif
 
 namespace gwmf {
 
@@ -257,8 +263,14 @@ struct P2EArgs {
 // SINGLE: every template of the launch has exactly one effective band (p = 1, or chi^2 on demand): z is that band's
 // transform, no sums over bands are kept, and the epilogue is one compare of |z|^2 against the threshold per sample
 // (chi^2 is 0 by definition for p = 1 and is filled in later by k_chisq_at in the on-demand mode).
-constexpr int kP2EWarps = 12;     // k_pass2_eff: 12 warps per SM with a ring of 2 rows each (192 KB): the kernel is bound by the
-constexpr int kP2ERing = 2;       // latency of its per-row chains, not by HBM, once a template needs ~2 transforms
+#ifndef GWMF_P2_WARPS
+#define GWMF_P2_WARPS 12
+#endif
+#ifndef GWMF_P2_RING
+#define GWMF_P2_RING 2
+#endif
+constexpr int kP2EWarps = GWMF_P2_WARPS;     // k_pass2_eff: 12 warps per SM with a ring of 2 rows each (192 KB): the kernel is bound by the
+constexpr int kP2ERing = GWMF_P2_RING;       // latency of its per-row chains, not by HBM, once a template needs ~2 transforms
 
 template <bool SERIES, bool SINGLE>
 __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, const __grid_constant__ CUtensorMap tmap) {
@@ -267,10 +279,13 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, con
   __shared__ int s_slot0[kMaxBatch + 2];      // first slot of template tb (batch-relative)
   __shared__ int s_neff[kMaxBatch + 2];       // rows to read | has_s << 8 | guest of a pair << 9
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float2* tw_s = smem2;                                               // [c][jm]
-  float2* bufs = smem2 + 1024 + warp * (kP2ERing * kN2);
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2EWarps * kP2ERing * kN2) + kP2ERing * warp;
-  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
+  float4* tw_s = reinterpret_cast<float4*>(smem2);                    // [c][jm]: {w, i w}, w = e^{2 pi i c jm/1024}
+  float2* bufs = smem2 + 2048 + warp * (kP2ERing * kN2);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 2048 + kP2EWarps * kP2ERing * kN2) + kP2ERing * warp;
+  for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
+    const float2 w = a.tw_p2[i];
+    tw_s[i] = make_float4(w.x, w.y, -w.y, w.x);
+  }
   for (int t = threadIdx.x; t < ea.batch; t += blockDim.x) {
     s_slot0[t] = a.meta[t].eff_prefix - ea.slot_base;
     const bool guest = a.meta[t].pair == 2;     // reads one row more than it owns: the pair band of template t - 1
@@ -341,7 +356,15 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, con
 #pragma unroll
       // pass 1 stores the 16-byte chunk ch of a 256 B piece at chunk ch ^ (jb & 15)
       const int sl = lane ^ (((j1 >> ea.log_na) & 15) << 1);
-      for (int c = 0; c < 32; ++c) x[brev<32>(c)] = cmul(cur[32 * c + sl], tw_s[32 * c + lane]);       // lane = jm
+      for (int c = 0; c < 32; ++c) {                                        // lane = jm
+        const float2 v = cur[32 * c + sl];
+#if GWMF_P2_TW4
+        const float4 w = tw_s[32 * c + lane];                              // v w = v.x w + v.y (i w): no negation of v
+        x[brev<32>(c)] = unpk(fma2(pk(v.y, v.y), pk(w.z, w.w), mul2(pk(v.x, v.x), pk(w.x, w.y))));
+#else
+        x[brev<32>(c)] = cmul(v, reinterpret_cast<const float2*>(tw_s)[2 * (32 * c + lane)]);
+#endif
+      }
       fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
       __syncwarp();                                                         // every lane holds its 32 values
       if (pf_row >= 0) {
@@ -353,16 +376,28 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, con
         const float scale = __ldg(&a.meta[tb].scale_rho2);
         const float thr_z2 = a.thresh * a.thresh * 0.999f / scale;            // rho^2 > thr^2  <=>  |z|^2 > thr^2 / scale
         Slot* slots_t = a.slots ? a.slots + (size_t)tb * a.n_windows : nullptr;
+        if constexpr (SERIES) {
 #pragma unroll
-        for (int jc = 0; jc < 32; ++jc) {
-          const float z2 = fmaf(x[jc].x, x[jc].x, x[jc].y * x[jc].y);
-          if constexpr (SERIES) {
+          for (int jc = 0; jc < 32; ++jc) {
+            const float z2 = fmaf(x[jc].x, x[jc].x, x[jc].y * x[jc].y);
             const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
             if (a.series_rho) a.series_rho[j] = sqrtf(z2 * scale);
             if (a.series_chi) a.series_chi[j] = 0.f;
+            if (z2 > thr_z2 && slots_t) emit_candidate(slots_t, j, z2 * scale, 0.f, a.thresh, a.log_w);
           }
-          if (z2 > thr_z2 && slots_t)
-            emit_candidate(slots_t, (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1), z2 * scale, 0.f, a.thresh, a.log_w);
+        } else {
+          // events are rare: one running maximum per lane, the per-sample test only where it crosses
+          float zmax = 0.f;
+#pragma unroll
+          for (int jc = 0; jc < 32; ++jc) zmax = fmaxf(zmax, fmaf(x[jc].x, x[jc].x, x[jc].y * x[jc].y));
+          if (zmax > thr_z2 && slots_t) {
+#pragma unroll
+            for (int jc = 0; jc < 32; ++jc) {
+              const float z2 = fmaf(x[jc].x, x[jc].x, x[jc].y * x[jc].y);
+              if (z2 > thr_z2)
+                emit_candidate(slots_t, (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1), z2 * scale, 0.f, a.thresh, a.log_w);
+            }
+          }
         }
         continue;
       }
@@ -392,20 +427,36 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, con
     const float fp_scale = (float)a.p * scale, inv_p = 1.0f / (float)a.p;
     const float thr2 = a.thresh * a.thresh * 0.999f;
     Slot* slots_t = a.slots ? a.slots + (size_t)tb * a.n_windows : nullptr;
+    if constexpr (SERIES) {
 #pragma unroll
-    for (int jc = 0; jc < 32; ++jc) {
-      const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
-      const float rho2 = z2 * scale;                                        // Eq. 3 squared
-      const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * fp_scale;         // Eq. 5
-      const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
-      if constexpr (SERIES) {
+      for (int jc = 0; jc < 32; ++jc) {
+        const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
+        const float rho2 = z2 * scale;                                        // Eq. 3 squared
+        const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * fp_scale;         // Eq. 5
+        const unsigned j = (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1);
         if (a.series_rho) a.series_rho[j] = sqrtf(rho2);
         if (a.series_chi) a.series_chi[j] = chi;
+        if (rho2 > thr2 && slots_t) emit_candidate(slots_t, j, rho2, chi, a.thresh, a.log_w);
       }
-      if (rho2 > thr2 && slots_t) emit_candidate(slots_t, j, rho2, chi, a.thresh, a.log_w);
-      az[jc] = make_float2(0.f, 0.f);
-      aq[jc] = 0.f;
+    } else {
+      // events are rare: one running maximum of |z|^2 per lane; rho, chi^2 and the slot update only where it crosses
+      float zmax = 0.f;
+#pragma unroll
+      for (int jc = 0; jc < 32; ++jc) zmax = fmaxf(zmax, fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y));
+      if (zmax * scale > thr2 && slots_t) {
+#pragma unroll
+        for (int jc = 0; jc < 32; ++jc) {
+          const float z2 = fmaf(az[jc].x, az[jc].x, az[jc].y * az[jc].y);
+          const float rho2 = z2 * scale;                                      // Eq. 3 squared
+          if (rho2 > thr2) {
+            const float chi = fmaxf(aq[jc] - z2 * inv_p, 0.f) * fp_scale;     // Eq. 5
+            emit_candidate(slots_t, (unsigned)j1 + ((unsigned)(lane + 32 * jc) << a.log_n1), rho2, chi, a.thresh, a.log_w);
+          }
+        }
+      }
     }
+#pragma unroll
+    for (int jc = 0; jc < 32; ++jc) { az[jc] = make_float2(0.f, 0.f); aq[jc] = 0.f; }
   }
 }
 
@@ -635,7 +686,7 @@ cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool u
 }
 
 constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
-constexpr size_t kP2ESmem = (size_t)(1024 + kP2EWarps * kP2ERing * kN2) * sizeof(float2) + kP2EWarps * kP2ERing * sizeof(unsigned long long);
+constexpr size_t kP2ESmem = (size_t)(2048 + kP2EWarps * kP2ERing * kN2) * sizeof(float2) + kP2EWarps * kP2ERing * sizeof(unsigned long long);
 
 // Opt-in to > 48 KB of dynamic shared memory on the CURRENT device (gwmf_create calls this for every context).
 cudaError_t configure_pass2() {
