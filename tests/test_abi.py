@@ -50,7 +50,7 @@ def test_workspace_bytes_host_only(lib):
     # (2 * 64 templates * p * 4 sub-grid rows * 32768 * 8 B = 2 GiB); double-buffered correlated spectra
     # (2 * 64 * 4 MiB = 512 MiB); tables / slots / staging
     assert (4 << 30) + (512 << 20) < b < (5 << 30)
-    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (360 << 20)
+    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (440 << 20)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
 
