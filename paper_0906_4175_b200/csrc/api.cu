@@ -107,10 +107,13 @@ Layout make_layout(const gwmf_params* p) {
   L.wbuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * (size_t)p->p * kSubMax * kUCap * sizeof(float2) : 256);
   L.ubuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * kUCap * sizeof(float2) : 256);
   L.bp_jobs = take(path == GWMF_PATH_DECIMATED ? bp_jobs_bytes() : 256);
+  L.pp_jobs = take((size_t)(L.y_slots + 8) * sizeof(int));
   size_t yb = (size_t)L.y_slots * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
   L.y_bytes = yb;
   L.y = take(yb);
+  // pre-passed bands of the decimated path (n1 >= 1024): a twin of the band buffer, slot for slot
+  L.vbuf = take(path == GWMF_PATH_DECIMATED && n1 >= 1024 ? (size_t)L.y_slots * n * sizeof(float2) : 256);
   L.total = off;
   return L;
 }
@@ -245,7 +248,8 @@ int gwmf_create(const gwmf_params* params, void* d_workspace, size_t workspace_b
   c->fused = c->path == GWMF_PATH_FUSED;
   c->device = dev;
   c->s_bins = (int)(params->n / 16 < kSBinsMax ? params->n / 16 : kSBinsMax);
-  c->t_max = 16;
+  // rounds of 32 input rows beyond which k_prepass pays (it leaves Q = NA / 32 rounds and costs about one transform's traffic)
+  c->t_max = c->n1 >= 1024 ? c->n1 / 1024 + 5 : (1 << 20);
   c->launches = 0;
   c->h_meta = nullptr;
   c->h_masks = nullptr;
@@ -438,23 +442,23 @@ static cudaError_t decimated_batch(Ctx* c, const Batch& b, const Batch* nx, int 
     if ((e = cudaEventRecord(ev[0], c->stream)) != cudaSuccess) return e;
     if ((e = launch_spectra(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
     if ((e = cudaEventRecord(ev[1], c->stream)) != cudaSuccess) return e;
-    if (gen && (e = launch_pass1_generic_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
+    if (gen && (e = launch_prepass(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
     if ((e = launch_pass1_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
     if ((e = cudaEventRecord(ev[2], c->stream)) != cudaSuccess) return e;
     if ((e = launch_pass2_eff(c, b.bfirst, b.bcount, b.first, b.count, update_slots, series_rho, series_chi)) != cudaSuccess) return e;
     return cudaEventRecord(ev[3], c->stream);
   }
   if (!ready && (e = launch_spectra(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
-  const bool side_work = gen || nx != nullptr;
+  const bool side_work = nx != nullptr;
   if (side_work) {
     // fork: everything enqueued so far on the main stream (this batch's spectra, the previous batch's pass 2, which
     // read the band buffer and the other half of the spectra buffers) precedes the side work
     if ((e = cudaEventRecord(c->ev_fork, c->stream)) != cudaSuccess) return e;
     if ((e = cudaStreamWaitEvent(c->side, c->ev_fork, 0)) != cudaSuccess) return e;
-    if (gen && (e = launch_pass1_generic_eff(c, b.bfirst, b.bcount, parity, c->side)) != cudaSuccess) return e;
     if (nx && (e = launch_spectra(c, nx->bfirst, nx->bcount, parity ^ 1, c->side)) != cudaSuccess) return e;
     if ((e = cudaEventRecord(c->ev_join, c->side)) != cudaSuccess) return e;
   }
+  if (gen && (e = launch_prepass(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
   if ((e = launch_pass1_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
   if (side_work && (e = cudaStreamWaitEvent(c->stream, c->ev_join, 0)) != cudaSuccess) return e;
   return launch_pass2_eff(c, b.bfirst, b.bcount, b.first, b.count, update_slots, series_rho, series_chi);

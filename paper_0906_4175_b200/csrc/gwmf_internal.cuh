@@ -44,7 +44,7 @@ struct TemplateMeta {
   //   then one per class-D band in ascending l (z_l itself: contributes to z and to sum |z_l|^2)
   uint32_t s_mask;               // bit l: band l is class S (0 < bins <= s_bins)
   uint32_t d_mask;               // bit l: band l is class D (bins > s_bins)
-  uint32_t gen_mask;             // bit e: effective band e goes through the generic pass-1 kernel (very many input rows)
+  uint32_t gen_mask;             // bit e: effective band e has very many input rows and is pre-passed (k_prepass)
   int32_t eff_prefix;            // effective bands of all earlier templates of the bank
   int32_t n_eff;                 // effective bands of this template
   int32_t z_lo, z_hi;            // hull of the class-S bands, bins [z_lo, z_hi)
@@ -64,7 +64,7 @@ struct alignas(32) SlotDesc {
   int32_t kind;                  // EffKind
   int32_t e_lo, e_hi;            // bins
   int32_t n_holes;               // Z only: class-D bands inside the hull (0 except for unusual spectra)
-  int32_t generic;               // 1: written by the generic kernel + row stage, not by k_pass1_eff
+  int32_t generic;               // 1: very many input rows: k_prepass reduces them to NA / 32 rounds read from vbuf
   int32_t pad0, pad1;
 };
 #ifdef __CUDACC__
@@ -105,7 +105,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, bp_jobs, total;
+         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, bp_jobs, vbuf, pp_jobs, total;
   size_t y_bytes;
   int batch;                     // most templates per launch
   int y_slots;                   // n-point transforms (n complex fp32 each) the band buffer holds
@@ -135,7 +135,7 @@ struct Ctx {
   int device;                    // CUDA device the context lives on
   CUtensorMap band_tmap;         // decimated path: the band buffer [tile = slot * NA + ja][c][jb][256 B] as a 4-d tensor (pass 2's row gather)
   int s_bins;                    // decimated path: class-S threshold in bins = min(kSBinsMax, n / 16)
-  int t_max;                     // decimated path: effective bands of more than 32 * t_max input rows use the generic kernel
+  int t_max;                     // decimated path: effective bands of more than 32 * t_max input rows are pre-passed (k_prepass)
   int32_t* h_eff;                // host mirror (pinned): eff_prefix[0 .. n_templates], then one "has generic band" flag per template
   bool mirror_ready;             // the host mirrors (h_masks, h_eff) have been waited for since the last bank setup
   int64_t launches;
@@ -188,7 +188,7 @@ cudaError_t configure_bandpower();
 size_t bp_jobs_bytes();                      // workspace of the band-power job lists (two batches)
 cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStream_t st);      // W_l, then U+
 cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
-cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st);
+cudaError_t launch_prepass(Ctx* c, int first, int count, int parity, cudaStream_t st);   // bands of very many rows -> vbuf
 cudaError_t launch_pass2_eff(Ctx* c, int bfirst, int bcount, int first, int count, bool update_slots, float* series_rho,
                              float* series_chi);
 cudaError_t launch_chisq_at_events(Ctx* c, int first, int count);      // chi^2 on demand: fills the slots' chi^2

@@ -13,6 +13,8 @@
 // Kernels:  k_correlate (Q once per template and bin), k_pass1_narrow (bands of <= 32 rows: column transform +
 // row stage in one CTA, writes A directly), k_pass1 (generic: wide bands and the dense transform, plain layout
 // Y) followed by k_rowstage (Y -> A in place).
+#include <limits.h>
+
 #include "fft_reg.cuh"
 #include "gwmf_internal.cuh"
 
@@ -37,6 +39,7 @@ struct P1Args {
   int first_template;         // bank index of the first template of the batch
   int ja_per_cta;             // k_pass1_eff: consecutive ja values a CTA walks over
   const float2* ubuf;         // [batch][kUCap] one-sided power spectra U+ (bandpower.cu)
+  const float2* vbuf;         // [slots][n] pre-passed bands (k_prepass)
 };
 
 // The effective bands of a batch whose bit is set in TemplateMeta::gen_mask, as (tb << 6 | e), ascending, identical
@@ -446,6 +449,7 @@ struct EffSrc {
   int e_lo, e_hi;
   int n_holes;            // Z only
   const int* holes;       // shared memory: [2h] = first bin of hole h, [2h+1] = one past its last bin
+  const float2* v;        // pre-passed band (k_prepass): V of this slot, else nullptr
 };
 
 // A warp's tile: 32 rows (jb) of 256 B, no padding; the 16-byte chunk ch of row r sits at chunk ch ^ (r & 15) (wz), which
@@ -535,18 +539,22 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
                                            float2* __restrict__ tile, int ja, int c, int lane, float2 (&v)[32]) {
   const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
-  const int T = RMAX < 32 ? 1 : (R + 31) >> 5;
+  const int T = RMAX < 32 ? 1 : es.v ? a.n1 >> 10 : (R + 31) >> 5;    // pre-passed band: Q = NA / 32 rounds, every row of V valid
   const int k2 = 32 * lane + c;
-  const int fr = row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);       // first / last row whose bin in THIS column is in the band
-  const int lr = row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
+  const int fr = es.v ? INT_MIN : row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);       // first / last row whose bin in THIS column is in the band
+  const int lr = es.v ? INT_MAX : row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
   const float2* __restrict__ base = es.src + c * 32 + lane;            // + k1 * 1024 (k1 < 0 in the lower half of a pair spectrum)
   const float2* safe = es.src + (size_t)(row_lo < 0 ? 0 : row_lo) * kN2;
   const unsigned col = (unsigned)__cvta_generic_to_shared(tile) | ((unsigned)lane << 3);     // the tile is 256 B aligned
 
+  // rows of round t: the band's rows row_lo + 32 t + i, or (pre-passed band, es.v != nullptr) the 32 rows b' = i of V[t][ja mod 32]
+  auto round_ptr = [&](int t) -> const float2* {
+    return es.v ? es.v + ((size_t)(t * 32 + (ja & 31)) * 32) * kN2 + c * 32 + lane : base + (ptrdiff_t)(row_lo + 32 * t) * kN2;
+  };
   // top round (t = T - 1) straight into the registers of the transform; the one below it through cp.async at the same time
   {
     const int r0 = row_lo + 32 * (T - 1);
-    const float2* __restrict__ p0 = base + (ptrdiff_t)r0 * kN2;
+    const float2* __restrict__ p0 = round_ptr(T - 1);
 #pragma unroll
     for (int i = 0; i < RMAX; ++i) {
       const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
@@ -560,7 +568,7 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
     if (T > 1) {
       auto request = [&](int t) {
         const int r0 = row_lo + 32 * t;
-        const float2* __restrict__ p0 = base + (ptrdiff_t)r0 * kN2;
+        const float2* __restrict__ p0 = round_ptr(t);
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
           const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
@@ -612,10 +620,10 @@ __global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Arg
   const unsigned nmask = (1u << a.log_n) - 1u;
 
   const SlotDesc d = slot_tab[a.slot_base + slot];      // one 32-byte load, same address in every thread
-  if (d.generic) return;                        // very many rows: k_pass1 (generic) + k_rowstage write this slot
   const int tb = d.t - a.first_template;
 
   EffSrc es;
+  es.v = d.generic ? a.vbuf + ((size_t)slot << a.log_n) : nullptr;      // very many rows: reduced to Q rounds by k_prepass
   es.e_lo = d.e_lo;
   es.e_hi = d.e_hi;
   es.holes = s_holes;
@@ -710,6 +718,59 @@ __global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Arg
   }
   }   // ja
   if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the copy's reads
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Pre-pass for effective bands of very many input rows (SlotDesc::generic; n1 >= 1024, NA = 32 Q).  The Horner sum
+// of k_pass1_eff over the T = ceil(R / 32) rounds t costs T multiply-adds per (ja, b', column) and re-reads the whole
+// band for every ja.  With t = t0 + Q t1 and G = e^{2 pi i ja/NA}, G^Q = e^{2 pi i ja/32} depends on ja mod 32 only:
+//     sum_t X_t G^t = sum_{t0 < Q} G^{t0} V[t0][ja mod 32],   V[t0][ja1][b'][.] = sum_{t1 < 32} X_{t0 + Q t1}[b'][.] e^{2 pi i ja1 t1/32}
+// so ONE 32-point transform per (t0, b', column) serves all ja, and k_pass1_eff is left with Q <= 4 rounds read from
+// V (n complex per band: the slot's twin in vbuf, rows c-major like Q).  Thread = (t0, b', position in the row);
+// the work items of a batch are listed by k_pp_jobs and walked grid-stride.
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_pp_jobs(const SlotDesc* __restrict__ slot_tab, int slot_base, int n_slots, int* __restrict__ list,
+                          int* __restrict__ n_list) {
+  __shared__ int s_n;
+  if (threadIdx.x == 0) s_n = 0;
+  __syncthreads();
+  for (int s = threadIdx.x; s < n_slots; s += blockDim.x)
+    if (slot_tab[slot_base + s].generic) list[atomicAdd(&s_n, 1)] = s;       // any order: a band's V is its own
+  __syncthreads();
+  if (threadIdx.x == 0) *n_list = s_n;
+}
+
+__global__ void __launch_bounds__(256) k_prepass(P1Args a, const SlotDesc* __restrict__ slot_tab, float2* __restrict__ vbuf,
+                                                  const int* __restrict__ list, const int* __restrict__ n_list) {
+  const int na = a.n1 >> 5, Q = na >> 5;
+  const int per_band = 4 * 32 * Q;               // CTAs per band: 4 position chunks x 32 b' x Q t0
+  const int n_items = *n_list * per_band;
+  const size_t n = (size_t)1 << a.log_n;
+#pragma unroll 1
+  for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const int slot = list[item / per_band];
+    int rem = item % per_band;
+    const int chunk = rem & 3;
+    rem >>= 2;
+    const int bp = rem & 31, t0 = rem >> 5;
+    const SlotDesc d = slot_tab[a.slot_base + slot];
+    const int tb = d.t - a.first_template;
+    const float2* __restrict__ src = a.q + (size_t)tb * (n >> 1);          // class D (or the whole template): read from Q
+    const int row_lo = d.e_lo >> kLogN2, row_hi = (d.e_hi - 1) >> kLogN2;
+    const int pos = chunk * 256 + threadIdx.x, k2 = cm_pos(pos);
+    const int fr = row_lo + (k2 < (d.e_lo & (kN2 - 1)) ? 1 : 0);           // first / last row whose bin in THIS column is in the band
+    const int lr = row_hi - (k2 > ((d.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
+    float2 x[32];
+#pragma unroll
+    for (int t1 = 0; t1 < 32; ++t1) {
+      const int k1 = row_lo + bp + 32 * (t0 + Q * t1);
+      x[brev<32>(t1)] = ldg_pred(src + (size_t)k1 * kN2 + pos, k1 >= fr && k1 <= lr);
+    }
+    fft_dit<32>(x);
+    float2* __restrict__ out = vbuf + (size_t)slot * n + ((size_t)(t0 * 32) * 32 + bp) * kN2 + pos;
+#pragma unroll
+    for (int ja1 = 0; ja1 < 32; ++ja1) out[(size_t)ja1 * 32 * kN2] = x[ja1];
+  }
 }
 
 constexpr size_t kNarrowSmem = (size_t)(32 * kStageStride + 32 * kT1Stride) * sizeof(float2);
@@ -847,6 +908,7 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   args.first_template = 0;
   args.ja_per_cta = 1;
   args.ubuf = nullptr;
+  args.vbuf = nullptr;
   args.tw_p2 = ws_ptr<float2>(c, c->lay.tw_p2);
   args.q = ws_ptr<float2>(c, c->lay.q) + (size_t)parity * c->lay.batch * (size_t)(c->n / 2);
   cudaError_t e;
@@ -920,6 +982,7 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid, cudaSt
   args.first_template = 0;
   args.ja_per_cta = 1;
   args.ubuf = nullptr;
+  args.vbuf = nullptr;
   return dispatch_p1<true>(c, args, st);
 }
 
@@ -944,6 +1007,7 @@ static void fill_eff_args(Ctx* c, P1Args& args, int first, int count, int parity
   args.first_template = first;
   args.ja_per_cta = 1;
   args.ubuf = ws_ptr<float2>(c, c->lay.ubuf) + (size_t)parity * c->lay.batch * kUCap;
+  args.vbuf = ws_ptr<float2>(c, c->lay.vbuf);
 }
 
 // first pass of every effective band of the batch (needs Q and U+ of the batch; host mirror h_eff valid)
@@ -958,13 +1022,17 @@ cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStrea
   return cudaGetLastError();
 }
 
-// the effective bands flagged in gen_mask: generic kernel (plain layout) + row stage, into their slots
-cudaError_t launch_pass1_generic_eff(Ctx* c, int first, int count, int parity, cudaStream_t st) {
+// the effective bands flagged in gen_mask (very many input rows): 32-point transform over the rounds, into vbuf
+cudaError_t launch_prepass(Ctx* c, int first, int count, int parity, cudaStream_t st) {
   P1Args args;
   fill_eff_args(c, args, first, count, parity);
-  cudaError_t e = dispatch_p1<false>(c, args, st);
-  if (e != cudaSuccess) return e;
-  return launch_rowstage(c, args.y, args.meta, count, 0, 2, st, args.slot_base);
+  const int n_slots = c->h_eff[first + count] - c->h_eff[first];
+  if (n_slots <= 0) return cudaSuccess;
+  int* list = ws_ptr<int>(c, c->lay.pp_jobs);
+  k_pp_jobs<<<1, 256, 0, st>>>(ws_ptr<SlotDesc>(c, c->lay.slot_tab), args.slot_base, n_slots, list + 1, list);
+  k_prepass<<<8 * c->n_sms, 256, 0, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab), ws_ptr<float2>(c, c->lay.vbuf), list + 1, list);
+  c->launches += 2;
+  return cudaGetLastError();
 }
 
 template <int NA, int NB>
