@@ -460,8 +460,11 @@ static cudaError_t decimated_batch(Ctx* c, const Batch& b, const Batch* nx, int 
   }
   if (gen && (e = launch_prepass(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
   if ((e = launch_pass1_eff(c, b.bfirst, b.bcount, parity, c->stream)) != cudaSuccess) return e;
+  if ((e = launch_pass2_eff(c, b.bfirst, b.bcount, b.first, b.count, update_slots, series_rho, series_chi)) != cudaSuccess) return e;
+  // join: the next batch's spectra may run beside BOTH passes of this batch (they fill the kernels' tails); the main
+  // stream only needs them before the next batch's first pass
   if (side_work && (e = cudaStreamWaitEvent(c->stream, c->ev_join, 0)) != cudaSuccess) return e;
-  return launch_pass2_eff(c, b.bfirst, b.bcount, b.first, b.count, update_slots, series_rho, series_chi);
+  return cudaSuccess;
 }
 
 // Cut [first, first + n) into launches: at most lay.batch templates each and, on the decimated path, at most

@@ -33,34 +33,13 @@ struct P1Args {
   int log_n;
   int n1;
   int batch;                  // templates in this launch
-  // decimated path (effective bands, gwmf_internal.cuh): y is indexed by slot = eff_prefix - slot_base + e
-  int eff;                    // 0: y is indexed by tb * p + l (two-pass / spill-free paths)
+  // decimated path (effective bands, gwmf_internal.cuh): the band buffer is indexed by slot = eff_prefix - slot_base + e
   int slot_base;              // eff_prefix of the first template of the batch
   int first_template;         // bank index of the first template of the batch
   int ja_per_cta;             // k_pass1_eff: consecutive ja values a CTA walks over
   const float2* ubuf;         // [batch][kUCap] one-sided power spectra U+ (bandpower.cu)
   const float2* vbuf;         // [slots][n] pre-passed bands (k_prepass)
 };
-
-// The effective bands of a batch whose bit is set in TemplateMeta::gen_mask, as (tb << 6 | e), ascending, identical
-// in every CTA.  s_list: batch * kMaxBands ints, s_cnt: batch + 1 ints of shared memory.  Returns the list length.
-__device__ inline int build_gen_list(const TemplateMeta* meta, int batch, int* s_list, int* s_cnt) {
-  for (int t = threadIdx.x; t < batch; t += blockDim.x) s_cnt[t] = __popc(meta[t].gen_mask);
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    int run = 0;
-    for (int t = 0; t < batch; ++t) { const int v = s_cnt[t]; s_cnt[t] = run; run += v; }
-    s_cnt[batch] = run;
-  }
-  __syncthreads();
-  for (int t = threadIdx.x; t < batch; t += blockDim.x) {
-    unsigned m = meta[t].gen_mask;
-    int o = s_cnt[t];
-    while (m) { const int e = __ffs(m) - 1; m &= m - 1; s_list[o++] = (t << 6) | e; }
-  }
-  __syncthreads();
-  return s_cnt[batch];
-}
 
 __device__ __forceinline__ float2 cis_frac(unsigned num, int log_n) {
   // e^{2 pi i num / 2^log_n}, num < 2^log_n <= 2^22: the argument 2 num / n is exact in fp32
@@ -87,7 +66,7 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
   // work list: the wide bands of the batch (DENSE: the one dense transform); every CTA builds the same list
   int n_list = 1;
   if constexpr (!DENSE)
-    n_list = a.eff ? build_gen_list(a.meta, a.batch, s_list, s_cnt) : build_wide_list(a.meta, a.batch, a.p, s_list, s_cnt);
+    n_list = build_wide_list(a.meta, a.batch, a.p, s_list, s_cnt);
 
   const int tid = threadIdx.x;
   const int x = tid >> 3, c = tid & 7;
@@ -98,21 +77,13 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 #pragma unroll 1
   for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
     const int tile = item % TILES, r = (item / TILES) % G;
-    int band_index = DENSE ? 0 : s_list[item / (TILES * G)];      // tb * p + l (eff: tb << 6 | e, replaced by the slot)
+    const int band_index = DENSE ? 0 : s_list[item / (TILES * G)];      // tb * p + l
     const int k2 = tile * C + c;
 
     int e_lo, e_hi, tb_q = 0;
     if constexpr (DENSE) {
       e_lo = 0;
       e_hi = 1 << a.log_n;
-    } else if (a.eff) {
-      const int tb = band_index >> 6, e = band_index & 63;
-      const TemplateMeta* m = a.meta + tb;
-      const EffBand eb = eff_band(m, e);                // only class-D bands are ever generic: src = Q, no holes
-      e_lo = eb.e_lo;
-      e_hi = eb.e_hi;
-      tb_q = tb;
-      band_index = m->eff_prefix - a.slot_base + e;
     } else {
       const int tb = band_index / a.p, l = band_index - tb * a.p;
       const TemplateMeta* m = a.meta + tb;
@@ -146,8 +117,7 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
             if constexpr (DENSE) {
               q = a.dense_in[k];
             } else {
-              // Q_I[k] from k_correlate (decimated path: rows stored c-major)
-              q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + (a.eff ? (k - k2) + cm_pos(k2) : k)];
+              q = a.q[(size_t)tb_q * (size_t)(1u << (a.log_n - 1)) + k];      // Q_I[k] from k_correlate
             }
             if constexpr (G > 1) {
               if (r > 0) q = cmul(q, a.tw_n1[(r * aa * NB) % n1]);         // w_NA^{r a}
@@ -174,13 +144,7 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) v[b] = S[m * SROW + b * C + c];
       fft_dif<NB>(v);
-      if (a.eff) {
-        // decimated path: the band buffer is [slot][ja][c][jb][.] (k_pass1_eff); Y[j1][32 mm + cc] goes to cell mm of
-        // the piece (ja, cc, jb), where the row stage (k_rowstage, mode 2) transforms it in place
-        float2* out = a.y + ((((size_t)band_index * NA + (size_t)(G * m + r)) * 32 + (k2 & 31)) << 10) + (k2 >> 5);
-#pragma unroll
-        for (int jb = 0; jb < NB; ++jb) out[jb * 32] = cmul(v[brev<NB>(jb)], Bt[jb * C + c]);
-      } else {
+      {
         float2* out = a.y + ((size_t)band_index * n1 + (size_t)(G * m + r)) * kN2 + k2;
 #pragma unroll
         for (int jb = 0; jb < NB; ++jb)
@@ -201,41 +165,16 @@ __global__ void __launch_bounds__(256, 2) k_pass1(P1Args a) {
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_rowstage(float2* __restrict__ y, const float2* __restrict__ tw_p2,
                                                   const TemplateMeta* __restrict__ meta, int batch, int p, int log_n1,
-                                                  int n_bands_all, int use_mask, int slot_base) {
-  // use_mask: 0 = every band, 1 = the wide bands (wide_mask), 2 = the generic effective bands (gen_mask, decimated path)
+                                                  int n_bands_all, int use_mask) {
+  // use_mask: 0 = every band, 1 = the wide bands (wide_mask)
   __shared__ int s_list[kMaxBatch * kMaxBands];
   __shared__ int s_cnt[kMaxBatch + 1];
-  const int n_list = use_mask == 2 ? build_gen_list(meta, batch, s_list, s_cnt)
-                   : use_mask ? build_wide_list(meta, batch, p, s_list, s_cnt) : n_bands_all;
-  if (use_mask == 2) {                                   // (tb << 6 | e) -> slot
-    for (int i = threadIdx.x; i < n_list; i += blockDim.x) {
-      const int v = s_list[i];
-      s_list[i] = meta[v >> 6].eff_prefix - slot_base + (v & 63);
-    }
-    __syncthreads();
-  }
+  const int n_list = use_mask ? build_wide_list(meta, batch, p, s_list, s_cnt) : n_bands_all;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long total_rows = (long long)n_list << log_n1;
   for (long long row = (long long)blockIdx.x * 8 + warp; row < total_rows; row += (long long)gridDim.x * 8) {
     const int w = (int)(row >> log_n1), j1 = (int)(row & ((1 << log_n1) - 1));
     const int band = use_mask ? s_list[w] : w;
-    if (use_mask == 2) {
-      // decimated path: lane = c owns the 256 B piece (ja, c, jb) of the slot, j1 = ja + NA jb; the result is stored
-      // with the 16-byte chunks swizzled as k_pass1_eff stores them (chunk ch at ch ^ (jb & 15))
-      const int log_na = log_n1 - 5, ja = j1 & ((1 << log_na) - 1), jb = j1 >> log_na;
-      float4* P = reinterpret_cast<float4*>(y + ((((((size_t)band << log_na) + ja) * 32 + lane) * 32 + jb) << 5));
-      float2 x[32];
-#pragma unroll
-      for (int m = 0; m < 32; m += 2) {
-        const float4 t = P[m >> 1];
-        x[brev<32>(m)] = make_float2(t.x, t.y);
-        x[brev<32>(m + 1)] = make_float2(t.z, t.w);
-      }
-      fft_dit<32>(x);                                                      // over m -> jm
-#pragma unroll
-      for (int jm = 0; jm < 32; jm += 2) P[(jm >> 1) ^ (jb & 15)] = make_float4(x[jm].x, x[jm].y, x[jm + 1].x, x[jm + 1].y);
-      continue;
-    }
     float2* Y = y + (((size_t)band << log_n1) + (size_t)j1) * kN2;
     float2 x[32];
 #pragma unroll
@@ -462,12 +401,15 @@ constexpr int kWTile = 32 * 32;                   // float2 per warp (8 KB)
 #ifndef GWMF_P1_CTAS
 #define GWMF_P1_CTAS 4
 #endif
+#ifndef GWMF_P1_VARIANTS
+#define GWMF_P1_VARIANTS 2
+#endif
 #ifndef GWMF_P1_JA
 #define GWMF_P1_JA 4
 #endif
 constexpr int kP1Warps = GWMF_P1_WARPS;           // warps (values of c) per CTA of k_pass1_eff
 constexpr int kP1Groups = 32 / kP1Warps;          // CTAs (column groups cg) per ja
-constexpr size_t kP1WSmem = (size_t)(kP1Warps * kWTile + kP1Warps * 32) * sizeof(float2);     // tiles + per-warp TW tables
+constexpr size_t kP1WSmem = (size_t)(kP1Warps * kWTile + kP1Warps * 64) * sizeof(float2);     // tiles + per-warp TW tables {w, i w}
 __device__ __forceinline__ int wz(int r, int m) { return r * 32 + (m ^ ((r & 15) << 1)); }   // cell (row r, element m)
 
 // 16-byte shared-memory access at (addr ^ x): the XOR is part of the asm so that the 16 addresses of a row are formed
@@ -535,7 +477,7 @@ __device__ __forceinline__ void ldgsts_pred(float2* slot, const float2* p, bool 
 // tile: the warp's tile; the lane's column of it (cells wz(i, lane)) is used as the landing zone of the
 // cp.async rounds, a lane only touches its own column.  TW: the warp's table (shared).
 template <int RMAX, bool HOLES>
-__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float2* __restrict__ TW,
+__device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float4* __restrict__ TW,
                                            float2* __restrict__ tile, int ja, int c, int lane, float2 (&v)[32]) {
   const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
@@ -577,32 +519,44 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
         cp_async_commit();
       };
       request(T - 2);
-      const tw4 g = make_tw4(a.tw_n1[(ja * 32) & (a.n1 - 1)]);                    // e^{2 pi i ja/NA}
+      const float2 g1 = a.tw_n1[(ja * 32) & (a.n1 - 1)];                          // e^{2 pi i ja/NA}
+      const pk2 g = pk(g1), ig = pk(-g1.y, g1.x);
 #pragma unroll 1
       for (int t = T - 2; t >= 0; --t) {
         cp_async_wait_all();
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
           const float2 val = lds64_xo(col, (i & 15) << 4, i * 256), w = v[brev<32>(i)];
-          v[brev<32>(i)] = unpk(fma2(pk(-w.y, w.x), g.yy, fma2(pk(w), g.xx, pk(val))));   // v g + val
+          v[brev<32>(i)] = unpk(fma2(pk(w.y, w.y), ig, fma2(pk(w.x, w.x), g, pk(val))));   // v g + val = w.x g + w.y (i g) + val
         }
         if (t > 0) request(t - 1);
       }
     }
   }
 #pragma unroll
-  for (int i = 0; i < RMAX; ++i) v[brev<32>(i)] = cmul(v[brev<32>(i)], TW[i]);
+  for (int i = 0; i < RMAX; ++i) {                 // v w = v.x w + v.y (i w): no negation of the data
+    const float4 w = TW[i];
+    const float2 x = v[brev<32>(i)];
+    v[brev<32>(i)] = unpk(fma2(pk(x.y, x.y), pk(w.z, w.w), mul2(pk(x.x, x.x), pk(w.x, w.y))));
+  }
   fft_dit<32, RMAX>(v);                     // inputs i >= RMAX are zero: leading stages pruned
 }
 
 template <bool HOLES>
-__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float2* TW, float2* tile, int ja, int c, int lane,
+__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float4* TW, float2* tile, int ja, int c, int lane,
                                          float2 (&v)[32]) {
   const int R = ((es.e_hi - 1) >> kLogN2) - (es.e_lo >> kLogN2) + 1;
+#if GWMF_P1_VARIANTS == 4
   if (R <= 4) eff_phase1<4, HOLES>(a, es, TW, tile, ja, c, lane, v);
   else if (R <= 8) eff_phase1<8, HOLES>(a, es, TW, tile, ja, c, lane, v);
   else if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, tile, ja, c, lane, v);
   else eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
+#elif GWMF_P1_VARIANTS == 2
+  if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, tile, ja, c, lane, v);
+  else eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
+#else
+  eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
+#endif
 }
 
 __global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
@@ -611,7 +565,7 @@ __global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Arg
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   float2* tile = smem + warp * kWTile;          // this warp's swizzled [32][32] tile (wz)
-  float2* TW = smem + kP1Warps * kWTile + warp * 32;   // this warp's e^{2 pi i ja (row_lo + i)/n1}
+  float4* TW = reinterpret_cast<float4*>(smem + kP1Warps * kWTile) + warp * 32;   // this warp's {w, i w}, w = e^{2 pi i ja (row_lo + i)/n1}
   const int na = a.n1 >> 5, n1m = a.n1 - 1;
   const int cg = blockIdx.x % kP1Groups, ja0 = (blockIdx.x / kP1Groups) * a.ja_per_cta;
   const int ja1 = ja0 + a.ja_per_cta < na ? ja0 + a.ja_per_cta : na;
@@ -650,7 +604,7 @@ __global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Arg
   float2 tw_next = __ldg(&a.tw_n1[(ja0 * (row_lo + lane)) & n1m]);
 #pragma unroll 1
   for (int ja = ja0; ja < ja1; ++ja) {
-  TW[lane] = tw_next;
+  TW[lane] = make_float4(tw_next.x, tw_next.y, -tw_next.y, tw_next.x);
   __syncwarp();
   if (ja + 1 < ja1) tw_next = __ldg(&a.tw_n1[((ja + 1) * (row_lo + lane)) & n1m]);
   float2 v[32];
@@ -816,9 +770,9 @@ static cudaError_t dispatch_p1(Ctx* c, const P1Args& args, cudaStream_t st) {
 }
 
 static cudaError_t launch_rowstage(Ctx* c, float2* y, const TemplateMeta* meta, int batch, int n_bands_all, int use_mask,
-                                   cudaStream_t st, int slot_base = 0) {
+                                   cudaStream_t st) {
   k_rowstage<<<4 * c->n_sms, 256, 0, st>>>(y, ws_ptr<float2>(c, c->lay.tw_p2), meta, batch, c->prm.p,
-                                                  c->log_n - kLogN2, n_bands_all, use_mask, slot_base);
+                                                  c->log_n - kLogN2, n_bands_all, use_mask);
   c->launches++;
   return cudaGetLastError();
 }
@@ -903,7 +857,6 @@ cudaError_t launch_pass1_filter(Ctx* c, int first, int count, int next_first, in
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = count;
-  args.eff = 0;
   args.slot_base = 0;
   args.first_template = 0;
   args.ja_per_cta = 1;
@@ -977,7 +930,6 @@ cudaError_t launch_pass1_dense(Ctx* c, const float2* d_in, float2* d_mid, cudaSt
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = 1;
-  args.eff = 0;
   args.slot_base = 0;
   args.first_template = 0;
   args.ja_per_cta = 1;
@@ -1002,7 +954,6 @@ static void fill_eff_args(Ctx* c, P1Args& args, int first, int count, int parity
   args.log_n = c->log_n;
   args.n1 = c->n1;
   args.batch = count;
-  args.eff = 1;
   args.slot_base = c->h_eff[first];
   args.first_template = first;
   args.ja_per_cta = 1;

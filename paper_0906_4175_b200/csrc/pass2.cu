@@ -22,12 +22,6 @@
 
 #include "fft_reg.cuh"
 #include "gwmf_internal.cuh"
-#ifndef GWMF_P2_TW4
-#define GWMF_P2_TW4 1
-#endif
-#ifndef GWMF_P2_EPI
-#define GWMF_P2_EPI 1
-#endif
 
 namespace gwmf {
 
@@ -279,13 +273,10 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, con
   __shared__ int s_slot0[kMaxBatch + 2];      // first slot of template tb (batch-relative)
   __shared__ int s_neff[kMaxBatch + 2];       // rows to read | has_s << 8 | guest of a pair << 9
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float4* tw_s = reinterpret_cast<float4*>(smem2);                    // [c][jm]: {w, i w}, w = e^{2 pi i c jm/1024}
-  float2* bufs = smem2 + 2048 + warp * (kP2ERing * kN2);
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 2048 + kP2EWarps * kP2ERing * kN2) + kP2ERing * warp;
-  for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
-    const float2 w = a.tw_p2[i];
-    tw_s[i] = make_float4(w.x, w.y, -w.y, w.x);
-  }
+  float2* tw_s = smem2;                                               // [c][jm]
+  float2* bufs = smem2 + 1024 + warp * (kP2ERing * kN2);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem2 + 1024 + kP2EWarps * kP2ERing * kN2) + kP2ERing * warp;
+  for (int i = threadIdx.x; i < 1024; i += blockDim.x) tw_s[i] = a.tw_p2[i];
   for (int t = threadIdx.x; t < ea.batch; t += blockDim.x) {
     s_slot0[t] = a.meta[t].eff_prefix - ea.slot_base;
     const bool guest = a.meta[t].pair == 2;     // reads one row more than it owns: the pair band of template t - 1
@@ -357,13 +348,7 @@ __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, con
       // pass 1 stores the 16-byte chunk ch of a 256 B piece at chunk ch ^ (jb & 15)
       const int sl = lane ^ (((j1 >> ea.log_na) & 15) << 1);
       for (int c = 0; c < 32; ++c) {                                        // lane = jm
-        const float2 v = cur[32 * c + sl];
-#if GWMF_P2_TW4
-        const float4 w = tw_s[32 * c + lane];                              // v w = v.x w + v.y (i w): no negation of v
-        x[brev<32>(c)] = unpk(fma2(pk(v.y, v.y), pk(w.z, w.w), mul2(pk(v.x, v.x), pk(w.x, w.y))));
-#else
-        x[brev<32>(c)] = cmul(v, reinterpret_cast<const float2*>(tw_s)[2 * (32 * c + lane)]);
-#endif
+        x[brev<32>(c)] = cmul(cur[32 * c + sl], tw_s[32 * c + lane]);
       }
       fft_dit<32>(x);                                                       // over c -> jc; j2 = lane + 32 jc
       __syncwarp();                                                         // every lane holds its 32 values
@@ -686,7 +671,7 @@ cudaError_t launch_fused_filter(Ctx* c, int first, int count, int parity, bool u
 }
 
 constexpr size_t kP2Smem = (size_t)(1024 + kP2Warps * kP2Ring * kN2) * sizeof(float2) + kP2Warps * kP2Ring * sizeof(unsigned long long);
-constexpr size_t kP2ESmem = (size_t)(2048 + kP2EWarps * kP2ERing * kN2) * sizeof(float2) + kP2EWarps * kP2ERing * sizeof(unsigned long long);
+constexpr size_t kP2ESmem = (size_t)(1024 + kP2EWarps * kP2ERing * kN2) * sizeof(float2) + kP2EWarps * kP2ERing * sizeof(unsigned long long);
 
 // Opt-in to > 48 KB of dynamic shared memory on the CURRENT device (gwmf_create calls this for every context).
 cudaError_t configure_pass2() {
