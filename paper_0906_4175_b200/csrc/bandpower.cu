@@ -26,8 +26,10 @@ namespace gwmf {
 
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }        // one float2 of padding per 16: the
                                                                             // stride-1 groups of the last stage become conflict-free
-constexpr int kBpThreads = 256;
-constexpr int kBpSubThreads = 512;   // sub-grid CTAs (one per SM, 140 KB of shared memory): twice the threads
+// threads per CTA = work items of a radix-32 stage (L / 32), so that every thread has one: 128 for L <= 4096 (4 CTAs per
+// SM), 256 for L = 8192 (2 per SM), 512 for L = 16384 (1 per SM: 140 KB of shared memory)
+constexpr int bp_threads(int log_l) { return log_l <= 12 ? 128 : log_l == 13 ? 256 : 512; }
+constexpr int bp_ctas(int log_l) { return log_l <= 12 ? 4 : log_l == 13 ? 2 : 1; }
 constexpr int kTwLo = 128;            // e^{2 pi i t/L} = TWH[t >> 7] * TWL[t & 127]: two small shared tables instead of one
                                       // scattered 8-byte global load per twiddle (every lane in its own sector)
 constexpr size_t bp_smem(int log_l) {
@@ -82,11 +84,11 @@ __global__ void __launch_bounds__(1024) k_bp_jobs(const TemplateMeta* __restrict
 //     U_l[m] += (1/LT) e^{-2 pi i r m/LT} W_r[m mod L],   W_r = L-point forward transform of |y[r + D j'']|^2,
 // goes to row r of the band's rows of wbuf; k_uspec adds the rows in a fixed order.
 template <int LOG_L, bool SUB>
-__global__ void __launch_bounds__(SUB ? kBpSubThreads : kBpThreads, LOG_L == 14 ? 1 : 2)
+__global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     k_bandpower(const TemplateMeta* __restrict__ meta, const float2* __restrict__ q, const float2* __restrict__ tw_l,
                 float2* __restrict__ wbuf, int p, int half_n, const int* __restrict__ jobs, const int* __restrict__ n_jobs) {
   constexpr int L = 1 << LOG_L;
-  constexpr int NT = SUB ? kBpSubThreads : kBpThreads;
+  constexpr int NT = bp_threads(LOG_L);
   constexpr int R3 = L / 1024;                    // last radix: 2, 4, 8, 16
   constexpr int S1 = L / 32;                      // stride of the first radix-32 stage
   constexpr int TWS = kLMax / L;                  // tw_l[t * TWS] = e^{2 pi i t / L}
@@ -389,8 +391,8 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
   cudaError_t e;
   const bool fork = c->s_bins > 1024;
   if (fork && (e = cudaEventRecord(c->ev_bp_fork, st)) != cudaSuccess) return e;
-  const int g2 = 2 * c->n_sms, g1 = c->n_sms;     // resident CTAs of a kernel (2 per SM; 1 per SM for the 2^14-point grids)
-  k_bandpower<11, false><<<g2, kBpThreads, bp_smem(11), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+  auto grid_of = [&](int log_l) { return bp_ctas(log_l) * c->n_sms; };    // the CTAs of a kernel that can be resident
+  k_bandpower<11, false><<<grid_of(11), bp_threads(11), bp_smem(11), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
   c->launches++;
   int used = 0;
   auto side = [&](int i) -> cudaStream_t {
@@ -398,11 +400,11 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
     used |= 1 << i;
     return c->bp[i];
   };
-  if (c->s_bins > 1024) { k_bandpower<12, false><<<g2, kBpThreads, bp_smem(12), side(0)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
-  if (c->s_bins > 2048) { k_bandpower<13, false><<<g2, kBpThreads, bp_smem(13), side(1)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
-  if (c->s_bins > 4096) { k_bandpower<14, false><<<g1, kBpThreads, bp_smem(14), side(2)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  if (c->s_bins > 1024) { k_bandpower<12, false><<<grid_of(12), bp_threads(12), bp_smem(12), side(0)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  if (c->s_bins > 2048) { k_bandpower<13, false><<<grid_of(13), bp_threads(13), bp_smem(13), side(1)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  if (c->s_bins > 4096) { k_bandpower<14, false><<<grid_of(14), bp_threads(14), bp_smem(14), side(2)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
   if (c->s_bins > kLMax / 2) {                    // bands on grids of 2^15 or 2^16 points: up to kSubMax sub-grid jobs each
-    k_bandpower<14, true><<<g1, kBpSubThreads, bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+    k_bandpower<14, true><<<grid_of(14), bp_threads(14), bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
     c->launches++;
   }
   for (int i = 0; i < 3; ++i) {

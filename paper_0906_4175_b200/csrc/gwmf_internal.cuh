@@ -217,7 +217,7 @@ __device__ inline int build_wide_list(const TemplateMeta* meta, int batch, int p
   return s_cnt[batch];
 }
 #endif
-constexpr int kMaxBatch = 64;    // templates per launch (bounds the shared-memory band list)
+constexpr int kMaxBatch = 128;   // templates per launch (bounds the shared-memory band list)
 
 template <typename T>
 inline T* ws_ptr(Ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }

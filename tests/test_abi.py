@@ -46,11 +46,11 @@ def test_workspace_bytes_host_only(lib):
     assert gwmf.workspace_bytes(1 << 23, 4, 4096, 1) == 0
     assert gwmf.workspace_bytes(1 << 14, 33, 4096, 1) == 0
     b = gwmf.workspace_bytes(1 << 20, 16, 4096, 1024)
-    # band intermediate: 256 n-point transforms * n * 8 B = 2 GiB; per-band power spectra of the decimated path
-    # (2 * 64 templates * p * 4 sub-grid rows * 32768 * 8 B = 2 GiB); double-buffered correlated spectra
-    # (2 * 64 * 4 MiB = 512 MiB); tables / slots / staging
-    assert (4 << 30) + (512 << 20) < b < (5 << 30)
-    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (440 << 20)
+    # band intermediate: 256 n-point transforms * n * 8 B = 2 GiB, and as much again for the pre-passed bands (vbuf);
+    # per-band power spectra of the decimated path (2 * 128 templates * p * 4 sub-grid rows * 32768 * 8 B = 4 GiB);
+    # double-buffered correlated spectra (2 * 128 * 4 MiB = 1 GiB); tables / slots / staging
+    assert (9 << 30) < b < (9 << 30) + (512 << 20)
+    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (700 << 20)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
 
