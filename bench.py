@@ -265,10 +265,11 @@ def spawn_ranks(args) -> int:
 STAGES = ("spectra", "pass1", "pass2", "chisq_at_events")
 STAGE_TEXT = {
     "decimated": {
-        "spectra": "k_correlate + k_bandpower + k_uspec (template phasors x data, coarse-grid band powers, U+); timed "
-                   "serialised, run beside pass 1 on a side stream in gwmf_filter",
+        "spectra": "k_correlate_cm + k_bp_jobs + k_bandpower (5 kernels side by side) + k_uspec (template phasors x data, "
+                   "coarse-grid band powers, U+); timed serialised, run beside the previous batch's passes on a side stream "
+                   "in gwmf_filter",
         "pass1": "k_pass1_eff (first FFT pass of every effective band: writes n complex fp32 per n-point transform) "
-                 "[+ generic kernel + row stage for bands of > 512 input rows]",
+                 "[+ k_prepass for bands of very many input rows: one more n complex written and read]",
         "pass2": "k_pass2_eff (last FFT stage + rho/chi^2/trigger epilogue: reads n complex fp32 per n-point transform)",
         "chisq_at_events": "k_chisq_at (chi^2 on demand: Eq. 5 evaluated from its definition at every event's sample)"},
     "two_pass": {

@@ -48,9 +48,9 @@ typedef enum {
 /* Which kernels compute the p band transforms of step a3 (all three compute the same rho, chi^2 and events):
  *   TWO_PASS   pass 1 writes every band's intermediate to HBM (p n complex per template), pass 2 reads it;
  *   FUSED      spill-free: narrow bands are formed inside the row-transform kernel (n <= 2^20);
- *   DECIMATED  narrow bands are transformed on a coarse grid of L >= 2 B points, their power spectra summed, and one
- *              n-point transform returns sum_l |z_l|^2; only z, that sum and the wide bands keep n-point transforms
- *              (n >= 2^15).  DESIGN.md section 5.
+ *   DECIMATED  bands of at most min(32768, n/16) bins are transformed on a coarse grid of L >= 2 B points, their power
+ *              spectra summed, and one n-point transform (shared by two templates) returns sum_l |z_l|^2; only z,
+ *              that sum and the wider bands keep n-point transforms (n >= 2^15).  DESIGN.md section 5.
  *   AUTO       the library's choice: DECIMATED for n >= 2^15, TWO_PASS below. */
 typedef enum {
   GWMF_PATH_AUTO = 0,
@@ -89,10 +89,10 @@ typedef struct {
   double  rho_thresh;    /* SNR threshold, strict '>'                                             */
   int32_t window;        /* W: trigger window in samples, power of two, divides n                 */
   int32_t max_templates; /* capacity of the bank                                                  */
-  int32_t batch;         /* most templates filtered per kernel launch, 0 .. 64; sizes the band-intermediate
+  int32_t batch;         /* most templates filtered per kernel launch, 0 .. 128; sizes the band-intermediate
                             buffer, batch * p * n * 8 bytes, and the correlated spectra, 2 * batch * n * 4 bytes.
                             0 = library default: a band buffer of about 2 GiB; the decimated path then takes up
-                            to 64 templates per launch, as many as fit in it (it needs ~3, not p, transforms each).
+                            to 128 templates per launch, as many as fit in it (it needs ~2, not p, transforms each).
                             The decimated path processes templates in pairs: an odd value is rounded up            */
   int32_t path;          /* a gwmf_path; GWMF_PATH_AUTO (0) = the library's choice.  A path that does not support n
                             (FUSED: 2^15 .. 2^20, DECIMATED: >= 2^15) is GWMF_E_ARG                               */
@@ -171,8 +171,8 @@ int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges);
 
 /* Measurement: the number of n-point transforms the library runs for every loaded template with its path, HOST array
  * of n_templates int32: the non-empty bands (two-pass and spill-free paths), or the effective bands of the
- * decimated path (2 + the number of bands wider than min(8192, n/16) bins; just the wide bands if no band is
- * narrow).  Each one is n complex fp32 written by pass 1 and read by pass 2: the byte model of bench.py.  syncs. */
+ * decimated path (1 for z + 1 for sum |z_l|^2, which the guest of a template pair does not count, + the number of
+ * bands wider than min(32768, n/16) bins; just the bands themselves if fewer than three are narrow).  Each one is n complex fp32 written by pass 1 and read by pass 2: the byte model of bench.py.  syncs. */
 int gwmf_transform_counts(gwmf_ctx* ctx, int32_t* host_counts);
 
 /* Debug/parity: full rho(t) and chi^2(t) of one template, n floats each, HOST arrays (either may be

@@ -33,8 +33,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         objs.append(o)
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_time):
             log = open(o + ".log", "w")
-            extra = os.environ.get("GWMF_NVCC_EXTRA", "").split()      # development only: -D switches of a kernel variant
-            procs.append((s, log, subprocess.Popen(["nvcc", *NVCC_FLAGS, *extra, "-c", s, "-o", o], stdout=log, stderr=log)))
+            procs.append((s, log, subprocess.Popen(["nvcc", *NVCC_FLAGS, "-c", s, "-o", o], stdout=log, stderr=log)))
     failed = False
     for s, log, pr in procs:
         rc = pr.wait()

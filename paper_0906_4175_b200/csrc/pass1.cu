@@ -395,19 +395,11 @@ struct EffSrc {
 // makes the column writes of phase 1, the row reads / writes of phase 2 (16 bytes per lane) and the bulk copy's linear
 // read all conflict-free.  The tile reaches the band buffer as it is (pass 2 undoes the swizzle when it reads).
 constexpr int kWTile = 32 * 32;                   // float2 per warp (8 KB)
-#ifndef GWMF_P1_WARPS
-#define GWMF_P1_WARPS 4
-#endif
-#ifndef GWMF_P1_CTAS
-#define GWMF_P1_CTAS 4
-#endif
-#ifndef GWMF_P1_VARIANTS
-#define GWMF_P1_VARIANTS 2
-#endif
-#ifndef GWMF_P1_JA
-#define GWMF_P1_JA 4
-#endif
-constexpr int kP1Warps = GWMF_P1_WARPS;           // warps (values of c) per CTA of k_pass1_eff
+// Measured on B200 (headline config): 4 warps x 4 CTAs per SM at 128 registers (no spills) beats 8 x 3 at 80 registers
+// (spills in the round loop) by 20 %; 2..8 ja per CTA are within 2 % of each other, 1 and 32 are worse.
+constexpr int kP1Warps = 4;                       // warps (values of c) per CTA of k_pass1_eff
+constexpr int kP1CtasPerSm = 4;
+constexpr int kP1JaPerCta = 4;                    // consecutive ja a CTA walks over
 constexpr int kP1Groups = 32 / kP1Warps;          // CTAs (column groups cg) per ja
 constexpr size_t kP1WSmem = (size_t)(kP1Warps * kWTile + kP1Warps * 64) * sizeof(float2);     // tiles + per-warp TW tables {w, i w}
 __device__ __forceinline__ int wz(int r, int m) { return r * 32 + (m ^ ((r & 15) << 1)); }   // cell (row r, element m)
@@ -546,20 +538,12 @@ template <bool HOLES>
 __device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float4* TW, float2* tile, int ja, int c, int lane,
                                          float2 (&v)[32]) {
   const int R = ((es.e_hi - 1) >> kLogN2) - (es.e_lo >> kLogN2) + 1;
-#if GWMF_P1_VARIANTS == 4
-  if (R <= 4) eff_phase1<4, HOLES>(a, es, TW, tile, ja, c, lane, v);
-  else if (R <= 8) eff_phase1<8, HOLES>(a, es, TW, tile, ja, c, lane, v);
-  else if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, tile, ja, c, lane, v);
-  else eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
-#elif GWMF_P1_VARIANTS == 2
+  // two pruned variants: more of them cost more in instruction-cache misses than their shorter transforms save
   if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, tile, ja, c, lane, v);
   else eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
-#else
-  eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
-#endif
 }
 
-__global__ void __launch_bounds__(kP1Warps * 32, GWMF_P1_CTAS) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
+__global__ void __launch_bounds__(kP1Warps * 32, kP1CtasPerSm) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
   extern __shared__ __align__(1024) float2 smem[];
   __shared__ int s_holes[2 * kMaxBands];
 
@@ -967,7 +951,7 @@ cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStrea
   fill_eff_args(c, args, first, count, parity);
   const int n_slots = c->h_eff[first + count] - c->h_eff[first];
   if (n_slots <= 0) return cudaSuccess;
-  args.ja_per_cta = c->na >= GWMF_P1_JA ? GWMF_P1_JA : c->na;
+  args.ja_per_cta = c->na >= kP1JaPerCta ? kP1JaPerCta : c->na;
   k_pass1_eff<<<dim3(kP1Groups * (c->na / args.ja_per_cta), n_slots), kP1Warps * 32, kP1WSmem, st>>>(args, ws_ptr<SlotDesc>(c, c->lay.slot_tab));
   c->launches++;
   return cudaGetLastError();

@@ -257,14 +257,8 @@ struct P2EArgs {
 // SINGLE: every template of the launch has exactly one effective band (p = 1, or chi^2 on demand): z is that band's
 // transform, no sums over bands are kept, and the epilogue is one compare of |z|^2 against the threshold per sample
 // (chi^2 is 0 by definition for p = 1 and is filled in later by k_chisq_at in the on-demand mode).
-#ifndef GWMF_P2_WARPS
-#define GWMF_P2_WARPS 12
-#endif
-#ifndef GWMF_P2_RING
-#define GWMF_P2_RING 2
-#endif
-constexpr int kP2EWarps = GWMF_P2_WARPS;     // k_pass2_eff: 12 warps per SM with a ring of 2 rows each (192 KB): the kernel is bound by the
-constexpr int kP2ERing = GWMF_P2_RING;       // latency of its per-row chains, not by HBM, once a template needs ~2 transforms
+constexpr int kP2EWarps = 12;    // k_pass2_eff: 12 warps per SM with a ring of 2 rows each (192 KB): the kernel is bound by the
+constexpr int kP2ERing = 2;     // latency of its per-row chains, not by HBM, once a template needs ~2 transforms
 
 template <bool SERIES, bool SINGLE>
 __global__ void __launch_bounds__(kP2EWarps * 32, 1) k_pass2_eff(P2EArgs ea, const __grid_constant__ CUtensorMap tmap) {
