@@ -45,6 +45,34 @@ struct BpTw {
   }
 };
 
+// The 32 twiddles e^{2 pi i step k/L}, k = 0..31, of one work item of a radix-32 stage: a geometric sequence.  Two table
+// look-ups (w = e^{2 pi i step/L} and w^8, both exact to one rounding) and short products: w^(8a + b) = (w^8)^a w^b, at
+// most 3 + 7 multiplications deep, instead of 31 look-ups (the shared-memory pipe is these kernels' busiest unit).
+template <int LOG_L>
+struct BpSeq {
+  float2 lo[8];      // w^b
+  float2 hi[4];      // w^(8a)
+  __device__ __forceinline__ BpSeq(const BpTw<LOG_L>& tw, int step) {
+    constexpr int L = 1 << LOG_L;
+    const float2 w1 = tw(step & (L - 1)), w8 = tw((8 * step) & (L - 1));
+    lo[0] = make_float2(1.f, 0.f);
+    lo[1] = w1;
+#pragma unroll
+    for (int b = 2; b < 8; ++b) lo[b] = cmul(lo[b - 1], w1);
+    hi[0] = make_float2(1.f, 0.f);
+    hi[1] = w8;
+    hi[2] = cmul(w8, w8);
+    hi[3] = cmul(hi[2], w8);
+  }
+  __device__ __forceinline__ float2 mul(float2 v, int k) const {      // v e^{2 pi i step k/L}, k a compile-time constant after unrolling
+    const int a = k >> 3, b = k & 7;
+    if (k == 0) return v;
+    if (a == 0) return cmul(v, lo[b]);
+    if (b == 0) return cmul(v, hi[a]);
+    return cmul(cmul(v, lo[b]), hi[a]);
+  }
+};
+
 // Job lists of a batch, one per kernel: class 0..3 = bands on a grid of 2^11..2^14 points, class 4 = the sub-grid jobs
 // (band, r) of the bands on 2^15 / 2^16 points.  jobs[class][i] = tb << 16 | l << 8 | r.  The order inside a list is
 // whatever the atomics give: every job writes rows of its own, so the results do not depend on it.
@@ -186,7 +214,9 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
       fft_dit<32>(x);
     }
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = k == 0 ? x[0] : cmul(x[k], tw((o * k) & (L - 1)));
+    const BpSeq<LOG_L> sq(tw, o);
+#pragma unroll
+    for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = sq.mul(x[k], k);
   }
   __syncthreads();
   // ---- stage 2: inside each block k1 of S1 = 32 R3 points
@@ -198,7 +228,9 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pad16(base + R3 * qq)];
     fft_dit<32>(x);
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = k == 0 ? x[0] : cmul(x[k], tw((32 * o2 * k) & (L - 1)));
+    const BpSeq<LOG_L> sq(tw, 32 * o2);
+#pragma unroll
+    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = sq.mul(x[k], k);
   }
   __syncthreads();
   // ---- stage 3 (R3 points, stride 1), |y|^2, and the first stage of the way back (same groups, no twiddle)
@@ -221,11 +253,12 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
 #pragma unroll 1
   for (int g = tid; g < S1; g += NT) {
     const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
+    const BpSeq<LOG_L> sq(tw, 32 * o2);
     float2 x[32];
 #pragma unroll
     for (int qq = 0; qq < 32; ++qq) {
       const float2 v = sm[pad16(base + R3 * qq)];
-      x[brev<32>(qq)] = qq == 0 ? v : cmul(v, tw((32 * o2 * qq) & (L - 1)));
+      x[brev<32>(qq)] = sq.mul(v, qq);
     }
     fft_dit<32>(x);
 #pragma unroll
@@ -236,11 +269,12 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
   const float inv_l = 1.0f / (float)(1u << log_lt);
 #pragma unroll 1
   for (int o = tid; o < S1; o += NT) {
+    const BpSeq<LOG_L> sq(tw, o);
     float2 x[32];
 #pragma unroll
     for (int qq = 0; qq < 32; ++qq) {
       const float2 v = sm[pad16(o + S1 * qq)];
-      x[brev<32>(qq)] = qq == 0 ? v : cmul(v, tw((o * qq) & (L - 1)));
+      x[brev<32>(qq)] = sq.mul(v, qq);
     }
     fft_dit<32>(x);
     if constexpr (!SUB) {

@@ -391,7 +391,7 @@ struct EffSrc {
   const float2* v;        // pre-passed band (k_prepass): V of this slot, else nullptr
 };
 
-// A warp's tile: 32 rows (jb) of 256 B, no padding; the 16-byte chunk ch of row r sits at chunk ch ^ (r & 15) (wz), which
+// A warp's tile: 32 rows (jb) of 256 B, no padding; the 16-byte chunk ch of row r sits at chunk ch ^ (r & 15), which
 // makes the column writes of phase 1, the row reads / writes of phase 2 (16 bytes per lane) and the bulk copy's linear
 // read all conflict-free.  The tile reaches the band buffer as it is (pass 2 undoes the swizzle when it reads).
 constexpr int kWTile = 32 * 32;                   // float2 per warp (8 KB)
@@ -402,7 +402,6 @@ constexpr int kP1CtasPerSm = 4;
 constexpr int kP1JaPerCta = 4;                    // consecutive ja a CTA walks over
 constexpr int kP1Groups = 32 / kP1Warps;          // CTAs (column groups cg) per ja
 constexpr size_t kP1WSmem = (size_t)(kP1Warps * kWTile + kP1Warps * 64) * sizeof(float2);     // tiles + per-warp TW tables {w, i w}
-__device__ __forceinline__ int wz(int r, int m) { return r * 32 + (m ^ ((r & 15) << 1)); }   // cell (row r, element m)
 
 // 16-byte shared-memory access at (addr ^ x): the XOR is part of the asm so that the 16 addresses of a row are formed
 // where they are used instead of being kept in registers
@@ -418,27 +417,13 @@ __device__ __forceinline__ void sts128_x(unsigned addr, unsigned x, float4 v) {
                "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w)
                : "memory");
 }
-// 8-byte accesses to cell (row i, element m = lane) of a warp's swizzled tile: byte address ((col ^ x) + off) with
+// 8-byte store to cell (row i, element m = lane) of a warp's swizzled tile: byte address ((col ^ x) + off) with
 // col = tile | lane * 8, x = (i & 15) << 4, off = i * 256 (the XOR and the offset are part of the asm: nothing is hoisted)
 __device__ __forceinline__ void sts64_xo(unsigned col, unsigned x, unsigned off, float2 v) {
   asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %0, %1;\n\tadd.u32 a, a, %2;\n\tst.shared.v2.f32 [a], {%3, %4};\n\t}" ::"r"(col), "r"(x),
                "r"(off), "f"(v.x), "f"(v.y)
                : "memory");
 }
-__device__ __forceinline__ float2 lds64_xo(unsigned col, unsigned x, unsigned off) {
-  float2 v;
-  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %2, %3;\n\tadd.u32 a, a, %4;\n\tld.shared.v2.f32 {%0, %1}, [a];\n\t}"
-               : "=f"(v.x), "=f"(v.y)
-               : "r"(col), "r"(x), "r"(off));
-  return v;
-}
-__device__ __forceinline__ void ldgsts_xo(unsigned col, unsigned x, unsigned off, const float2* p, bool ok) {
-  asm volatile("{\n\t.reg .u32 a;\n\txor.b32 a, %0, %1;\n\tadd.u32 a, a, %2;\n\tcp.async.ca.shared.global [a], [%3], 8, %4;\n\t}" ::"r"(col),
-               "r"(x), "r"(off), "l"(p), "r"(ok ? 8 : 0)
-               : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 template <bool HOLES>
 __device__ __forceinline__ bool eff_ok(const EffSrc& es, int k1, int k2, int fr, int lr) {
@@ -458,16 +443,11 @@ __device__ __forceinline__ float2 ldg_pred(const float2* p, bool ok) {
       : "l"(p), "r"((int)ok));
   return v;
 }
-// the same element through an 8-byte cp.async into shared memory (zero-filled where !ok): no register is tied up
-__device__ __forceinline__ void ldgsts_pred(float2* slot, const float2* p, bool ok) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((unsigned)__cvta_generic_to_shared(slot)), "l"(p),
-               "r"(ok ? 8 : 0)
-               : "memory");
-}
+
 
 // Phase 1 of a warp (lane = m, column k2 = 32 lane + c): leaves v[jb], jb = 0..31 in natural order.
-// tile: the warp's tile; the lane's column of it (cells wz(i, lane)) is used as the landing zone of the
-// cp.async rounds, a lane only touches its own column.  TW: the warp's table (shared).
+// The tile is only waited for here (the previous ja's bulk store must have read it before it is written again).
+// TW: the warp's table (shared).
 template <int RMAX, bool HOLES>
 __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float4* __restrict__ TW,
                                            float2* __restrict__ tile, int ja, int c, int lane, float2 (&v)[32]) {
@@ -478,14 +458,12 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
   const int fr = es.v ? INT_MIN : row_lo + (k2 < (es.e_lo & (kN2 - 1)) ? 1 : 0);       // first / last row whose bin in THIS column is in the band
   const int lr = es.v ? INT_MAX : row_hi - (k2 > ((es.e_hi - 1) & (kN2 - 1)) ? 1 : 0);
   const float2* __restrict__ base = es.src + c * 32 + lane;            // + k1 * 1024 (k1 < 0 in the lower half of a pair spectrum)
-  const float2* safe = es.src + (size_t)(row_lo < 0 ? 0 : row_lo) * kN2;
-  const unsigned col = (unsigned)__cvta_generic_to_shared(tile) | ((unsigned)lane << 3);     // the tile is 256 B aligned
 
   // rows of round t: the band's rows row_lo + 32 t + i, or (pre-passed band, es.v != nullptr) the 32 rows b' = i of V[t][ja mod 32]
   auto round_ptr = [&](int t) -> const float2* {
     return es.v ? es.v + ((size_t)(t * 32 + (ja & 31)) * 32) * kN2 + c * 32 + lane : base + (ptrdiff_t)(row_lo + 32 * t) * kN2;
   };
-  // top round (t = T - 1) straight into the registers of the transform; the one below it through cp.async at the same time
+  // top round (t = T - 1) straight into the registers of the transform
   {
     const int r0 = row_lo + 32 * (T - 1);
     const float2* __restrict__ p0 = round_ptr(T - 1);
@@ -500,28 +478,34 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
   __syncwarp();
   if constexpr (RMAX == 32) {
     if (T > 1) {
-      auto request = [&](int t) {
-        const int r0 = row_lo + 32 * t;
-        const float2* __restrict__ p0 = round_ptr(t);
+      // The rounds below the top one, highest first: v = v g + X_t (Horner), the rows of a round loaded in groups of 8
+      // straight into registers, one group in flight while the previous one is consumed (no shared-memory staging:
+      // the L1 data pipe is this kernel's busiest unit).
+      auto load_group = [&](int t, int gq, float2 (&dst)[8]) {
+        const int r0 = row_lo + 32 * t + 8 * gq;
+        const float2* __restrict__ p0 = round_ptr(t) + (size_t)(8 * gq) * kN2;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
-          ldgsts_xo(col, (i & 15) << 4, i * 256, ok ? p0 + i * kN2 : safe, ok);
-        }
-        cp_async_commit();
+        for (int j = 0; j < 8; ++j) dst[j] = ldg_pred(p0 + j * kN2, eff_ok<HOLES>(es, r0 + j, k2, fr, lr));
       };
-      request(T - 2);
       const float2 g1 = a.tw_n1[(ja * 32) & (a.n1 - 1)];                          // e^{2 pi i ja/NA}
       const pk2 g = pk(g1), ig = pk(-g1.y, g1.x);
+      float2 nx[8];
+      load_group(T - 2, 0, nx);
 #pragma unroll 1
       for (int t = T - 2; t >= 0; --t) {
-        cp_async_wait_all();
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          const float2 val = lds64_xo(col, (i & 15) << 4, i * 256), w = v[brev<32>(i)];
-          v[brev<32>(i)] = unpk(fma2(pk(w.y, w.y), ig, fma2(pk(w.x, w.x), g, pk(val))));   // v g + val = w.x g + w.y (i g) + val
+        for (int gq = 0; gq < 4; ++gq) {
+          float2 cur[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) cur[j] = nx[j];
+          if (gq < 3) load_group(t, gq + 1, nx);
+          else if (t > 0) load_group(t - 1, 0, nx);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const float2 w = v[brev<32>(8 * gq + j)];
+            v[brev<32>(8 * gq + j)] = unpk(fma2(pk(w.y, w.y), ig, fma2(pk(w.x, w.x), g, pk(cur[j]))));   // v g + X = w.x g + w.y (i g) + X
+          }
         }
-        if (t > 0) request(t - 1);
       }
     }
   }
