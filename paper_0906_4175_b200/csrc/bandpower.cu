@@ -24,8 +24,6 @@
 
 namespace gwmf {
 
-__device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }        // one float2 of padding per 16: the
-                                                                            // stride-1 groups of the last stage become conflict-free
 // threads per CTA = work items of a radix-32 stage (L / 32), so that every thread has one: 128 for L <= 4096 (4 CTAs per
 // SM), 256 for L = 8192 (2 per SM), 512 for L = 16384 (1 per SM: 140 KB of shared memory)
 constexpr int bp_threads(int log_l) { return log_l <= 12 ? 128 : log_l == 13 ? 256 : 512; }
@@ -33,7 +31,7 @@ constexpr int bp_ctas(int log_l) { return log_l <= 12 ? 4 : log_l == 13 ? 2 : 1;
 constexpr int kTwLo = 128;            // e^{2 pi i t/L} = TWH[t >> 7] * TWL[t & 127]: two small shared tables instead of one
                                       // scattered 8-byte global load per twiddle (every lane in its own sector)
 constexpr size_t bp_smem(int log_l) {
-  return (size_t)((1 << log_l) + ((1 << log_l) >> 4) + kTwLo + ((1 << log_l) / kTwLo)) * sizeof(float2);
+  return (size_t)((1 << log_l) + ((1 << log_l) >> 4) + ((1 << log_l) >> 5) + kTwLo + ((1 << log_l) / kTwLo)) * sizeof(float2);
 }
 
 template <int LOG_L>
@@ -122,11 +120,15 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
   constexpr int TWS = kLMax / L;                  // tw_l[t * TWS] = e^{2 pi i t / L}
   constexpr int CLS = SUB ? 4 : LOG_L - kLogLMin; // job class (k_bp_jobs)
   extern __shared__ __align__(16) float2 sm[];
+  // element i of the L-point array: one float2 of padding per 16 (the stride-1 groups of the last radix become
+  // conflict-free) and R3 more per block of S1 = L / 32 (so do the stride-R3 accesses of the middle radix-32 stage, whose
+  // lanes sit in different blocks)
+  auto pd = [](int i) { return i + (i >> 4) + (i >> (LOG_L - 5)) * R3; };
   __shared__ float2 s_fine[4];
   const int n_job = n_jobs[CLS];
   if ((int)blockIdx.x >= n_job) return;
   const int tid = threadIdx.x;
-  float2* twl = sm + L + (L >> 4);
+  float2* twl = sm + L + (L >> 4) + (L >> 5);
   float2* twh = twl + kTwLo;
   for (int i = tid; i < kTwLo; i += NT) twl[i] = tw_l[i * TWS];
   for (int i = tid; i < L / kTwLo; i += NT) twh[i] = tw_l[i * kTwLo * TWS];
@@ -167,15 +169,15 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     const int row_lo = e_lo >> kLogN2, n_rows = ((e_lo + B - 1) >> kLogN2) - row_lo + 1;
     const float2* __restrict__ qrows = q + (size_t)tb * half_n + (size_t)row_lo * kN2;
     if constexpr (!SUB) {
-      for (int i = B + tid; i < L; i += NT) sm[pad16(i)] = make_float2(0.f, 0.f);
+      for (int i = B + tid; i < L; i += NT) sm[pd(i)] = make_float2(0.f, 0.f);
       for (int idx = tid; idx < n_rows * kN2; idx += NT) {
         const int i = ((row_lo + (idx >> kLogN2)) << kLogN2) + cm_pos(idx & (kN2 - 1)) - e_lo;
-        if (i >= 0 && i < B) sm[pad16(i)] = qrows[idx];
+        if (i >= 0 && i < B) sm[pd(i)] = qrows[idx];
       }
     } else {
       // X_r[i mod L] += Q[e_l + i] e^{2 pi i r i/LT}: a cell receives at most two terms (B <= LT / 2 = 2 L), so the
       // shared-memory adds commute and the result does not depend on their order
-      for (int i = tid; i < L; i += NT) sm[pad16(i)] = make_float2(0.f, 0.f);
+      for (int i = tid; i < L; i += NT) sm[pd(i)] = make_float2(0.f, 0.f);
       __syncthreads();
       for (int idx0 = tid; idx0 < n_rows * kN2; idx0 += 4 * NT) {
         float2 v[4];
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
         for (int u = 0; u < 4; ++u) {
           if (ii[u] < 0) continue;
           const float2 t = r ? cmul(v[u], sub_tw((unsigned)r * (unsigned)ii[u])) : v[u];
-          float* dst = reinterpret_cast<float*>(&sm[pad16(ii[u] & (L - 1))]);
+          float* dst = reinterpret_cast<float*>(&sm[pd(ii[u] & (L - 1))]);
           atomicAdd(dst, t.x);
           atomicAdd(dst + 1, t.y);
         }
@@ -206,17 +208,17 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
 #pragma unroll
     if constexpr (!SUB) {
 #pragma unroll
-      for (int qq = 0; qq < 16; ++qq) x[brev<32>(qq)] = sm[pad16(o + S1 * qq)];
+      for (int qq = 0; qq < 16; ++qq) x[brev<32>(qq)] = sm[pd(o + S1 * qq)];
       fft_dit<32, 16>(x);
     } else {                                      // a folded band fills the whole sub-grid spectrum
 #pragma unroll
-      for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pad16(o + S1 * qq)];
+      for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pd(o + S1 * qq)];
       fft_dit<32>(x);
     }
 #pragma unroll
     const BpSeq<LOG_L> sq(tw, o);
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(o + S1 * k)] = sq.mul(x[k], k);
+    for (int k = 0; k < 32; ++k) sm[pd(o + S1 * k)] = sq.mul(x[k], k);
   }
   __syncthreads();
   // ---- stage 2: inside each block k1 of S1 = 32 R3 points
@@ -225,12 +227,12 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     const int k1 = g / R3, o2 = g - k1 * R3, base = k1 * S1 + o2;
     float2 x[32];
 #pragma unroll
-    for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pad16(base + R3 * qq)];
+    for (int qq = 0; qq < 32; ++qq) x[brev<32>(qq)] = sm[pd(base + R3 * qq)];
     fft_dit<32>(x);
 #pragma unroll
     const BpSeq<LOG_L> sq(tw, 32 * o2);
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = sq.mul(x[k], k);
+    for (int k = 0; k < 32; ++k) sm[pd(base + R3 * k)] = sq.mul(x[k], k);
   }
   __syncthreads();
   // ---- stage 3 (R3 points, stride 1), |y|^2, and the first stage of the way back (same groups, no twiddle)
@@ -239,14 +241,14 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     const int base = g * R3;
     float2 x[R3];
 #pragma unroll
-    for (int qq = 0; qq < R3; ++qq) x[brev<R3>(qq)] = sm[pad16(base + qq)];
+    for (int qq = 0; qq < R3; ++qq) x[brev<R3>(qq)] = sm[pd(base + qq)];
     fft_dit<R3>(x);
     float2 w[R3];
 #pragma unroll
     for (int qq = 0; qq < R3; ++qq) w[brev<R3>(qq)] = make_float2(fmaf(x[qq].x, x[qq].x, x[qq].y * x[qq].y), 0.f);
     fft_dit<R3>(w);
 #pragma unroll
-    for (int k = 0; k < R3; ++k) sm[pad16(base + k)] = w[k];
+    for (int k = 0; k < R3; ++k) sm[pd(base + k)] = w[k];
   }
   __syncthreads();
   // ---- decimation in time: twiddle first, then the radix-32 transform (transposes of stages 2 and 1)
@@ -257,12 +259,12 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     float2 x[32];
 #pragma unroll
     for (int qq = 0; qq < 32; ++qq) {
-      const float2 v = sm[pad16(base + R3 * qq)];
+      const float2 v = sm[pd(base + R3 * qq)];
       x[brev<32>(qq)] = sq.mul(v, qq);
     }
     fft_dit<32>(x);
 #pragma unroll
-    for (int k = 0; k < 32; ++k) sm[pad16(base + R3 * k)] = x[k];
+    for (int k = 0; k < 32; ++k) sm[pd(base + R3 * k)] = x[k];
   }
   __syncthreads();
   // last stage: only the outputs m = o + S1 k < B <= L/2 are wanted, i.e. k < 16; they leave straight to global memory
@@ -273,7 +275,7 @@ __global__ void __launch_bounds__(bp_threads(LOG_L), bp_ctas(LOG_L))
     float2 x[32];
 #pragma unroll
     for (int qq = 0; qq < 32; ++qq) {
-      const float2 v = sm[pad16(o + S1 * qq)];
+      const float2 v = sm[pd(o + S1 * qq)];
       x[brev<32>(qq)] = sq.mul(v, qq);
     }
     fft_dit<32>(x);
