@@ -375,6 +375,34 @@ def test_snr_only_mode_is_p1(gw):
     assert all(abs(k16[c] - k1[c]) <= 1e-3 + 1e-4 * k16[c] for c in common)
 
 
+def test_sub_grid_bands_and_prepass_are_exercised(gw):
+    # Decimated path, the two branches that only wide bands reach: a class-S band of 8193..32768 bins is
+    # transformed as 2 or 4 interleaved sub-grids of 2^14 points (k_bandpower<14, true>), and an effective band of more
+    # than 32 * 6 input rows at n = 2^20 is pre-passed (k_prepass, one 32-point transform over the Horner rounds).
+    # The bank is chosen so that both occur (checked from the band edges), then every sample is compared.
+    n, p = 1 << 20, 7
+    masses = [(1.4, 1.4), (3.0, 2.5), (8.0, 6.0)]
+    D = inputs.noise_spectrum(n, 77) + inputs.injection_spectrum(n, 3.0, 2.5, 10.0, 123457)
+    s = inputs.time_series(D, n).astype(np.float32)
+    Sn = inputs.psd_array(n)
+    w = inputs.Workload(config=-1, n=n, p=p, rho_thresh=5.5, window=4096, masses=masses, seed=0)
+    f = _run_gpu(gw, w, s, Sn, path="decimated")
+    edges = f.band_edges()
+    widths = np.diff(edges, axis=1)
+    assert np.any((widths > 8192) & (widths <= 16384)), "no band on a 2^15-point grid (2 sub-grids)"
+    assert np.any((widths > 16384) & (widths <= 32768)), "no band on a 2^16-point grid (4 sub-grids)"
+    rows = (edges[:, 1:] - 1) // 1024 - edges[:, :-1] // 1024 + 1
+    assert np.any((widths > 32768) & (rows > 192)), "no pre-passed band"
+    out = oracle.filter_bank(s.astype(np.float64), Sn, masses, p, 4096, 5.5)
+    parity.assert_sigma_edges(f.sigma(), edges, out["sigma"], out["edges"])
+    for t, (m1, m2) in enumerate(masses):
+        rho_o, chi_o, _, _ = oracle.filter_template(s.astype(np.float64), Sn, m1, m2, p)
+        rho_g, chi_g = f.series(t)
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, p, f"sub-grid / pre-pass case, template {t}")
+    compared, _ = parity.assert_triggers(f.triggers(), out, 5.5, 4096, p)
+    assert compared >= 1
+
+
 def test_config3_sweep_256_pairs_overlapped_loads(gw):
     # BASELINE.json:configs[3]: half-overlapping segments of one stream against the 4096-template bank, driven the way
     # bench.py --workload sweep drives it: the next segment is uploaded and prepared (gwmf_load_segment with Sn = NULL,
