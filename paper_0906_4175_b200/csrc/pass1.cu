@@ -479,7 +479,7 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
   if constexpr (RMAX == 32) {
     if (T > 1) {
       // The rounds below the top one, highest first: v = v g + X_t (Horner), the rows of a round loaded in groups of 8
-      // straight into registers, one group in flight while the previous one is consumed (no shared-memory staging:
+      // straight into registers, two groups in flight while the one before them is consumed (no shared-memory staging:
       // the L1 data pipe is this kernel's busiest unit).
       auto load_group = [&](int t, int gq, float2 (&dst)[8]) {
         const int r0 = row_lo + 32 * t + 8 * gq;
@@ -489,23 +489,26 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
       };
       const float2 g1 = a.tw_n1[(ja * 32) & (a.n1 - 1)];                          // e^{2 pi i ja/NA}
       const pk2 g = pk(g1), ig = pk(-g1.y, g1.x);
-      float2 nx[8];
-      load_group(T - 2, 0, nx);
+      float2 bufA[8], bufB[8];                      // two groups in flight: A holds the even groups of a round, B the odd ones
+      load_group(T - 2, 0, bufA);
+      load_group(T - 2, 1, bufB);
+      auto consume = [&](int gq, const float2 (&cur)[8]) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float2 w = v[brev<32>(8 * gq + j)];
+          v[brev<32>(8 * gq + j)] = unpk(fma2(pk(w.y, w.y), ig, fma2(pk(w.x, w.x), g, pk(cur[j]))));   // v g + X = w.x g + w.y (i g) + X
+        }
+      };
 #pragma unroll 1
       for (int t = T - 2; t >= 0; --t) {
-#pragma unroll
-        for (int gq = 0; gq < 4; ++gq) {
-          float2 cur[8];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) cur[j] = nx[j];
-          if (gq < 3) load_group(t, gq + 1, nx);
-          else if (t > 0) load_group(t - 1, 0, nx);
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            const float2 w = v[brev<32>(8 * gq + j)];
-            v[brev<32>(8 * gq + j)] = unpk(fma2(pk(w.y, w.y), ig, fma2(pk(w.x, w.x), g, pk(cur[j]))));   // v g + X = w.x g + w.y (i g) + X
-          }
-        }
+        consume(0, bufA);
+        load_group(t, 2, bufA);
+        consume(1, bufB);
+        load_group(t, 3, bufB);
+        consume(2, bufA);
+        if (t > 0) load_group(t - 1, 0, bufA);
+        consume(3, bufB);
+        if (t > 0) load_group(t - 1, 1, bufB);
       }
     }
   }
