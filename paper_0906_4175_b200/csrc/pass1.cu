@@ -445,12 +445,11 @@ __device__ __forceinline__ float2 ldg_pred(const float2* p, bool ok) {
 }
 
 
-// Phase 1 of a warp (lane = m, column k2 = 32 lane + c): leaves v[jb], jb = 0..31 in natural order.
-// The tile is only waited for here (the previous ja's bulk store must have read it before it is written again).
-// TW: the warp's table (shared).
+// Phase 1 of a warp (lane = m, column k2 = 32 lane + c): leaves v[jb], jb = 0..31 in natural order.  Registers and global
+// loads only.  TW: the warp's table (shared).
 template <int RMAX, bool HOLES>
 __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, const float4* __restrict__ TW,
-                                           float2* __restrict__ tile, int ja, int c, int lane, float2 (&v)[32]) {
+                                           int ja, int c, int lane, float2 (&v)[32]) {
   const int row_lo = es.e_lo >> kLogN2, row_hi = (es.e_hi - 1) >> kLogN2;
   const int R = row_hi - row_lo + 1;
   const int T = RMAX < 32 ? 1 : es.v ? a.n1 >> 10 : (R + 31) >> 5;    // pre-passed band: Q = NA / 32 rounds, every row of V valid
@@ -473,9 +472,6 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
       v[brev<32>(i)] = ldg_pred(p0 + i * kN2, ok);
     }
   }
-  // the previous tile's bulk store must have read the tile before anything is written to it
-  if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-  __syncwarp();
   if constexpr (RMAX == 32) {
     if (T > 1) {
       // The rounds below the top one, highest first: v = v g + X_t (Horner), the rows of a round loaded in groups of 8
@@ -522,12 +518,12 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
 }
 
 template <bool HOLES>
-__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float4* TW, float2* tile, int ja, int c, int lane,
+__device__ __forceinline__ void eff_warp(const P1Args& a, const EffSrc& es, const float4* TW, int ja, int c, int lane,
                                          float2 (&v)[32]) {
   const int R = ((es.e_hi - 1) >> kLogN2) - (es.e_lo >> kLogN2) + 1;
   // two pruned variants: more of them cost more in instruction-cache misses than their shorter transforms save
-  if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, tile, ja, c, lane, v);
-  else eff_phase1<32, HOLES>(a, es, TW, tile, ja, c, lane, v);
+  if (R <= 16) eff_phase1<16, HOLES>(a, es, TW, ja, c, lane, v);
+  else eff_phase1<32, HOLES>(a, es, TW, ja, c, lane, v);
 }
 
 __global__ void __launch_bounds__(kP1Warps * 32, kP1CtasPerSm) k_pass1_eff(P1Args a, const SlotDesc* __restrict__ slot_tab) {
@@ -570,8 +566,8 @@ __global__ void __launch_bounds__(kP1Warps * 32, kP1CtasPerSm) k_pass1_eff(P1Arg
     }
     __syncthreads();
   }
-  // The warp walks over its ja values.  The bulk store of a tile is only waited for when the tile is written again
-  // (eff_phase1, after the next tile's loads have been issued); TW of the next ja is fetched one iteration ahead.
+  // The warp walks over its ja values.  The bulk store of a tile is only waited for when the tile is written again,
+  // after the next ja's first 32-point transform; TW of the next ja is fetched one iteration ahead.
   float2 tw_next = __ldg(&a.tw_n1[(ja0 * (row_lo + lane)) & n1m]);
 #pragma unroll 1
   for (int ja = ja0; ja < ja1; ++ja) {
@@ -579,8 +575,11 @@ __global__ void __launch_bounds__(kP1Warps * 32, kP1CtasPerSm) k_pass1_eff(P1Arg
   __syncwarp();
   if (ja + 1 < ja1) tw_next = __ldg(&a.tw_n1[((ja + 1) * (row_lo + lane)) & n1m]);
   float2 v[32];
-  if (d.n_holes > 0) eff_warp<true>(a, es, TW, tile, ja, c, lane, v);
-  else eff_warp<false>(a, es, TW, tile, ja, c, lane, v);
+  if (d.n_holes > 0) eff_warp<true>(a, es, TW, ja, c, lane, v);
+  else eff_warp<false>(a, es, TW, ja, c, lane, v);
+  // the previous ja's bulk store must have read the tile before it is written again
+  if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+  __syncwarp();
   // the lane's column of the tile: tile[jb][m = lane]
   const unsigned col = (unsigned)__cvta_generic_to_shared(tile) | ((unsigned)lane << 3);
 #pragma unroll
