@@ -435,12 +435,6 @@ __device__ __forceinline__ bool eff_ok(const EffSrc& es, int k1, int k2, int fr,
   return ok;
 }
 
-// bit i = row r0 + i lies in [fr, lr] (the lane's valid rows of the band), i = 0..31
-__device__ __forceinline__ unsigned row_mask(int r0, int fr, int lr) {
-  const int lo = min(max(fr - r0, 0), 32), hi = min(max(lr - r0 + 1, 0), 32);
-  const unsigned below_hi = hi >= 32 ? 0xFFFFFFFFu : (1u << hi) - 1u, below_lo = lo >= 32 ? 0xFFFFFFFFu : (1u << lo) - 1u;
-  return below_hi & ~below_lo;
-}
 // predicated 8-byte load (no branch): 0 where !ok
 __device__ __forceinline__ float2 ldg_pred(const float2* p, bool ok) {
   float2 v = make_float2(0.f, 0.f);
@@ -472,11 +466,9 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
   {
     const int r0 = row_lo + 32 * (T - 1);
     const float2* __restrict__ p0 = round_ptr(T - 1);
-    const unsigned rm = row_mask(r0, fr, lr);
 #pragma unroll
     for (int i = 0; i < RMAX; ++i) {
-      bool ok = (rm >> i) & 1u;
-      if constexpr (HOLES) ok = ok && eff_ok<true>(es, r0 + i, k2, fr, lr);
+      const bool ok = eff_ok<HOLES>(es, r0 + i, k2, fr, lr);
       v[brev<32>(i)] = ldg_pred(p0 + i * kN2, ok);
     }
   }
@@ -488,13 +480,8 @@ __device__ __forceinline__ void eff_phase1(const P1Args& a, const EffSrc& es, co
       auto load_group = [&](int t, int gq, float2 (&dst)[8]) {
         const int r0 = row_lo + 32 * t + 8 * gq;
         const float2* __restrict__ p0 = round_ptr(t) + (size_t)(8 * gq) * kN2;
-        const unsigned rm = row_mask(r0, fr, lr);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          bool ok = (rm >> j) & 1u;
-          if constexpr (HOLES) ok = ok && eff_ok<true>(es, r0 + j, k2, fr, lr);
-          dst[j] = ldg_pred(p0 + j * kN2, ok);
-        }
+        for (int j = 0; j < 8; ++j) dst[j] = ldg_pred(p0 + j * kN2, eff_ok<HOLES>(es, r0 + j, k2, fr, lr));
       };
       const float2 g1 = a.tw_n1[(ja * 32) & (a.n1 - 1)];                          // e^{2 pi i ja/NA}
       const pk2 g = pk(g1), ig = pk(-g1.y, g1.x);
