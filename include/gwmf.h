@@ -203,6 +203,38 @@ int gwmf_path_in_use(const gwmf_ctx* ctx);
  * NULL = default stream); best of `repeats` >= 1 timed launches after one warm-up.  Needs no context.  syncs. */
 int gwmf_fma_peak(void* cuda_stream, int32_t repeats, double* host_tflops);
 
+/* The power table of Eq. 4 without a context, a workspace or any allocation:
+ *     C[k] = sum_{k' <= k} f_k'^(-7/3) / S_n[k']   over k_low = ceil(f_low n / fs) <= k' <= k,   C[k] = 0 below k_low,
+ * from which sigma^2 = 4 (fs/n) C[k_high - 1] and the p + 1 equal-power band edges of any template follow
+ * (e_l = 1 + min{k : C[k] >= (l/p) C[k_high - 1]}).  It is the table gwmf_load_segment builds inside its
+ * workspace, summed in the same fixed order, so the two agree bit for bit.
+ *
+ * Meant for callers that must not allocate device memory when the PSD changes: an online search whose running
+ * filters a cudaMalloc / cudaFree would stall (both serialise the whole device), a process whose memory a caching
+ * allocator or another pipeline already holds, a plug-in that may only touch the buffers it is handed.  The
+ * function calls no cudaMalloc, cudaFree or other allocating routine.  Its scratch (1024 partial sums and a status
+ * word, GWMF_STATIC_SCRATCH_BYTES in all) is a static array inside the library's device image: every GPU that loads
+ * the library carries those bytes until the process exits.
+ *
+ *   d_sn : DEVICE, n/2 + 1 fp64 samples of the one-sided PSD at f_k = k fs/n (input; entries below f_low and the
+ *          Nyquist entry are ignored, the others must be finite and > 0, else GWMF_E_ARG).
+ *   d_c  : DEVICE, n/2 fp64 entries (output, fully overwritten; must not overlap d_sn).  Caller-owned, as is d_sn.
+ *   n    : power of two, 2^14 .. GWMF_STATIC_MAX_N.  A larger n is refused with GWMF_E_CAPACITY (the scratch and the
+ *          kernels' shared-memory tiles are laid out for at most that many samples); other bad values are GWMF_E_ARG.
+ *   cuda_stream : a cudaStream_t of the CURRENT device (NULL = legacy default stream); the work runs on it.
+ *   err, err_len: optional HOST buffer that receives a one-line description of a failure ("" on success).
+ *
+ * Runs on the device that is current in the calling thread.  The first call on each device looks up the device
+ * address of the static array (cudaGetSymbolAddress; this may also make the driver load the library's device code),
+ * so make one call per device at start-up, outside any stream capture; later calls only launch three small kernels.
+ * All calls on a device share the one array and it keeps the previous call's contents; the function itself resets the
+ * part that must start from zero, on the given stream.  Two calls whose kernels can overlap on the same GPU (different
+ * streams, different host threads) race on it: serialise them.  syncs (it reads the status word back). */
+#define GWMF_STATIC_MAX_N (1 << 22)
+#define GWMF_STATIC_SCRATCH_BYTES 8448
+int gwmf_power_table_static(const double* d_sn, double* d_c, int64_t n, double fs, double f_low, void* cuda_stream,
+                            char* err, size_t err_len);
+
 /* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
 int64_t gwmf_launch_count(const gwmf_ctx* ctx);
 

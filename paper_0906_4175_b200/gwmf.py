@@ -22,7 +22,7 @@ PATH_NAMES = {v: k for k, v in PATHS.items()}
 EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
     "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_transform_counts", "gwmf_series", "gwmf_correlate",
-    "gwmf_fft_inverse",
+    "gwmf_fft_inverse", "gwmf_power_table_static",
     "gwmf_uses_fused", "gwmf_path_in_use", "gwmf_fma_peak", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
 
@@ -73,6 +73,8 @@ def load_library():
     L.gwmf_series.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.gwmf_correlate.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     L.gwmf_fft_inverse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.gwmf_power_table_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_void_p,
+                                          C.c_char_p, C.c_size_t]
     L.gwmf_uses_fused.argtypes = [C.c_void_p]
     L.gwmf_path_in_use.argtypes = [C.c_void_p]
     L.gwmf_fma_peak.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
@@ -102,6 +104,39 @@ def fma_peak(repeats=5, stream=None) -> float:
     if rc != OK:
         raise GwmfError(rc, load_library().gwmf_strerror(rc).decode())
     return out.value
+
+
+STATIC_MAX_N = 1 << 22            # GWMF_STATIC_MAX_N
+
+
+def power_table_static(Sn, n, fs=4096.0, f_low=40.0, out=None, stream=None):
+    """gwmf_power_table_static: the Eq. 4 power table C[k] (n/2 fp64 entries) of the PSD `Sn`, computed without a
+    context or a workspace and without any device allocation inside the library (its scratch is a static array in the
+    library image) -- for callers that must not cudaMalloc when the PSD changes; see include/gwmf.h.
+
+    Sn: torch float64 CUDA tensor of n/2 + 1 samples.  out: optional torch float64 CUDA tensor of n/2 entries on the
+    same device (pass one to keep this wrapper allocation-free too; otherwise it is created here, which is the
+    wrapper's doing, not the library's).  The work runs on `stream` (default: torch's current stream of Sn's device)
+    and the call returns when it is done.  Calls that may overlap on one GPU must be serialised by the caller."""
+    import torch
+    L = load_library()
+    if not (isinstance(Sn, torch.Tensor) and Sn.is_cuda and Sn.dtype == torch.float64 and Sn.is_contiguous()):
+        raise TypeError("Sn must be a contiguous float64 CUDA tensor")
+    if Sn.numel() != int(n) // 2 + 1:
+        raise ValueError("Sn must hold n/2 + 1 samples")
+    if out is None:
+        out = torch.empty(int(n) // 2, dtype=torch.float64, device=Sn.device)
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == int(n) // 2
+            and out.device == Sn.device):
+        raise TypeError("out must be a contiguous float64 CUDA tensor of n/2 entries on Sn's device")
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(Sn.device):
+        st = stream if stream is not None else torch.cuda.current_stream(Sn.device)
+        rc = L.gwmf_power_table_static(C.c_void_p(Sn.data_ptr()), C.c_void_p(out.data_ptr()), int(n), float(fs),
+                                       float(f_low), C.c_void_p(st.cuda_stream), err, len(err))
+    if rc != OK:
+        raise GwmfError(rc, err.value.decode() or L.gwmf_strerror(rc).decode())
+    return out
 
 
 class Filter:
