@@ -2,6 +2,7 @@
 // arithmetic (phase coefficients, k_high) and the launch sequences.  No compute happens on the host
 // beyond a handful of scalars per template.
 #include <math.h>
+#include <memory>
 #include <new>
 #include <stdlib.h>
 #include <string.h>
@@ -104,9 +105,11 @@ Layout make_layout(const gwmf_params* p) {
   L.q = take(2 * (size_t)L.batch * half * sizeof(float2));     // double-buffered across batches
   L.qb = take(path == GWMF_PATH_FUSED ? 2 * (size_t)L.batch * (n1 / 2 + kMaxBands + 2) * kN2 * sizeof(float2) : 256);   // band-separated copy (k_fused)
   // decimated path: per-band one-sided power spectra W_l and their sum U+, double-buffered across batches
-  L.wbuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * (size_t)p->p * kSubMax * kUCap * sizeof(float2) : 256);
-  L.ubuf = take(path == GWMF_PATH_DECIMATED ? 2 * (size_t)L.batch * kUCap * sizeof(float2) : 256);
-  L.bp_jobs = take(path == GWMF_PATH_DECIMATED ? bp_jobs_bytes() : 256);
+  // (not with chi^2 on demand: launch_bandpower never runs there and no effective band reads U+)
+  const bool band_powers = path == GWMF_PATH_DECIMATED && p->chisq_mode != GWMF_CHISQ_ON_DEMAND;
+  L.wbuf = take(band_powers ? 2 * (size_t)L.batch * (size_t)p->p * kSubMax * kUCap * sizeof(float2) : 256);
+  L.ubuf = take(band_powers ? 2 * (size_t)L.batch * kUCap * sizeof(float2) : 256);
+  L.bp_jobs = take(band_powers ? bp_jobs_bytes() : 256);
   L.pp_jobs = take((size_t)(L.y_slots + 8) * sizeof(int));
   size_t yb = (size_t)L.y_slots * n * sizeof(float2);
   if (yb < 3 * n * sizeof(float2)) yb = 3 * n * sizeof(float2);   // the dense transform needs in/mid/out
@@ -328,11 +331,16 @@ int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_t
   Ctx* c = reinterpret_cast<Ctx*>(ctx);
   DeviceGuard guard(c->device);
   if (n_templates < 1 || n_templates > c->prm.max_templates) return GWMF_E_ARG;
-  CU(cudaStreamSynchronize(c->stream));            // h_meta may still be in flight from a previous call
+  // Failure-atomic: h_meta is also the host mirror launch_correlate trims its grid with (k_high), so a bank that is
+  // rejected half way must leave it -- like the device bank, n_templates and have_bank -- describing the old bank.
+  std::unique_ptr<TemplateMeta[]> fresh(new (std::nothrow) TemplateMeta[(size_t)n_templates]);
+  if (!fresh) return GWMF_E_ARG;
   for (int t = 0; t < n_templates; ++t) {
-    int rc = fill_template(c, host_masses[t], &c->h_meta[t]);
+    int rc = fill_template(c, host_masses[t], &fresh[(size_t)t]);
     if (rc != GWMF_OK) return rc;
   }
+  CU(cudaStreamSynchronize(c->stream));            // h_meta may still be in flight from a previous call
+  memcpy(c->h_meta, fresh.get(), sizeof(TemplateMeta) * (size_t)n_templates);
   CU(cudaMemcpyAsync(ws_ptr<TemplateMeta>(c, c->lay.meta), c->h_meta, sizeof(TemplateMeta) * (size_t)n_templates,
                      cudaMemcpyHostToDevice, c->stream));
   c->n_templates = n_templates;

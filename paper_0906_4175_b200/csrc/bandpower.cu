@@ -424,24 +424,47 @@ cudaError_t launch_bandpower(Ctx* c, int first, int count, int parity, cudaStrea
   int* n_jobs = jobs + kBpClasses * kBpJobCap;
   k_bp_jobs<<<1, 1024, 0, st>>>(meta, p, count, jobs, n_jobs);
   c->launches++;
-  cudaError_t e;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
   const bool fork = c->s_bins > 1024;
   if (fork && (e = cudaEventRecord(c->ev_bp_fork, st)) != cudaSuccess) return e;
   auto grid_of = [&](int log_l) { return bp_ctas(log_l) * c->n_sms; };    // the CTAs of a kernel that can be resident
   k_bandpower<11, false><<<grid_of(11), bp_threads(11), bp_smem(11), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
   c->launches++;
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  // A side stream must have waited for the fork (the job list of THIS batch) before anything is launched on it: a
+  // failed wait is returned, not launched past.
   int used = 0;
-  auto side = [&](int i) -> cudaStream_t {
-    cudaStreamWaitEvent(c->bp[i], c->ev_bp_fork, 0);
+  auto side = [&](int i, cudaStream_t* out) -> cudaError_t {
+    const cudaError_t w = cudaStreamWaitEvent(c->bp[i], c->ev_bp_fork, 0);
+    if (w != cudaSuccess) return w;
     used |= 1 << i;
-    return c->bp[i];
+    *out = c->bp[i];
+    return cudaSuccess;
   };
-  if (c->s_bins > 1024) { k_bandpower<12, false><<<grid_of(12), bp_threads(12), bp_smem(12), side(0)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
-  if (c->s_bins > 2048) { k_bandpower<13, false><<<grid_of(13), bp_threads(13), bp_smem(13), side(1)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
-  if (c->s_bins > 4096) { k_bandpower<14, false><<<grid_of(14), bp_threads(14), bp_smem(14), side(2)>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs); c->launches++; }
+  cudaStream_t sx = nullptr;
+  if (c->s_bins > 1024) {
+    if ((e = side(0, &sx)) != cudaSuccess) return e;
+    k_bandpower<12, false><<<grid_of(12), bp_threads(12), bp_smem(12), sx>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+    c->launches++;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  if (c->s_bins > 2048) {
+    if ((e = side(1, &sx)) != cudaSuccess) return e;
+    k_bandpower<13, false><<<grid_of(13), bp_threads(13), bp_smem(13), sx>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+    c->launches++;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  if (c->s_bins > 4096) {
+    if ((e = side(2, &sx)) != cudaSuccess) return e;
+    k_bandpower<14, false><<<grid_of(14), bp_threads(14), bp_smem(14), sx>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
+    c->launches++;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
   if (c->s_bins > kLMax / 2) {                    // bands on grids of 2^15 or 2^16 points: up to kSubMax sub-grid jobs each
     k_bandpower<14, true><<<grid_of(14), bp_threads(14), bp_smem(14), st>>>(meta, q, tw_l, wbuf, p, (int)half, jobs, n_jobs);
     c->launches++;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
   for (int i = 0; i < 3; ++i) {
     if (!(used & (1 << i))) continue;

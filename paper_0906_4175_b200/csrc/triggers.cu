@@ -138,12 +138,18 @@ __global__ void __launch_bounds__(256) k_chisq_at(Slot* __restrict__ slots, cons
 }
 
 cudaError_t launch_chisq_at_events(Ctx* c, int first, int count) {
-  if (count <= 0) return cudaSuccess;
-  k_chisq_at<<<dim3(c->n_windows, count), 256, 0, c->stream>>>(
-      ws_ptr<Slot>(c, c->lay.slots) + (size_t)first * c->n_windows, ws_ptr<TemplateMeta>(c, c->lay.meta) + first,
-      wq_buf(c, c->front), ws_ptr<double>(c, c->lay.u_tab), c->prm.p, c->n_windows, c->log_n);
-  c->launches++;
-  return cudaGetLastError();
+  // the template index rides on gridDim.y (at most 65535): a longer range goes out in several launches
+  constexpr int kMaxGridY = 65535;
+  for (int done = 0; done < count; done += kMaxGridY) {
+    const int t0 = first + done, cnt = count - done < kMaxGridY ? count - done : kMaxGridY;
+    k_chisq_at<<<dim3(c->n_windows, cnt), 256, 0, c->stream>>>(
+        ws_ptr<Slot>(c, c->lay.slots) + (size_t)t0 * c->n_windows, ws_ptr<TemplateMeta>(c, c->lay.meta) + t0,
+        wq_buf(c, c->front), ws_ptr<double>(c, c->lay.u_tab), c->prm.p, c->n_windows, c->log_n);
+    c->launches++;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 cudaError_t launch_reset_slots(Ctx* c, int first, int count) {

@@ -46,7 +46,7 @@ def assert_triggers(trig_gpu, bank_out, thresh, W, p, template_ids=None, series_
     # the device list must be sorted by (template, window) with one entry per cell
     keys = [(int(t["template_id"]), int(t["sample"]) // W) for t in trig_gpu]
     assert keys == sorted(keys) and len(set(keys)) == len(keys), "trigger order / uniqueness"
-    compared = exempt = 0
+    compared = exempt = shifted = 0
     for i, tid in enumerate(ids):
         for w in range(nw):
             rho = bank_out["best_rho"][i, w]
@@ -67,6 +67,7 @@ def assert_triggers(trig_gpu, bank_out, thresh, W, p, template_ids=None, series_
                     assert rho_s[jo] - rho_s[jg] <= NEIGHBOUR_MARGIN, (tid, w, g, jo, rho_s[jo], rho_s[jg])
                     rho, chi = float(rho_s[jg]), float(chi_s[jg])
                     exempt += 1
+                    shifted += 1
                 else:
                     assert jg == jo, (tid, w, g, jo)
                 assert abs(float(g["rho"]) - rho) <= RHO_ABS + RHO_REL * rho
@@ -74,4 +75,9 @@ def assert_triggers(trig_gpu, bank_out, thresh, W, p, template_ids=None, series_
                 compared += 1
             else:
                 assert g is None, f"spurious trigger: template {tid} window {w}: {g} (oracle max {rho})"
+    # an event one sample off the oracle's is accepted only as a near-tie of two neighbouring samples, which is rare: a
+    # systematic shift (an off-by-one in the index mapping) must not slip through as many such "ties"
+    if shifted:
+        print(f"assert_triggers: {shifted} of {compared} compared events sit one sample off the oracle's (near-ties)")
+    assert shifted <= max(2, 0.02 * compared), f"{shifted} of {compared} events are one sample off the oracle's"
     return compared, exempt

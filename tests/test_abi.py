@@ -51,6 +51,8 @@ def test_workspace_bytes_host_only(lib):
     # double-buffered correlated spectra (2 * 128 * 4 MiB = 1 GiB); tables / slots / staging
     assert (9 << 30) < b < (9 << 30) + (512 << 20)
     assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, batch=2) < (700 << 20)
+    # chi^2 on demand runs no band-power stage: its 4 GiB of per-band spectra (and U+, and the job lists) are not carved
+    assert gwmf.workspace_bytes(1 << 20, 16, 4096, 1024, chisq_on_demand=True) < b - (4 << 30)
     assert lib.gwmf_strerror(-2).decode().startswith("empty template")
     assert lib.gwmf_strerror(0).decode() == "ok"
 

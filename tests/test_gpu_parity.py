@@ -496,6 +496,41 @@ def test_wide_band_inside_narrow_ones(gw, path):
     parity.assert_triggers(f.triggers(), out, 5.0, 4096, 16)
 
 
+@pytest.mark.parametrize("snr", [100.0, 300.0])
+def test_loud_events(gw, path, snr):
+    # The veto exists for loud events (section 1.2).  A matched injection of optimal SNR 100, 300, 1000 in
+    # Eq. 2 noise at the headline shape: every sample of the matched template and of a mismatched one (large chi^2),
+    # and the events of the whole bank, at the tolerances of every other test.  chi^2 at such a sample is a small
+    # number next to rho^2; reading 17 says how the library evaluates it there.
+    n, p, W = 1 << 20, 16, 4096
+    masses = [(3.0, 1.2), (3.3, 1.25), (1.4, 1.4), (10.0, 8.0)]
+    jc = 5 * n // 8 + 123
+    D = inputs.noise_spectrum(n, 91) + inputs.injection_spectrum(n, 3.0, 1.2, snr, jc)
+    s = inputs.time_series(D, n).astype(np.float32)
+    s64 = s.astype(np.float64)
+    Sn = inputs.psd_array(n)
+    w = inputs.Workload(config=-1, n=n, p=p, rho_thresh=6.0, window=W, masses=masses, seed=0)
+    f = _run_gpu(gw, w, s, Sn, path=path)
+    out = oracle.filter_bank(s64, Sn, masses, p, W, 6.0)
+    parity.assert_sigma_edges(f.sigma(), f.band_edges(), out["sigma"], out["edges"])
+    assert abs(out["best_rho"][0].max() - snr) < 5.0          # the injection is found at about its SNR
+    series = {}
+
+    def series_of(tid):
+        if tid not in series:
+            series[tid] = oracle.filter_template(s64, Sn, masses[tid][0], masses[tid][1], p)[:2]
+        return series[tid]
+
+    compared, _ = parity.assert_triggers(f.triggers(), out, 6.0, W, p, series_of=series_of)
+    assert compared >= 4
+    for t in (0, 1):
+        rho_o, chi_o = series_of(t)
+        rho_g, chi_g = f.series(t)
+        parity.assert_series(rho_g, chi_g, rho_o, chi_o, p, f"loud injection, SNR {snr}, template {t}")
+    j = int(np.argmax(series_of(0)[0]))
+    assert abs(j - jc) <= 1 and series_of(1)[1].max() > 50.0 * series_of(0)[1][j]   # matched: small chi^2; mismatched: large
+
+
 # ----------------------------------------------------------------------------- edge cases and the boundary
 def test_p_extremes_and_covariance(gw, path):
     n = 1 << 15
@@ -609,6 +644,30 @@ def test_error_codes(gw):
     with pytest.raises(gw.GwmfError) as e:
         f.triggers()
     assert e.value.status == gw.E_ARG
+
+
+def test_rejected_bank_leaves_the_old_bank_intact(gw, path):
+    # gwmf_make_bank is failure-atomic: a bank that is refused half way (here its second template is empty) must not
+    # disturb the loaded one, including the host mirror of k_high the correlate grid is trimmed with.  The filter of
+    # templates 2, 3 in between leaves THEIR spectra in the buffers template 0 uses next, so a grid cut at the
+    # rejected bank's smaller k_high would pick up foreign bins.
+    n = 1 << 16
+    masses = [(1.4, 1.4), (1.2, 1.0), (3.0, 1.2), (5.0, 5.0)]
+    s = inputs.time_series(inputs.noise_spectrum(n, 31) + inputs.injection_spectrum(n, 1.4, 1.4, 9.0, 20000), n)
+    f = gw.Filter(n, 8, 4096, 4, rho_thresh=4.0, batch=2, path=_path_for(path, n))
+    f.make_bank(masses)
+    f.load_segment(s.astype(np.float32), inputs.psd_array(n))
+    f.filter()
+    ref = f.triggers().copy()
+    sig, edges = f.sigma().copy(), f.band_edges().copy()
+    assert len(ref) > 8
+    f.filter(2, 2)
+    with pytest.raises(gw.GwmfError) as e:
+        f.make_bank([(30.0, 30.0), (80.0, 80.0)])              # template 0 would get a far smaller k_high; template 1 is empty
+    assert e.value.status == gw.E_EMPTY_TEMPLATE
+    f.filter()
+    assert f.triggers().tobytes() == ref.tobytes()
+    assert np.array_equal(f.sigma(), sig) and np.array_equal(f.band_edges(), edges)
 
 
 def test_no_triggers_when_threshold_is_high(gw):
