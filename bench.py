@@ -263,6 +263,8 @@ def spawn_ranks(args) -> int:
 
 
 STAGES = ("spectra", "pass1", "pass2", "chisq_at_events")
+CHISQ_AT_TEXT = ("Eq. 5 evaluated from its definition at event samples: k_chisq_loud (every-sample mode: only events with "
+                 "rho > 48 or in loud data, DESIGN.md reading 23) or k_chisq_at (chi^2 on demand: every event)")
 STAGE_TEXT = {
     "decimated": {
         "spectra": "k_correlate_cm + k_bp_jobs + k_bandpower (5 kernels side by side) + k_uspec (template phasors x data, "
@@ -271,17 +273,19 @@ STAGE_TEXT = {
         "pass1": "k_pass1_eff (first FFT pass of every effective band: writes n complex fp32 per n-point transform) "
                  "[+ k_prepass for bands of very many input rows: one more n complex written and read]",
         "pass2": "k_pass2_eff (last FFT stage + rho/chi^2/trigger epilogue: reads n complex fp32 per n-point transform)",
-        "chisq_at_events": "k_chisq_at (chi^2 on demand: Eq. 5 evaluated from its definition at every event's sample)"},
+        "chisq_at_events": CHISQ_AT_TEXT},
     "two_pass": {
         "spectra": "-",
         "pass1": "k_pass1_narrow (pruned column FFT + first row stage, writes p*N*8 B/template) with the low-volume kernels "
                  "(k_correlate, k_pass1 generic, k_rowstage) beside it on the side stream; timed fork to join",
-        "pass2": "k_pass2 (last FFT stage + rho/chi^2/trigger epilogue, reads p*N*8 B/template)"},
+        "pass2": "k_pass2 (last FFT stage + rho/chi^2/trigger epilogue, reads p*N*8 B/template)",
+        "chisq_at_events": CHISQ_AT_TEXT},
     "fused": {
         "spectra": "-",
         "pass1": "wide bands only: k_pass1 generic + k_rowstage (side stream; the next batch's correlates run beside k_fused)",
         "pass2": "k_fused (spill-free: narrow bands formed from the correlated spectrum, both row-transform stages, "
-                 "rho/chi^2/trigger epilogue; no band intermediate in HBM)"},
+                 "rho/chi^2/trigger epilogue; no band intermediate in HBM)",
+        "chisq_at_events": CHISQ_AT_TEXT},
 }
 
 

@@ -139,7 +139,14 @@ int gwmf_load_segment(gwmf_ctx* ctx, const float* s, const double* Sn);
  * (the FIRST call after a bank or PSD change waits on the host for the bank setup to finish: it reads back how
  * many transforms each template needs; later calls do not wait):
  * p band inverse FFTs, rho and chi^2 at every sample (Eq. 3, 5) and the per-window
- * maxima above threshold.  Trigger slots of those templates are reset first.  async. */
+ * maxima above threshold.  Trigger slots of those templates are reset first.
+ * Loud data (reading 23): the transforms' epilogue forms chi^2 in fp32 as sum_l |z_l|^2 - |z|^2 / p, two
+ * terms of size rho^2 / p whose difference keeps about rho^2 * 5e-7 of absolute error, and the transforms' own fp32
+ * error grows with the mean power of the data in the template's band.  The call therefore re-evaluates chi^2 at the
+ * event's sample from Eq. 5 as printed, sum_l |z_l - z/p|^2 with z_l[j] = sum_{k in band l} Q[k] e^{2 pi i jk/n} (one
+ * pass over the template's bins per event), for every event with rho > 48 and for every event of a template in whose
+ * band the segment's mean power (sum_l |z_l|^2 averaged over the n samples, 2 in noise) exceeds 4 -- a signal of
+ * SNR >~ 300 at n = 2^20, matched by that template or not.  gwmf_series applies the same rule per sample.  async. */
 int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
 
 /* Measurement: the same work as gwmf_filter, with CUDA events recorded on the context's stream around the
@@ -150,7 +157,8 @@ int gwmf_filter(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates);
  *   [1] pass 1: first FFT pass of every (effective) band -> band intermediate in HBM; for the spill-free path only
  *       the wide bands' kernels;
  *   [2] pass 2: last FFT stage + rho/chi^2/trigger epilogue (spill-free path: k_fused);
- *   [3] chi^2 at the event samples (chisq_mode = ON_DEMAND only, else 0).
+ *   [3] chi^2 from its definition at event samples: every event with chisq_mode = ON_DEMAND, otherwise only the
+ *       loud ones (see gwmf_filter).
  * host_launches: HOST array of 4 int32, launches / batches timed in each stage.  syncs. */
 int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates, double* host_ms,
                       int32_t* host_launches);

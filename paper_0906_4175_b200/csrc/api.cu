@@ -85,6 +85,8 @@ Layout make_layout(const gwmf_params* p) {
   L.g_tab = take(half * sizeof(double));
   L.sn = take((half + 1) * sizeof(double));
   L.wq = take(2 * half * sizeof(float2));                      // double-buffered across segments
+  L.pw_tab = take(2 * half * sizeof(double));                  // prefix power of each wq buffer (reading 23)
+  L.pw_totals = take(2 * 1024 * sizeof(double));
   L.s_in = take(2 * n * sizeof(float));
   L.prep = take(3 * n * sizeof(float2));                       // segment preparation scratch: input, intermediate, transform
   L.tw_n1 = take(n1 * sizeof(float2));
@@ -529,9 +531,12 @@ static int run_batches(Ctx* c, int first_template, int n_templates, cudaEvent_t*
       if (evb) CU(cudaEventRecord(evb[3], c->stream));
     }
   }
-  if (c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND) {
+  // chi^2 from its definition (Eq. 5 as printed): at every event with chi^2 on demand, else at the loud ones, where the
+  // epilogue's fp32 difference sum |z_l|^2 - |z|^2 / p has lost its digits (readings 21, 23)
+  {
+    const bool on_demand = c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND;
     if (ev) CU(cudaEventRecord(ev[4 * batches.size()], c->stream));
-    CU(launch_chisq_at_events(c, first_template, n_templates));
+    CU(launch_chisq_at_events(c, first_template, n_templates, !on_demand));
     if (ev) CU(cudaEventRecord(ev[4 * batches.size() + 1], c->stream));
   }
   return end_segment_use(c);
@@ -586,13 +591,11 @@ int gwmf_filter_timed(gwmf_ctx* ctx, int32_t first_template, int32_t n_templates
     }
   host_launches[0] = c->path == GWMF_PATH_DECIMATED ? nb : 0;
   host_launches[1] = host_launches[2] = nb;
-  host_ms[3] = 0.0;
-  host_launches[3] = 0;
-  if (c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND) {
+  {
     float m = 0.f;
     CU(cudaEventElapsedTime(&m, ev.v[4 * nb], ev.v[4 * nb + 1]));
     host_ms[3] = m;
-    host_launches[3] = 1;
+    host_launches[3] = c->prm.chisq_mode == GWMF_CHISQ_ON_DEMAND ? (n_templates + 65534) / 65535 : 1;
   }
   return GWMF_OK;
 }
@@ -706,6 +709,7 @@ int gwmf_series(gwmf_ctx* ctx, int32_t template_id, float* host_rho, float* host
     if (c->fused) CU(launch_fused_filter(c, template_id, 1, 0, false, d_rho, d_chi));
     else CU(launch_pass2_filter(c, template_id, 1, false, d_rho, d_chi));
   }
+  if (c->prm.chisq_mode != GWMF_CHISQ_ON_DEMAND) CU(launch_chisq_series_loud(c, template_id, d_rho, d_chi));
   if (host_rho)
     CU(cudaMemcpyAsync(host_rho, d_rho, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
   if (host_chisq)

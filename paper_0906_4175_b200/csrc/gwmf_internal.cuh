@@ -105,7 +105,7 @@ struct alignas(16) Slot {
 
 struct Layout {                  // byte offsets into the caller's workspace
   size_t u_tab, c_tab, g_tab, sn, wq, s_in, tw_n1, tw_p2, meta, masks, prefix_totals, slots, counts, offsets, trig_out,
-         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, bp_jobs, vbuf, pp_jobs, total;
+         series_rho, series_chi, flags, q, qb, y, tw_l, wbuf, ubuf, eff, slot_tab, prep, bp_jobs, vbuf, pp_jobs, pw_tab, pw_totals, total;
   size_t y_bytes;
   int batch;                     // most templates per launch
   int y_slots;                   // n-point transforms (n complex fp32 each) the band buffer holds
@@ -156,6 +156,7 @@ struct Ctx {
   cudaEvent_t ev_last_load;      // end of the latest load (orders the shared preparation scratch between streams)
 };
 inline float2* wq_buf(Ctx* c, int b) { return reinterpret_cast<float2*>(c->ws + c->lay.wq) + (size_t)b * (size_t)(c->n / 2); }
+inline double* pw_buf(Ctx* c, int b) { return reinterpret_cast<double*>(c->ws + c->lay.pw_tab) + (size_t)b * (size_t)(c->n / 2); }   // P[k] of wq[b]
 inline float* s_buf(Ctx* c, int b) { return reinterpret_cast<float*>(c->ws + c->lay.s_in) + (size_t)b * (size_t)c->n; }
 
 // ---- launchers (defined in the .cu files) --------------------------------------------------------
@@ -191,7 +192,8 @@ cudaError_t launch_pass1_eff(Ctx* c, int first, int count, int parity, cudaStrea
 cudaError_t launch_prepass(Ctx* c, int first, int count, int parity, cudaStream_t st);   // bands of very many rows -> vbuf
 cudaError_t launch_pass2_eff(Ctx* c, int bfirst, int bcount, int first, int count, bool update_slots, float* series_rho,
                              float* series_chi);
-cudaError_t launch_chisq_at_events(Ctx* c, int first, int count);      // chi^2 on demand: fills the slots' chi^2
+cudaError_t launch_chisq_at_events(Ctx* c, int first, int count, bool loud_only);   // chi^2 from its definition at the events (all, or rho > kRhoLoud)
+cudaError_t launch_chisq_series_loud(Ctx* c, int template_id, const float* series_rho, float* series_chi);   // the same for a series
 cudaError_t launch_reset_slots(Ctx* c, int first, int count);
 cudaError_t launch_compact(Ctx* c);
 

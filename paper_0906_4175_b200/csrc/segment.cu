@@ -134,6 +134,41 @@ __global__ void k_weighted_spectrum(const float2* __restrict__ Z, const double* 
   wq[k] = out;
 }
 
+// Mean power of the segment in a template's band (reading 23): P[k] = sum_{k' <= k} |wq[k']|^2, the same
+// fixed-order chunked fp64 prefix sum as C[k] with the terms formed on the fly.  By Parseval the mean over the n samples
+// of sum_l |z_l|^2, in units of rho^2, is scale_rho2 * P[k_high - 1] for every template: 2 in noise alone, more when the
+// data hold a loud signal in the band -- matched by this template or not.
+__device__ __forceinline__ double wq_power(const float2* __restrict__ wq, int k) {
+  const float2 v = wq[k];
+  return (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+}
+
+__global__ void __launch_bounds__(32) k_pw_totals(const float2* __restrict__ wq, double* __restrict__ totals, int half_n, int L) {
+  extern __shared__ double sh[];
+  const int lo = blockIdx.x * L, hi = min(lo + L, half_n);
+  for (int k = lo + threadIdx.x; k < hi; k += 32) sh[k - lo] = wq_power(wq, k);
+  __syncwarp();
+  if (threadIdx.x == 0) {
+    double acc = 0.0;
+    for (int k = 0; k < hi - lo; ++k) acc += sh[k];
+    totals[blockIdx.x] = acc;
+  }
+}
+
+__global__ void __launch_bounds__(32) k_pw_write(const float2* __restrict__ wq, const double* __restrict__ offsets,
+                                                 double* __restrict__ pw, int half_n, int L) {
+  extern __shared__ double sh[];
+  const int lo = blockIdx.x * L, hi = min(lo + L, half_n);
+  for (int k = lo + threadIdx.x; k < hi; k += 32) sh[k - lo] = wq_power(wq, k);
+  __syncwarp();
+  if (threadIdx.x == 0) {
+    double acc = offsets[blockIdx.x];
+    for (int k = 0; k < hi - lo; ++k) { acc += sh[k]; sh[k] = acc; }
+  }
+  __syncwarp();
+  for (int k = lo + threadIdx.x; k < hi; k += 32) pw[k] = sh[k - lo];
+}
+
 // The preparation is cut in three so that the part that depends only on the samples (the transform) can run on the
 // upload stream while filters of the previous segment still use the PSD tables and the other wq buffer.
 // Scratch (own region of the workspace, 3 n complex): X = the segment as complex input, mid, Z = its transform.
@@ -172,6 +207,16 @@ cudaError_t launch_weighted_spectrum(Ctx* c, int buf, cudaStream_t st) {
                                                           ws_ptr<double>(c, c->lay.c_tab), wq_buf(c, buf), c->k_low, half,
                                                           4.0 / (double)c->n, 4.0 * c->df);
   c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  // power table of this buffer's weighted spectrum (own chunk totals per buffer: loads of the two buffers may overlap)
+  const int L = (half + kPrefixChunks - 1) / kPrefixChunks;
+  const size_t sm = (size_t)L * sizeof(double);
+  double* totals = ws_ptr<double>(c, c->lay.pw_totals) + (size_t)buf * kPrefixChunks;
+  k_pw_totals<<<kPrefixChunks, 32, sm, st>>>(wq_buf(c, buf), totals, half, L);
+  k_prefix_scan<<<1, 1, 0, st>>>(totals);
+  k_pw_write<<<kPrefixChunks, 32, sm, st>>>(wq_buf(c, buf), totals, pw_buf(c, buf), half, L);
+  c->launches += 3;
   return cudaGetLastError();
 }
 

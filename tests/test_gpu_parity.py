@@ -496,12 +496,12 @@ def test_wide_band_inside_narrow_ones(gw, path):
     parity.assert_triggers(f.triggers(), out, 5.0, 4096, 16)
 
 
-@pytest.mark.parametrize("snr", [100.0, 300.0])
+@pytest.mark.parametrize("snr", [100.0, 300.0, 1000.0])
 def test_loud_events(gw, path, snr):
     # The veto exists for loud events (section 1.2).  A matched injection of optimal SNR 100, 300, 1000 in
     # Eq. 2 noise at the headline shape: every sample of the matched template and of a mismatched one (large chi^2),
     # and the events of the whole bank, at the tolerances of every other test.  chi^2 at such a sample is a small
-    # number next to rho^2; reading 17 says how the library evaluates it there.
+    # number next to rho^2; reading 23 says how the library evaluates it there.
     n, p, W = 1 << 20, 16, 4096
     masses = [(3.0, 1.2), (3.3, 1.25), (1.4, 1.4), (10.0, 8.0)]
     jc = 5 * n // 8 + 123
@@ -529,6 +529,37 @@ def test_loud_events(gw, path, snr):
         parity.assert_series(rho_g, chi_g, rho_o, chi_o, p, f"loud injection, SNR {snr}, template {t}")
     j = int(np.argmax(series_of(0)[0]))
     assert abs(j - jc) <= 1 and series_of(1)[1].max() > 50.0 * series_of(0)[1][j]   # matched: small chi^2; mismatched: large
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_template_sharded_plan_on_the_cuda_path(gw, world):
+    # SURVEY.md 8(e) / 8(f)-4, PAPER.md:75,196 (independent work, the multi-GPU extrapolation): bench.py's
+    # template-sharded mode gives rank r the range shard_plan(world, r, T, "templates") of ONE bank against ONE segment
+    # and concatenates the ranks' event lists in rank order (gather_triggers).  Here every "rank" is a context of its
+    # own on cuda:0: the concatenated list must be byte-identical to the single-context list.  world = 3 cuts config
+    # 1's 256 templates at odd indices, i.e. through the template pairs (2i, 2i+1) that share a transform.
+    import bench
+    w = inputs.workload(1)
+    s = inputs.segment(w).astype(np.float32)
+    T = len(w.masses)
+    whole = _run_gpu(gw, w, s, w.psd, thresh=4.5)
+    ref = whole.triggers()
+    assert len(ref) > 2 * T                                  # a dense list: several events per template at rho* = 4.5
+    parts, covered = [], 0
+    for r in range(world):
+        _, first, count = bench.shard_plan(world, r, T, "templates")
+        assert first == covered
+        covered += count
+        f = gw.Filter(w.n, w.p, w.window, T, rho_thresh=4.5)
+        f.make_bank(w.masses)
+        f.load_segment(s, w.psd)
+        f.filter(first, count)
+        t = f.triggers()
+        assert np.all((t["template_id"] >= first) & (t["template_id"] < first + count))
+        parts.append(t)
+        f.close()
+    assert covered == T
+    assert np.concatenate(parts).tobytes() == ref.tobytes()
 
 
 # ----------------------------------------------------------------------------- edge cases and the boundary
