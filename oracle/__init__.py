@@ -51,6 +51,8 @@ def lib():
         L.orc_k_low.argtypes = [C.c_long, C.c_double, C.c_double]
         L.orc_k_low.restype = C.c_long
         L.orc_phase.argtypes = [C.c_double, C.c_double, C.c_double]
+        L.orc_amplitude.argtypes = [C.c_double, C.c_double, C.c_double]
+        L.orc_amplitude.restype = C.c_double
         L.orc_phase.restype = C.c_double
         L.orc_template.argtypes = [C.c_double, C.c_double, C.c_long, C.c_double, C.c_double, _dp, _dp]
         L.orc_power_table.argtypes = [_dp, C.c_long, C.c_double, C.c_double, _dp]
@@ -117,6 +119,11 @@ def k_high(m1, m2, n, fs=4096.0) -> int:
 
 def phase(m1, m2, f) -> float:
     return lib().orc_phase(float(m1), float(m2), float(f))
+
+
+def amplitude(m1, m2, d_eff_mpc=1.0) -> float:
+    """Physical amplitude constant of the template for a source at d_eff_mpc megaparsecs (O10)."""
+    return lib().orc_amplitude(float(m1), float(m2), float(d_eff_mpc))
 
 
 def template(m1, m2, n, fs=4096.0, f_low=40.0) -> np.ndarray:

@@ -33,6 +33,25 @@ static const double ORC_T_SUN = 4.9254909476412675e-6;
 
 double orc_t_sun(void) { return ORC_T_SUN; }
 
+/* O10. Physical amplitude of the Newtonian-amplitude stationary-phase template ("Newtonian
+ * amplitude", "effective distance D_eff"; the paper prints no value -- SURVEY.md 8(c2) reading 4 writes the
+ * constant out):  h~(f) = A f^(-7/6) e^{i Psi(f)},
+ *     A = sqrt(5/24) pi^(-2/3) (c / D_eff) (T_sun M_chirp / M_sun)^(5/6),   M_chirp = (m1 m2)^(3/5) / (m1+m2)^(1/5),
+ * in seconds^(-1/6) (strain per Hz times Hz^(7/6)) for D_eff in megaparsecs and masses in solar masses.
+ * c = 299792458 m/s exactly; 1 Mpc = 3.0856775814913673e22 m (IAU 2015: 648000/pi au, au = 149597870700 m).
+ * With the library's sigma (Eq. 4 with A = 1) and a PSD given in units of `psd_unit` strain^2/Hz, a source at D_eff
+ * has optimal SNR  rho_opt = A(D_eff) sigma / sqrt(psd_unit); the distance at which rho_opt = 1 is
+ * D_1 = A(1 Mpc) sigma / sqrt(psd_unit) Mpc, and an event of SNR rho lies at D_eff = D_1 / rho.
+ * Pins (tests/test_oracle_pins.py): the M_chirp^(5/6) and 1/D_eff scaling laws, a value evaluated by hand from the
+ * constants in tests/golden/p12_amplitude.txt, and the textbook horizon of a 1.4+1.4 binary in the initial-LIGO
+ * design curve. */
+double orc_amplitude(double m1, double m2, double d_eff_mpc)
+{
+    const double c_light = 299792458.0, mpc = 3.0856775814913673e22;
+    double mchirp = pow(m1 * m2, 0.6) / pow(m1 + m2, 0.2);
+    return sqrt(5.0 / 24.0) * pow(ORC_PI, -2.0 / 3.0) * (c_light / (d_eff_mpc * mpc)) * pow(ORC_T_SUN * mchirp, 5.0 / 6.0);
+}
+
 /* ------------------------------------------------------------------------------------------
  * Discrete Fourier transforms.  sign = +1: X[k] = sum_j x[j] e^{+2 pi i jk/n} (the "e^{2 pi i f t}"
  * of Eq. 1); sign = -1: the ordinary forward DFT.  Unnormalised, in place.

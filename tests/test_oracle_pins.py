@@ -327,3 +327,26 @@ def test_trigger_rule():
     assert ru[0] == 7.0        # the tied sample is a competing peak
     assert ru[1] == 5.0
     assert ru[2] == 3.0        # 22 is a neighbour of the peak, not a competing peak
+
+
+# ----------------------------------------------------------------------------- P12: physical amplitude / D_eff
+def test_p12_amplitude_value_scaling_laws_and_horizon(golden_dir):
+    # O10 (SURVEY.md 8(c2) reading 4).  (a) the value evaluated by hand, by logarithms, in the golden file;
+    for m1, m2, d, want in _rows(os.path.join(golden_dir, "p12_amplitude.txt")):
+        assert abs(oracle.amplitude(m1, m2, d) - want) <= 2e-11 * want
+    # (b) scaling laws: A ~ 1 / D_eff; A depends on the masses through M_chirp^(5/6) only, so scaling both masses by k
+    # scales A by k^(5/6), and two different pairs with one chirp mass share A
+    a = oracle.amplitude(3.0, 1.2, 1.0)
+    assert abs(oracle.amplitude(3.0, 1.2, 40.0) * 40.0 / a - 1.0) < 1e-14
+    assert abs(oracle.amplitude(6.0, 2.4, 1.0) / a - 2.0 ** (5.0 / 6.0)) < 1e-14
+    assert abs(oracle.amplitude(1.2, 3.0, 1.0) / a - 1.0) < 1e-15
+    mc = (3.0 * 1.2) ** 0.6 / 4.2 ** 0.2
+    m = mc * 2.0 ** 0.2                                   # the equal-mass pair with the same chirp mass
+    assert abs(oracle.amplitude(m, m, 1.0) / a - 1.0) < 1e-13
+    # (c) the literature's number (not this code's): the SNR-8 horizon of a 1.4+1.4 binary in the initial-LIGO design
+    # curve, of which Eq. 2 x 9e-46/Hz is the fit, is about 33 Mpc (sky-averaged range 14-15 Mpc)
+    n = 1 << 18
+    C = oracle.power_table(inputs.psd_array(n), n)
+    sigma, _ = oracle.sigma_edges(C, n, oracle.k_high(1.4, 1.4, n), 16)
+    horizon = oracle.amplitude(1.4, 1.4, 1.0) * sigma / math.sqrt(9e-46) / 8.0
+    assert 28.0 < horizon < 36.0, horizon
