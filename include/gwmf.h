@@ -174,6 +174,24 @@ int gwmf_triggers(gwmf_ctx* ctx, gwmf_trigger* host_out, int64_t capacity, int64
  * doubles.  Needs a bank and a segment.  syncs. */
 int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma);
 
+/* Physical amplitude / effective distance (templates carry "Newtonian amplitude" and an "effective
+ * distance D_eff from the detector"; the paper prints no constant, reading 4 writes it out):
+ *     h~(f) = A f^(-7/6) e^{i Psi(f)},  A(D_eff) = sqrt(5/24) pi^(-2/3) (c / D_eff) (G M_chirp / c^3)^(5/6),
+ *     M_chirp = (m1 m2)^(3/5) / (m1 + m2)^(1/5).
+ * rho and chi^2 do not depend on A; distances do.  psd_unit is the physical value, in strain^2 / Hz, of ONE unit of
+ * the S_n array given to gwmf_load_segment (9e-46 for Eq. 2 as printed; 1 if S_n was already physical).
+ * host_d1_mpc: HOST array of n_templates doubles, the effective distance in megaparsecs at which template t has optimal
+ * SNR 1 in the loaded PSD: D_1 = A(1 Mpc) sigma / sqrt(psd_unit) (divide by 8 for the usual SNR-8 horizon).
+ * Needs a bank and a segment; GWMF_E_ARG for psd_unit <= 0.  syncs. */
+int gwmf_effective_distance(gwmf_ctx* ctx, double psd_unit, double* host_d1_mpc);
+
+/* Effective distance of events: host_deff_mpc[i] = D_1[template of event i] / rho_i, the distance at which that template
+ * would be seen with the event's SNR.  host_triggers: HOST array of n_triggers events as returned by gwmf_triggers
+ * (template_id inside the loaded bank and rho > 0, else GWMF_E_ARG); host_deff_mpc: HOST array of n_triggers doubles.
+ * syncs. */
+int gwmf_trigger_distances(gwmf_ctx* ctx, double psd_unit, const gwmf_trigger* host_triggers, int64_t n_triggers,
+                           double* host_deff_mpc);
+
 /* Band edges e_0..e_p of every loaded template, HOST array of n_templates*(p+1) int32.  syncs. */
 int gwmf_band_edges(gwmf_ctx* ctx, int32_t* host_edges);
 

@@ -343,6 +343,7 @@ int gwmf_make_bank(gwmf_ctx* ctx, const gwmf_mass_pair* host_masses, int32_t n_t
   }
   CU(cudaStreamSynchronize(c->stream));            // h_meta may still be in flight from a previous call
   memcpy(c->h_meta, fresh.get(), sizeof(TemplateMeta) * (size_t)n_templates);
+  try { c->h_masses.assign(host_masses, host_masses + n_templates); } catch (...) { return GWMF_E_ARG; }
   CU(cudaMemcpyAsync(ws_ptr<TemplateMeta>(c, c->lay.meta), c->h_meta, sizeof(TemplateMeta) * (size_t)n_templates,
                      cudaMemcpyHostToDevice, c->stream));
   c->n_templates = n_templates;
@@ -652,6 +653,48 @@ int gwmf_sigma(gwmf_ctx* ctx, double* host_sigma) {
   int rc = fetch_meta(c, v);
   if (rc != GWMF_OK) return rc;
   for (size_t t = 0; t < v.size(); ++t) host_sigma[t] = v[t].sigma;
+  return GWMF_OK;
+}
+
+// Physical amplitude of template (m1, m2) at 1 Mpc ("Newtonian amplitude", "effective distance"; the constant
+// is SURVEY.md 8(c2) reading 4): sqrt(5/24) pi^(-2/3) (c / 1 Mpc) (T_sun M_chirp)^(5/6), host scalars like fill_template.
+static double amplitude_1mpc(const gwmf_mass_pair& mp) {
+  const double pi = 3.14159265358979323846;
+  const double c_over_mpc = 299792458.0 / 3.0856775814913673e22;              // 1/s
+  const double mt = mp.m1 + mp.m2, eta = mp.m1 * mp.m2 / (mt * mt);
+  const double mchirp_s = GWMF_T_SUN * mt * pow(eta, 0.6);                    // chirp mass in seconds
+  return sqrt(5.0 / 24.0) / cbrt(pi * pi) * c_over_mpc * pow(mchirp_s, 5.0 / 6.0);
+}
+
+int gwmf_effective_distance(gwmf_ctx* ctx, double psd_unit, double* host_d1_mpc) {
+  if (!ctx || !host_d1_mpc || !(psd_unit > 0.0) || !isfinite(psd_unit)) return GWMF_E_ARG;
+  Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
+  std::vector<TemplateMeta> v;
+  int rc = fetch_meta(c, v);
+  if (rc != GWMF_OK) return rc;
+  const double inv_root = 1.0 / sqrt(psd_unit);
+  for (size_t t = 0; t < v.size(); ++t) host_d1_mpc[t] = amplitude_1mpc(c->h_masses[t]) * v[t].sigma * inv_root;
+  return GWMF_OK;
+}
+
+int gwmf_trigger_distances(gwmf_ctx* ctx, double psd_unit, const gwmf_trigger* host_triggers, int64_t n_triggers,
+                           double* host_deff_mpc) {
+  if (!ctx || n_triggers < 0 || (n_triggers > 0 && (!host_triggers || !host_deff_mpc))) return GWMF_E_ARG;
+  if (!(psd_unit > 0.0) || !isfinite(psd_unit)) return GWMF_E_ARG;
+  Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  DeviceGuard guard(c->device);
+  for (int64_t i = 0; i < n_triggers; ++i)
+    if (host_triggers[i].template_id < 0 || host_triggers[i].template_id >= c->n_templates || !(host_triggers[i].rho > 0.f))
+      return GWMF_E_ARG;
+  std::vector<TemplateMeta> v;
+  int rc = fetch_meta(c, v);
+  if (rc != GWMF_OK) return rc;
+  const double inv_root = 1.0 / sqrt(psd_unit);
+  for (int64_t i = 0; i < n_triggers; ++i) {
+    const int t = host_triggers[i].template_id;
+    host_deff_mpc[i] = amplitude_1mpc(c->h_masses[(size_t)t]) * v[(size_t)t].sigma * inv_root / (double)host_triggers[i].rho;
+  }
   return GWMF_OK;
 }
 

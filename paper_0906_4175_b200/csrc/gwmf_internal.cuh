@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "../../include/gwmf.h"
 
@@ -141,6 +142,7 @@ struct Ctx {
   int64_t launches;
   std::string cuda_err;
   TemplateMeta* h_meta;          // host staging of the bank (pinned)
+  std::vector<gwmf_mass_pair> h_masses;   // the loaded bank's masses (gwmf_effective_distance)
   uint32_t* h_masks;             // host mirror of TemplateMeta::wide_mask (pinned), valid once ev_masks has fired
   cudaEvent_t ev_masks;
   // ---- double-buffered segment (s_in, wq): a segment can be uploaded and prepared on the upload stream while the

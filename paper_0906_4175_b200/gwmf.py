@@ -21,7 +21,7 @@ PATH_NAMES = {v: k for k, v in PATHS.items()}
 
 EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
-    "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_band_edges", "gwmf_transform_counts", "gwmf_series", "gwmf_correlate",
+    "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_effective_distance", "gwmf_trigger_distances", "gwmf_band_edges", "gwmf_transform_counts", "gwmf_series", "gwmf_correlate",
     "gwmf_fft_inverse", "gwmf_power_table_static",
     "gwmf_uses_fused", "gwmf_path_in_use", "gwmf_fma_peak", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
@@ -69,6 +69,8 @@ def load_library():
     L.gwmf_triggers.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
     L.gwmf_sigma.argtypes = [C.c_void_p, C.c_void_p]
     L.gwmf_band_edges.argtypes = [C.c_void_p, C.c_void_p]
+    L.gwmf_effective_distance.argtypes = [C.c_void_p, C.c_double, C.c_void_p]
+    L.gwmf_trigger_distances.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_int64, C.c_void_p]
     L.gwmf_transform_counts.argtypes = [C.c_void_p, C.c_void_p]
     L.gwmf_series.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.gwmf_correlate.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
@@ -263,6 +265,20 @@ class Filter:
     def sigma(self) -> np.ndarray:
         out = np.zeros(self.n_templates, dtype=np.float64)
         self._check(self._L.gwmf_sigma(self._h, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def effective_distance(self, psd_unit=9e-46) -> np.ndarray:
+        """Mpc at which each template has optimal SNR 1 in the loaded PSD (psd_unit: strain^2/Hz per unit of S_n)."""
+        out = np.zeros(self.n_templates, dtype=np.float64)
+        self._check(self._L.gwmf_effective_distance(self._h, float(psd_unit), out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def trigger_distances(self, triggers, psd_unit=9e-46) -> np.ndarray:
+        """Effective distance in Mpc of each event of a Filter.triggers() array."""
+        trig = np.ascontiguousarray(triggers, dtype=TRIGGER_DTYPE)
+        out = np.zeros(len(trig), dtype=np.float64)
+        self._check(self._L.gwmf_trigger_distances(self._h, float(psd_unit), trig.ctypes.data_as(C.c_void_p), len(trig),
+                                                   out.ctypes.data_as(C.c_void_p)))
         return out
 
     def band_edges(self) -> np.ndarray:

@@ -701,6 +701,35 @@ def test_rejected_bank_leaves_the_old_bank_intact(gw, path):
     assert np.array_equal(f.sigma(), sig) and np.array_equal(f.band_edges(), edges)
 
 
+def test_effective_distance_matches_oracle(gw):
+    # SURVEY.md 8(f)-4 / PAPER.md:21 (D_eff is one of the template's parameters): the distance at which each template has
+    # optimal SNR 1 in the loaded PSD, D_1 = A(1 Mpc) sigma / sqrt(psd_unit), and D_eff = D_1 / rho of every event,
+    # against the oracle's amplitude (O10) times the oracle's sigma, to 1e-5 relative (sigma's tolerance)
+    w = inputs.workload(1)
+    s = inputs.segment(w).astype(np.float32)
+    f = _run_gpu(gw, w, s, w.psd)
+    unit = 9e-46                                             # Eq. 2 as printed is the design curve / 9e-46
+    C = oracle.power_table(w.psd, w.n)
+    want = np.array([oracle.amplitude(m1, m2, 1.0) * oracle.sigma_edges(C, w.n, oracle.k_high(m1, m2, w.n), w.p)[0]
+                     for m1, m2 in w.masses]) / math.sqrt(unit)
+    d1 = f.effective_distance(unit)
+    assert np.all(np.abs(d1 - want) <= 1e-5 * want)
+    trig = f.triggers()
+    assert len(trig) >= 3
+    deff = f.trigger_distances(trig, unit)
+    ref = want[trig["template_id"]] / trig["rho"].astype(np.float64)
+    assert np.all(np.abs(deff - ref) <= 1e-5 * ref)
+    assert np.allclose(f.effective_distance(1.0), d1 * math.sqrt(unit), rtol=1e-12)      # D_1 ~ 1 / sqrt(psd_unit)
+    with pytest.raises(gw.GwmfError) as e:
+        f.effective_distance(0.0)
+    assert e.value.status == gw.E_ARG
+    bad = trig[:1].copy()
+    bad["template_id"] = len(w.masses)
+    with pytest.raises(gw.GwmfError) as e:
+        f.trigger_distances(bad, unit)
+    assert e.value.status == gw.E_ARG
+
+
 def test_no_triggers_when_threshold_is_high(gw):
     w = inputs.workload(0)
     f = _run_gpu(gw, w, inputs.segment(w), w.psd, thresh=50.0)
