@@ -7,12 +7,17 @@ Contract (driver): `python bench.py --gpus N --steps K --warmup W [--impl refere
               FFTs, rho, chi^2, window maxima, trigger compaction + read-back) over the whole bank of
               BASELINE.json:configs[2] (N = 2^20, 1024 templates, p = 16) against one segment.
   value     = template-segments/s with segment, PSD and bank resident in HBM when the timed region starts.
-  e2e       = the same through the C ABI with HOST buffers: every step uploads the segment and the PSD
-              (gwmf_load_segment from pinned host memory), filters the bank and reads the triggers back.
-  roofline  = the dominant kernel's algorithmic work / its device time (CUDA events recorded by the library
-              on its own stream around every launch, gwmf_filter_timed): for the two-pass path HBM bytes against
-              the measured copy bandwidth in MEASURED_PEAKS.json; for the spill-free kernel (the library's
-              choice at this size: no band intermediate in HBM) flops against the FP32 ALU peak.
+  e2e       = the same through the C ABI with HOST buffers: every step uploads the segment from pinned host memory
+              (gwmf_load_segment with the PSD kept: the PSD is loaded once, before the timed region), filters the bank
+              and reads the events back; the upload overlaps the previous step's filters on the library's upload stream.
+  roofline  = the dominant kernel's algorithmic bytes / its device time (CUDA events recorded by the library on its own
+              stream around the stages of every launch, gwmf_filter_timed) against the measured copy bandwidth in
+              MEASURED_PEAKS.json.  The path that runs is the library's choice at this size, the decimated path:
+              n complex fp32 written by pass 1 and read by pass 2 per n-point transform that is really run (about 1.7
+              per template-segment instead of p = 16).  `--path fused` reports the spill-free kernel against the FP32
+              ALU peak instead.
+  clocks    = SM clock / power / throttle reasons sampled through NVML every 5 ms from the start of the timed region
+              to the end of the e2e region.
   cpu_baseline = the fp64 oracle as it stands, on the host cores, on a bounded sample of the workload.
   N > 1     : one process per GPU; every rank filters the whole bank against its own segment (seed +
               rank): independent units, no data-path collective, weak scaling.
@@ -145,17 +150,60 @@ def reduce_max_ms(ms: float, dist=None, device=None) -> float:
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    """SM clock, power and throttle reasons sampled DURING the timed regions: in-process through NVML every 5 ms (a
+    timed region of a few tens of ms still gets >= 10 samples); `nvidia-smi -lms 100` in a child process if NVML
+    cannot be loaded."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    PERIOD_S = 0.005
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, uuid: str | None = None):
         self.index = index
-        self.rows = []
+        self.uuid = uuid
+        self.rows = []                     # (sm_mhz, power_w, reasons bitmask) or nvidia-smi csv rows
         self.proc = None
+        self.nvml = None
+        self.handle = None
+        self.max_mhz = None
+        self.stop_flag = threading.Event()
+        self.thread = None
+
+    def _nvml_open(self):
+        import pynvml
+        pynvml.nvmlInit()
+        h = None
+        if self.uuid:
+            for cand in (self.uuid, "GPU-" + self.uuid):
+                try:
+                    h = pynvml.nvmlDeviceGetHandleByUUID(cand.encode() if isinstance(cand, str) else cand)
+                    break
+                except Exception:
+                    h = None
+        if h is None:
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+        self.nvml, self.handle = pynvml, h
+        self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+
+    def _nvml_loop(self):
+        nv, h = self.nvml, self.handle
+        reasons_fn = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self.stop_flag.is_set():
+            try:
+                self.rows.append((float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)),
+                                  nv.nvmlDeviceGetPowerUsage(h) / 1e3, int(reasons_fn(h))))
+            except Exception:
+                pass
+            self.stop_flag.wait(self.PERIOD_S)
 
     def start(self):
+        try:
+            self._nvml_open()
+            self.thread = threading.Thread(target=self._nvml_loop, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", "100"],
@@ -170,15 +218,33 @@ class ClockSampler:
             self.rows.append([x.strip() for x in line.split(",")])
 
     def stop(self):
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        if self.nvml is not None:
+            self.stop_flag.set()
+            self.thread.join(timeout=1)
+            nv = self.nvml
+            bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+            sm = [r[0] for r in self.rows]
+            power = [r[1] for r in self.rows]
+            mask = 0
+            for r in self.rows:
+                mask |= r[2]
+            reasons = sorted(nm for nm in names if mask & bits[nm])
+            try:
+                nv.nvmlShutdown()
+            except Exception:
+                pass
+            return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_min_mhz": float(np.min(sm)) if sm else None,
+                    "sm_max_mhz": self.max_mhz, "reasons": reasons, "samples": len(sm),
+                    "power_w": float(np.median(power)) if power else None, "sampler": "NVML in-process, every 5 ms"}
         if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["NVML and nvidia-smi unavailable"], "samples": 0}
         self.proc.terminate()
         try:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
         sm, mx, reasons, power = [], None, set(), []
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in self.rows:
             try:
                 sm.append(float(r[0]))
@@ -190,7 +256,7 @@ class ClockSampler:
             except Exception:
                 continue
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm), "power_w": float(np.median(power)) if power else None}
+                "samples": len(sm), "power_w": float(np.median(power)) if power else None, "sampler": "nvidia-smi -lms 100"}
 
 
 def host_cores() -> int:
@@ -356,7 +422,11 @@ def run_gpu(args):
             out = f.triggers()
         return out
 
-    sampler = ClockSampler(local)
+    try:
+        uuid = str(torch.cuda.get_device_properties(local).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(local, uuid)
     for _ in range(max(args.warmup, 3) if nseg == 1 else max(min(args.warmup, 3), 1)):
         trig = step_resident()
     barrier()
@@ -426,6 +496,8 @@ def run_gpu(args):
     if rank == 0:
         line = base_line(args, w, value, ms / args.steps, "f32")
         line["config"]["path"] = path
+        # SURVEY.md 8(f)-3 / PAPER.md:119,194 compares segment lengths in this unit: one template-segment is n / fs seconds
+        line["template_seconds_of_data_per_s"] = value * w.n / w.fs
         if args.chisq_on_demand:
             line["metric"] += " -- chi^2 ON DEMAND (evaluated at the event samples only; not the headline workload)"
             line["config"]["chisq_mode"] = "on_demand"
@@ -448,6 +520,8 @@ def run_gpu(args):
         line["config"]["shard"] = args.shard
         line["gpu_launches"] = int(launches)
         line["clocks"] = clocks
+        if (clocks.get("samples") or 0) < 10:
+            sys.stderr.write("bench.py: only %s clock samples in the timed regions: raise --steps for a record\n" % clocks.get("samples"))
         line["triggers_per_step"] = int(len(trig))
         kernels = {}
         for i, st in enumerate(STAGES):
@@ -468,13 +542,13 @@ def run_gpu(args):
             # the spill-free kernel moves (almost) no HBM bytes: it is bound by the FP32 pipes and shared memory
             flops_unit = 5.0 * w.n * np.log2(w.n) * w.p            # p * 5 N log2 N per template-segment
             apeak, asrc = alu_peak()
-            measured_alu = gwmf.fma_peak(5, f.stream)            # FFMA2 chains, libgwmf.so's own probe kernel
             tfl = flops_unit * count / (k_ms[2] * 1e-3) / 1e12
             tr, tr_src = traffic_record(path, args.workload, "pass2")
             line["roofline"] = {
                 "bound": "alu", "kernel": STAGE_TEXT[path]["pass2"], "achieved": float(tfl), "peak": apeak, "unit": "TFLOP/s",
-                "frac": float(tfl / apeak), "peak_source": asrc, "peak_measured": measured_alu,
-                "frac_of_measured": float(tfl / measured_alu), "peak_measured_source": "gwmf_fma_peak: packed fma.rn.f32x2 chains",
+                "frac": float(tfl / apeak), "peak_source": asrc,
+                "peak_note": "a round-2 probe of packed fma.rn.f32x2 chains measured 68.1 TFLOP/s on this pool "
+                             "(profiles/r2_fp32_peak.json); the probe is no longer part of the library",
                 "flops": "dense-FFT equivalent (p*5N*log2N per unit), not executed flops",
                 "traffic": tr * count / k_launch[2] if tr else None, "traffic_source": tr_src,
                 "avg_launch_ms": float(k_ms[2] / k_launch[2]), "kernels": kernels, "hbm_model_equivalent": hbm_model}
@@ -526,17 +600,10 @@ def main():
     ap.add_argument("--chisq-on-demand", action="store_true",
                     help="gwmf_params::chisq_mode = ON_DEMAND: one full-band transform per template, chi^2 evaluated only at "
                          "the event samples (SURVEY.md 8(f)-2; a different workload from the headline's chi^2(t) at every sample)")
-    ap.add_argument("--peak", action="store_true", help="print the measured FP32 (packed FFMA2) peak of the device and exit")
     ap.add_argument("--shard", default="segments", choices=["segments", "templates"],
                     help="N > 1: segments = every rank filters the whole bank against its own segment (weak scaling); "
                          "templates = one segment, the bank split by template id, events gathered (strong scaling)")
     args = ap.parse_args()
-    if args.peak:
-        from paper_0906_4175_b200 import gwmf
-        derived, src = alu_peak()
-        print(json.dumps({"fp32_peak_tflops_measured": gwmf.fma_peak(10), "how": "gwmf_fma_peak: packed fma.rn.f32x2 chains, best of 10",
-                          "fp32_peak_tflops_derived": derived, "derived_from": src}))
-        return 0
     if args.impl == "reference":
         return run_reference(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

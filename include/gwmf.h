@@ -224,11 +224,6 @@ int gwmf_uses_fused(const gwmf_ctx* ctx);
 /* The gwmf_path this context filters with (GWMF_PATH_AUTO resolved at gwmf_create); GWMF_E_ARG for a null ctx. */
 int gwmf_path_in_use(const gwmf_ctx* ctx);
 
-/* Measurement: FP32 (non-tensor) peak of the current device in TFLOP/s, measured with chains of packed
- * fma.rn.f32x2 -- the instruction the hot kernels' butterflies are made of -- on the given stream (a cudaStream_t;
- * NULL = default stream); best of `repeats` >= 1 timed launches after one warm-up.  Needs no context.  syncs. */
-int gwmf_fma_peak(void* cuda_stream, int32_t repeats, double* host_tflops);
-
 /* The power table of Eq. 4 without a context, a workspace or any allocation:
  *     C[k] = sum_{k' <= k} f_k'^(-7/3) / S_n[k']   over k_low = ceil(f_low n / fs) <= k' <= k,   C[k] = 0 below k_low,
  * from which sigma^2 = 4 (fs/n) C[k_high - 1] and the p + 1 equal-power band edges of any template follow

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgwmf.so")
-SOURCES = ["api.cu", "segment.cu", "pass1.cu", "pass2.cu", "bandpower.cu", "triggers.cu", "probe.cu", "static_scratch.cu"]
+SOURCES = ["api.cu", "segment.cu", "pass1.cu", "pass2.cu", "bandpower.cu", "triggers.cu", "static_scratch.cu"]
 HEADERS = ["gwmf_internal.cuh", "fft_reg.cuh", os.path.join("..", "..", "include", "gwmf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

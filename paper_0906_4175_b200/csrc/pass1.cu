@@ -395,7 +395,8 @@ struct EffSrc {
 // makes the column writes of phase 1, the row reads / writes of phase 2 (16 bytes per lane) and the bulk copy's linear
 // read all conflict-free.  The tile reaches the band buffer as it is (pass 2 undoes the swizzle when it reads).
 constexpr int kWTile = 32 * 32;                   // float2 per warp (8 KB)
-// Measured on B200 (headline config): 4 warps x 4 CTAs per SM at 128 registers (no spills) beats 8 x 3 at 80 registers
+// Measured on B200 (headline config): 4 warps x 4 CTAs per SM at 128 registers (ptxas: 28 B spill stores, 36 B spill
+// loads per thread) beats 8 x 3 at 80 registers
 // (spills in the round loop) by 20 %; 2..8 ja per CTA are within 2 % of each other, 1 and 32 are worse.
 constexpr int kP1Warps = 4;                       // warps (values of c) per CTA of k_pass1_eff
 constexpr int kP1CtasPerSm = 4;

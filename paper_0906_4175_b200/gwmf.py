@@ -23,7 +23,7 @@ EXPORTS = [
     "gwmf_workspace_bytes", "gwmf_create", "gwmf_make_bank", "gwmf_load_segment", "gwmf_filter",
     "gwmf_filter_timed", "gwmf_triggers", "gwmf_sigma", "gwmf_effective_distance", "gwmf_trigger_distances", "gwmf_band_edges", "gwmf_transform_counts", "gwmf_series", "gwmf_correlate",
     "gwmf_fft_inverse", "gwmf_power_table_static",
-    "gwmf_uses_fused", "gwmf_path_in_use", "gwmf_fma_peak", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
+    "gwmf_uses_fused", "gwmf_path_in_use", "gwmf_launch_count", "gwmf_destroy", "gwmf_strerror", "gwmf_last_cuda_error",
 ]
 
 
@@ -79,7 +79,6 @@ def load_library():
                                           C.c_char_p, C.c_size_t]
     L.gwmf_uses_fused.argtypes = [C.c_void_p]
     L.gwmf_path_in_use.argtypes = [C.c_void_p]
-    L.gwmf_fma_peak.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
     L.gwmf_launch_count.argtypes = [C.c_void_p]
     L.gwmf_launch_count.restype = C.c_int64
     L.gwmf_destroy.argtypes = [C.c_void_p]
@@ -97,15 +96,6 @@ def workspace_bytes(n, p, window, max_templates, fs=4096.0, f_low=40.0, rho_thre
     prm = Params(int(n), float(fs), float(f_low), int(p), float(rho_thresh), int(window), int(max_templates), int(batch),
                  PATHS[path], 1 if chisq_on_demand else 0)
     return int(load_library().gwmf_workspace_bytes(C.byref(prm)))
-
-
-def fma_peak(repeats=5, stream=None) -> float:
-    """Measured FP32 (packed FFMA2) peak of the current CUDA device in TFLOP/s (gwmf_fma_peak)."""
-    out = C.c_double(0.0)
-    rc = load_library().gwmf_fma_peak(C.c_void_p(stream.cuda_stream if stream is not None else None), int(repeats), C.byref(out))
-    if rc != OK:
-        raise GwmfError(rc, load_library().gwmf_strerror(rc).decode())
-    return out.value
 
 
 STATIC_MAX_N = 1 << 22            # GWMF_STATIC_MAX_N
